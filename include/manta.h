@@ -1,0 +1,160 @@
+/*
+ * manta.h -- C ABI of the B200-native MANTA vehicle-update hot path (libmanta.so).
+ *
+ * What the library computes: the per-timestep (dt = 0.5 s) update of every active vehicle of a
+ * metropolitan traffic microsimulation over the "traffic atlas": leader look-ahead, IDM car
+ * following (Eq. 1), lane change with gap acceptance (Eq. 2-4), integration, edge /
+ * intersection transfer along precomputed routes, departure release, and
+ * the per-edge counts / travel times the paper reports.  The exact rules (R0-R9) and the
+ * readings taken where the paper is silent are in DESIGN.md sections 2-3.  Routing and initialisation are outside
+ * the timed path: manta_create / manta_load_trips are initialisation, manta_step is the hot path.
+ *
+ * Conventions
+ *   - Every pointer argument is a HOST pointer unless its name ends in _dev.  Input arrays are copied during the
+ *     call; the caller may free them on return.  Output arrays are caller-allocated.
+ *   - Every call returns 0 (MANTA_OK) or a negative MANTA_ERR_* code; no exceptions, no abort.  After an error
+ *     manta_last_error() gives a text; a failed call leaves the simulation state as it was (manta_step excepted:
+ *     a CUDA fault is sticky and every later call returns MANTA_ERR_CUDA).
+ *   - All kernels run on one CUDA device and on the stream given by manta_set_stream (default: the legacy
+ *     default stream).  Device memory comes from cudaMalloc unless manta_set_allocator installed callbacks
+ *     (the Python binding hands out PyTorch caching-allocator blocks that way).
+ *   - There is no CPU fallback: without a CUDA device manta_create returns MANTA_ERR_CUDA.
+ */
+#ifndef MANTA_H
+#define MANTA_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MANTA_OK 0
+#define MANTA_ERR_INVALID_ARG (-1)
+#define MANTA_ERR_BAD_NETWORK (-2)
+#define MANTA_ERR_BAD_ROUTE (-3)
+#define MANTA_ERR_OOM (-4)
+#define MANTA_ERR_CUDA (-5)
+#define MANTA_ERR_STATE (-6)
+
+#define MANTA_GREEN 0    /* case 2: every vehicle passes; conflicts per (edge, lane) entry  */
+#define MANTA_PRIORITY 1 /* case 1 exclusivity: one vehicle per node per step, smallest vehicle id first */
+
+#define MANTA_WAITING 0
+#define MANTA_ACTIVE 1
+#define MANTA_DONE 2
+
+#define MANTA_NONE 0xFFFFFFFFu
+#define MANTA_MAX_LANES 8
+#define MANTA_MAX_EDGE_CELLS 65535u
+
+/* manta_params.flags */
+#define MANTA_FLAG_SCALAR_SCAN 1u      /* per-thread look-ahead instead of the warp-cooperative scan (A/B evidence) */
+#define MANTA_FLAG_MULTI_KERNEL 2u     /* three launches per step instead of the persistent cooperative kernel */
+#define MANTA_FLAG_RECORD_ACC 4u       /* keep each vehicle's last acceleration for manta_state.acc (tests)  */
+
+typedef struct manta_sim manta_sim; /* opaque; owned by the library; one simulation on one device */
+
+/* Street network (per edge lanes, length in metres, free-flow speed).  Edges are numbered in
+ * CSR order by TAIL node: edges row_ptr[u] .. row_ptr[u+1]-1 leave node u. */
+typedef struct {
+    uint32_t n_nodes, n_edges;
+    const uint32_t *row_ptr;     /* [n_nodes+1]                                                         */
+    const uint32_t *head;        /* [n_edges]  head node of each edge                                   */
+    const float *length_m;       /* [n_edges]  > 0; rounded to whole 1 m cells; >= LEN_MIN (R0) */
+    const uint8_t *lanes;        /* [n_edges]  1..8                                                     */
+    const float *speed_limit;    /* [n_edges]  m/s, > 0; used as IDM v0                   */
+    const uint8_t *node_ctrl;    /* [n_nodes] MANTA_GREEN / MANTA_PRIORITY, or NULL = all GREEN         */
+} manta_network;
+
+/* Model parameters; one set shared by all vehicles.  delta of Eq. 1 is fixed at 4. */
+typedef struct {
+    uint32_t size;             /* = sizeof(manta_params): versioning                                     */
+    float dt;                  /* timestep, s                                                            */
+    float a, b, T, s0;         /* IDM: acceleration, braking, headway, standstill gap (Eq. 1, Table I)   */
+    float veh_len;             /* vehicle length L, m                                                    */
+    uint32_t lookahead_cells;  /* H of R2                                                                */
+    uint32_t lookback_cells;   /* lag search range of R5; must be >= ceil(L) + Z_out                     */
+    float mlc_scale_m;         /* Lambda: unit of x_i, x_0 in Eq. 2 (reading G6)                         */
+    float dlc_gain_thr;        /* discretionary gain threshold, m/s^2 (reading G9)                       */
+    float lc_alpha;            /* anticipation time alpha, s (Eq. 3, 4)                                  */
+    float lc_gap_low;          /* desired gap below 25 mph, m                             */
+    float lc_gap_high;         /* desired gap above 25 mph, m                                            */
+    float lc_eps_sigma;        /* standard deviation of epsilon, m (Eq. 3, 4)                            */
+    uint64_t seed;             /* counter-based generator seed (G22)                                     */
+    uint32_t flags;            /* MANTA_FLAG_*                                                           */
+} manta_params;
+
+/* Per-trip state snapshot, indexed by the CALLER's trip index.  Any member may be NULL (skipped). */
+typedef struct {
+    uint8_t *status;           /* MANTA_WAITING / ACTIVE / DONE                                          */
+    uint32_t *route_pos;       /* index into the trip's route (ACTIVE only, else 0)                      */
+    uint8_t *lane;             /* ACTIVE only                                                            */
+    uint8_t *tag;              /* mandatory-lane-change tag of Eq. 2 (ACTIVE only)                       */
+    uint32_t *x_fx;            /* position on the edge, Q22.10 metres (ACTIVE only)                      */
+    float *v;                  /* speed m/s (ACTIVE only)                                                */
+    float *acc;                /* acceleration applied in the last step (ACTIVE only)                    */
+} manta_state;
+
+typedef struct {
+    uint32_t admit_step;       /* step at which the trip entered the network, MANTA_NONE if still waiting */
+    uint32_t arrive_step;      /* step count at arrival (travel steps = arrive - admit), MANTA_NONE if not done */
+} manta_trip_result;
+
+typedef struct {
+    uint64_t t;                /* steps simulated so far                                                 */
+    uint64_t n_waiting, n_active, n_done;
+    uint64_t sum_travel_steps; /* sum over DONE trips of arrive_step - admit_step                        */
+    uint64_t vehicle_updates;  /* ACTIVE vehicles processed by the update, summed over steps (the metric's unit) */
+    uint64_t lane_changes;     /* executed lane changes                                                  */
+    uint64_t cells_examined;   /* atlas cells examined by the own-lane look-ahead (R2), summed           */
+    uint64_t lc_evals;         /* updates that evaluated the adjacent lane (R5)                          */
+} manta_summary;
+
+/* Optional device-memory callbacks (process-wide; install before manta_create).  alloc returns a device pointer
+ * valid on `device` or NULL; free receives that pointer.  NULL, NULL restores cudaMalloc / cudaFree. */
+typedef void *(*manta_alloc_fn)(uint64_t bytes, int device, void *ctx);
+typedef void (*manta_free_fn)(void *ptr_dev, int device, void *ctx);
+int manta_set_allocator(manta_alloc_fn alloc, manta_free_fn free_, void *ctx);
+
+/* Builds the atlas (one row of 1 m cells per (edge, lane)) and the static tables of R0 on
+ * `cuda_device`.  Errors: INVALID_ARG (NULL, params->size mismatch, non-positive dt/a/b/...), BAD_NETWORK (lanes
+ * outside 1..8, length < LEN_MIN or > 65535 cells, non-finite values, head out of range, out-degree > 255,
+ * more than 2^32 - 1 atlas cells), OOM, CUDA. */
+int manta_create(const manta_network *net, const manta_params *params, int cuda_device, manta_sim **out);
+
+/* Loads the demand: trip i follows route_edges[route_ptr[i] .. route_ptr[i+1]-1] ("routes are
+ * fixed") and is released at depart_time_s[i].  init_pos_m / init_speed may be NULL; a trip with
+ * init_pos_m[i] >= 0 is pre-placed at that position on its first edge, lane 0, with speed init_speed[i], active from
+ * step 0 (R1).  Vehicle ids are ranks in the stable (depart_step, trip index) order.  May be called once per
+ * simulation.  Errors: BAD_ROUTE (empty route, edge id out of range, head(e_k) != tail(e_k+1), negative departure,
+ * negative / non-finite init_speed, pre-placed vehicles closer than L in one row or beyond the edge), INVALID_ARG
+ * (lookback_cells too small for R5), STATE (already loaded), OOM, CUDA. */
+int manta_load_trips(manta_sim *sim, uint32_t n_trips, const uint64_t *route_ptr, const uint32_t *route_edges,
+                     const float *depart_time_s, const float *init_pos_m, const float *init_speed);
+
+/* THE HOT PATH.  Advances the simulation by n_steps timesteps (rules R1-R9) and returns when they completed.
+ * manta_step_async only enqueues the work on the simulation's stream; manta_sync waits for it. */
+int manta_step(manta_sim *sim, uint32_t n_steps);
+int manta_step_async(manta_sim *sim, uint32_t n_steps);
+int manta_sync(manta_sim *sim);
+
+/* Copies results to host buffers (each may be NULL): per-trip state, cumulative per-edge entry counts
+ * ([n_edges]), per-trip admit/arrive steps ([n_trips]), and the summary counters. */
+int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,
+                   manta_summary *summary);
+
+/* Logical atlas of the current step for tests: occ[i] = 0 (empty) or 1 + frac10 per padded cell, spd[i] the
+ * occupant's speed; row (e, lane) starts at cell_off[e] + lane * pitch[e].  Sizes via manta_atlas_cells. */
+uint64_t manta_atlas_cells(const manta_sim *sim);
+int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch);
+
+int manta_set_stream(manta_sim *sim, void *cuda_stream);   /* cudaStream_t; work already enqueued is not moved */
+uint64_t manta_launch_count(const manta_sim *sim);         /* kernels launched by this simulation so far   */
+uint64_t manta_device_bytes(const manta_sim *sim);         /* device memory held                           */
+void manta_destroy(manta_sim *sim);
+const char *manta_last_error(const manta_sim *sim);        /* sim may be NULL: error of the last failed create */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

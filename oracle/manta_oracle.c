@@ -151,6 +151,7 @@ static void derive_constants(mo_sim *S, double max_init_speed)
     S->Z_out = (uint32_t)ceil(vcap * (double)p->dt) + 1u;
     S->Z_in = S->L_c + S->Z_out;
     S->LEN_MIN = S->Z_out + 1u;
+    if (S->LEN_MIN < S->L_c + 1u) S->LEN_MIN = S->L_c + 1u; /* R1 reads cells [0, L_c] of a row */
 }
 
 mo_sim *mo_create(uint32_t n_nodes, uint32_t n_edges, const uint32_t *row_ptr, const uint32_t *head,

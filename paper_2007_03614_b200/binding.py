@@ -1,0 +1,227 @@
+"""Thin ctypes binding of libmanta.so (include/manta.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for plumbing: device memory
+(the library's allocator callbacks hand out torch caching-allocator blocks) and the CUDA stream.  There is no
+CPU fallback: loading fails loudly if the library is missing, and Sim() fails if no CUDA device is present.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmanta.so")
+
+OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
+GREEN, PRIORITY = 0, 1
+WAITING, ACTIVE, DONE = 0, 1, 2
+NONE = 0xFFFFFFFF
+FLAG_SCALAR_SCAN, FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 1, 2, 4
+
+EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
+           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_launch_count",
+           "manta_device_bytes", "manta_destroy", "manta_last_error")
+
+
+class MantaError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("manta error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Network(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint32), ("n_edges", C.c_uint32), ("row_ptr", C.c_void_p), ("head", C.c_void_p),
+                ("length_m", C.c_void_p), ("lanes", C.c_void_p), ("speed_limit", C.c_void_p),
+                ("node_ctrl", C.c_void_p)]
+
+
+class Params(C.Structure):
+    _fields_ = [("size", C.c_uint32), ("dt", C.c_float), ("a", C.c_float), ("b", C.c_float), ("T", C.c_float),
+                ("s0", C.c_float), ("veh_len", C.c_float), ("lookahead_cells", C.c_uint32),
+                ("lookback_cells", C.c_uint32), ("mlc_scale_m", C.c_float), ("dlc_gain_thr", C.c_float),
+                ("lc_alpha", C.c_float), ("lc_gap_low", C.c_float), ("lc_gap_high", C.c_float),
+                ("lc_eps_sigma", C.c_float), ("seed", C.c_uint64), ("flags", C.c_uint32)]
+
+
+class State(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc")]
+
+
+class Summary(C.Structure):
+    _fields_ = [(k, C.c_uint64) for k in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps",
+                                          "vehicle_updates", "lane_changes", "cells_examined", "lc_evals")]
+
+
+DEFAULT_PARAMS = dict(dt=0.5, a=1.0, b=2.0, T=1.5, s0=2.0, veh_len=5.0, lookahead_cells=128, lookback_cells=64,
+                      mlc_scale_m=100.0, dlc_gain_thr=0.2, lc_alpha=0.2, lc_gap_low=3.0, lc_gap_high=7.5,
+                      lc_eps_sigma=1.0, seed=20070361, flags=0)
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_int, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.c_void_p)
+
+_lib = None
+_blocks = {}
+_cb = None
+
+
+def load_library():
+    """dlopen libmanta.so and declare the prototypes.  Raises if the CUDA library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libmanta.so is missing: run `python -m paper_2007_03614_b200.build` (nvcc, sm_100a). "
+                          "There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    L.manta_set_allocator.argtypes = [ALLOC_FN, FREE_FN, C.c_void_p]
+    L.manta_create.argtypes = [C.POINTER(Network), C.POINTER(Params), C.c_int, C.POINTER(C.c_void_p)]
+    L.manta_load_trips.argtypes = [C.c_void_p, C.c_uint32] + [C.c_void_p] * 5
+    for f in ("manta_step", "manta_step_async"):
+        getattr(L, f).argtypes = [C.c_void_p, C.c_uint32]
+    L.manta_sync.argtypes = [C.c_void_p]
+    L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
+    L.manta_atlas_cells.argtypes = [C.c_void_p]
+    L.manta_atlas_cells.restype = C.c_uint64
+    L.manta_readback_atlas.argtypes = [C.c_void_p] * 5
+    L.manta_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    L.manta_launch_count.argtypes = [C.c_void_p]
+    L.manta_launch_count.restype = C.c_uint64
+    L.manta_device_bytes.argtypes = [C.c_void_p]
+    L.manta_device_bytes.restype = C.c_uint64
+    L.manta_destroy.argtypes = [C.c_void_p]
+    L.manta_destroy.restype = None
+    L.manta_last_error.argtypes = [C.c_void_p]
+    L.manta_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def use_torch_allocator():
+    """Route the library's device allocations through PyTorch's caching allocator."""
+    global _cb
+    import torch
+    L = load_library()
+
+    def _alloc(nbytes, device, _ctx):
+        try:
+            t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
+        except Exception:
+            return None
+        _blocks[t.data_ptr()] = t
+        return t.data_ptr()
+
+    def _free(ptr, _device, _ctx):
+        _blocks.pop(ptr, None)
+
+    _cb = (ALLOC_FN(_alloc), FREE_FN(_free))
+    L.manta_set_allocator(_cb[0], _cb[1], None)
+
+
+def _ptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+class Sim:
+    """One simulation on one GPU: manta_create + manta_load_trips + manta_step + manta_readback."""
+
+    def __init__(self, net, params=None, trips=None, device=0, torch_alloc=True, stream=None):
+        L = load_library()
+        if torch_alloc and _cb is None:
+            use_torch_allocator()
+        pd = dict(DEFAULT_PARAMS)
+        pd.update(params or {})
+        self.params = pd
+        P = Params(size=C.sizeof(Params), **pd)
+        self._net_arrays = [np.ascontiguousarray(net["row_ptr"], np.uint32), np.ascontiguousarray(net["head"], np.uint32),
+                            np.ascontiguousarray(net["length_m"], np.float32), np.ascontiguousarray(net["lanes"], np.uint8),
+                            np.ascontiguousarray(net["speed_limit"], np.float32),
+                            None if net.get("node_ctrl") is None else np.ascontiguousarray(net["node_ctrl"], np.uint8)]
+        N = Network(int(net["n_nodes"]), int(net["n_edges"]), *[_ptr(a) for a in self._net_arrays])
+        self.n_edges = int(net["n_edges"])
+        self.h = C.c_void_p()
+        rc = L.manta_create(C.byref(N), C.byref(P), int(device), C.byref(self.h))
+        if rc != OK:
+            self.h = None
+            raise MantaError(rc, L.manta_last_error(None).decode())
+        self.n_trips = 0
+        if stream is not None:
+            self.set_stream(stream)
+        if trips is not None:
+            self.load_trips(trips)
+
+    def _check(self, rc):
+        if rc != OK:
+            raise MantaError(rc, load_library().manta_last_error(self.h).decode())
+
+    def set_stream(self, stream):
+        """stream: torch.cuda.Stream or a raw cudaStream_t integer."""
+        self._stream = stream
+        handle = getattr(stream, "cuda_stream", stream)
+        self._check(load_library().manta_set_stream(self.h, C.c_void_p(int(handle))))
+
+    def load_trips(self, trips):
+        rp = np.ascontiguousarray(trips["route_ptr"], np.uint64)
+        re_ = np.ascontiguousarray(trips["route_edges"], np.uint32)
+        dep = np.ascontiguousarray(trips["depart_time_s"], np.float32)
+        ip, iv = trips.get("init_pos_m"), trips.get("init_speed")
+        ip = None if ip is None else np.ascontiguousarray(ip, np.float32)
+        iv = None if iv is None else np.ascontiguousarray(iv, np.float32)
+        self._check(load_library().manta_load_trips(self.h, len(dep), _ptr(rp), _ptr(re_), _ptr(dep), _ptr(ip), _ptr(iv)))
+        self.n_trips = len(dep)
+
+    def step(self, n=1):
+        self._check(load_library().manta_step(self.h, int(n)))
+
+    def step_async(self, n=1):
+        self._check(load_library().manta_step_async(self.h, int(n)))
+
+    def sync(self):
+        self._check(load_library().manta_sync(self.h))
+
+    def readback(self, state=True, edge_entries=True, trips=True, summary=True):
+        n = self.n_trips
+        out = {}
+        S = None
+        if state:
+            out.update(status=np.zeros(n, np.uint8), route_pos=np.zeros(n, np.uint32), lane=np.zeros(n, np.uint8),
+                       tag=np.zeros(n, np.uint8), x_fx=np.zeros(n, np.uint32), v=np.zeros(n, np.float32),
+                       acc=np.zeros(n, np.float32))
+            S = State(*[_ptr(out[k]) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc")])
+        ee = np.zeros(self.n_edges, np.uint32) if edge_entries else None
+        tr = np.zeros((n, 2), np.uint32) if trips else None
+        sm = Summary() if summary else None
+        self._check(load_library().manta_readback(self.h, None if S is None else C.byref(S), _ptr(ee), _ptr(tr),
+                                                  None if sm is None else C.byref(sm)))
+        if trips:
+            out["admit_step"], out["arrive_step"] = tr[:, 0].copy(), tr[:, 1].copy()
+        if edge_entries:
+            out["edge_entries"] = ee
+        if summary:
+            out["summary"] = {k: int(getattr(sm, k)) for k, _ in Summary._fields_}
+        return out
+
+    def readback_atlas(self):
+        n = int(load_library().manta_atlas_cells(self.h))
+        occ, spd = np.zeros(n, np.uint16), np.zeros(n, np.float32)
+        off, pitch = np.zeros(self.n_edges, np.uint32), np.zeros(self.n_edges, np.uint32)
+        self._check(load_library().manta_readback_atlas(self.h, _ptr(occ), _ptr(spd), _ptr(off), _ptr(pitch)))
+        return dict(occ=occ, spd=spd, cell_off=off, pitch=pitch)
+
+    @property
+    def launch_count(self):
+        return int(load_library().manta_launch_count(self.h))
+
+    @property
+    def device_bytes(self):
+        return int(load_library().manta_device_bytes(self.h))
+
+    def close(self):
+        if getattr(self, "h", None):
+            load_library().manta_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

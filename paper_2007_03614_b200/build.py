@@ -1,0 +1,55 @@
+"""Build steps of the package: libmanta.so (nvcc, sm_100a) and libmanta_workloads.so (gcc).
+
+Deterministic mode: -fmad=false, IEEE division and square root (nvcc defaults
+-prec-div=true -prec-sqrt=true, stated explicitly), no fast-math.
+"""
+import os
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_HERE)
+CSRC = os.path.join(_HERE, "csrc")
+LIB = os.path.join(_HERE, "libmanta.so")
+SOURCES = [os.path.join(CSRC, "manta_api.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, "manta_kernels.cuh"), os.path.join(CSRC, "manta_device.cuh"),
+                  os.path.join(_ROOT, "include", "manta.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
+              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+
+
+def nvcc():
+    for c in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if c and (os.path.isabs(c) and os.path.exists(c) or not os.path.isabs(c)):
+            return c
+    raise RuntimeError("nvcc not found")
+
+
+def build_cuda(force=False, verbose=False):
+    if (not force and os.path.exists(LIB)
+            and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in DEPS)):
+        return LIB
+    cmd = [nvcc()] + NVCC_FLAGS + ["-o", LIB] + SOURCES + ["-lcudart"]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed")
+    with open(os.path.join(_HERE, "libmanta.ptxas.txt"), "w") as f:
+        f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return LIB
+
+
+def build_all(force=False, verbose=False):
+    from . import workloads
+    workloads.build_routing(force)
+    return build_cuda(force, verbose)
+
+
+if __name__ == "__main__":
+    sys.path.insert(0, _ROOT)
+    from paper_2007_03614_b200 import workloads as _w
+    _w.build_routing("--force" in sys.argv)
+    build_cuda("--force" in sys.argv, verbose=True)
+    print(LIB)

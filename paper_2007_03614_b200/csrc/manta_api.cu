@@ -1,0 +1,564 @@
+// manta_api.cu -- host side of libmanta.so: the C ABI of include/manta.h.
+// Initialisation (manta_create, manta_load_trips) validates, lays out the atlas / route store / queues and uploads;
+// manta_step only enqueues kernels.  No simulator arithmetic runs on the host.
+#include "../../include/manta.h"
+#include "manta_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+using namespace manta;
+
+namespace {
+
+manta_alloc_fn g_alloc = nullptr;
+manta_free_fn g_free = nullptr;
+void *g_alloc_ctx = nullptr;
+thread_local std::string g_last_error;
+
+struct Alloc {
+    void *p;
+    uint64_t bytes;
+};
+
+}  // namespace
+
+struct manta_sim {
+    int device = 0;
+    cudaStream_t stream = 0;
+    manta_params prm{};
+    DevP P{};
+    std::string err;
+    bool sticky_cuda = false;
+    std::vector<Alloc> allocs;
+    uint64_t dev_bytes = 0, launches = 0;
+    // host copies of the network
+    uint32_t n_nodes = 0, n_edges = 0;
+    std::vector<uint32_t> row_ptr, head, tail, len_c, cell_off;
+    std::vector<uint8_t> lanes;
+    double max_limit = 0.0;
+    uint64_t n_cells = 0;
+    // trips
+    uint32_t n_trips = 0;
+    bool loaded = false;
+    uint32_t *d_trip_of_id = nullptr;
+    uint32_t t = 0;
+    int sm_count = 148;
+    int grid_update = 1, grid_admit = 1;
+    uint32_t n_blk_stats = 0;
+};
+
+namespace {
+
+int fail(manta_sim *s, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    if (s) s->err = buf;
+    return code;
+}
+
+#define CUDA_TRY(s, expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e_ = (expr);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            if (s) (s)->sticky_cuda = true;                                                        \
+            return fail(s, e_ == cudaErrorMemoryAllocation ? MANTA_ERR_OOM : MANTA_ERR_CUDA,       \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                                  \
+        }                                                                                          \
+    } while (0)
+
+void *dev_alloc(manta_sim *s, uint64_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    void *p = nullptr;
+    if (g_alloc)
+        p = g_alloc(bytes, s->device, g_alloc_ctx);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        p = nullptr;
+    }
+    if (p) {
+        s->allocs.push_back({p, bytes});
+        s->dev_bytes += bytes;
+    }
+    return p;
+}
+void dev_free(manta_sim *s, void *p)
+{
+    for (size_t i = 0; i < s->allocs.size(); i++)
+        if (s->allocs[i].p == p) {
+            s->dev_bytes -= s->allocs[i].bytes;
+            s->allocs.erase(s->allocs.begin() + (long)i);
+            break;
+        }
+    if (g_free)
+        g_free(p, s->device, g_alloc_ctx);
+    else if (!g_alloc)
+        cudaFree(p);
+}
+
+template <class T>
+int upload(manta_sim *s, T **dst, const T *src, uint64_t n)
+{
+    *dst = (T *)dev_alloc(s, n * sizeof(T));
+    if (!*dst) return fail(s, MANTA_ERR_OOM, "device allocation of %llu bytes failed", (unsigned long long)(n * sizeof(T)));
+    if (n) CUDA_TRY(s, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, s->stream));
+    return MANTA_OK;
+}
+template <class T>
+int alloc_fill(manta_sim *s, T **dst, uint64_t n, int byte)
+{
+    *dst = (T *)dev_alloc(s, n * sizeof(T));
+    if (!*dst) return fail(s, MANTA_ERR_OOM, "device allocation of %llu bytes failed", (unsigned long long)(n * sizeof(T)));
+    CUDA_TRY(s, cudaMemsetAsync(*dst, byte, std::max<uint64_t>(n * sizeof(T), 1), s->stream));
+    return MANTA_OK;
+}
+
+// R0 constants that depend on the fastest possible vehicle
+void derive_constants(manta_sim *s, double max_init_speed)
+{
+    const manta_params &p = s->prm;
+    const double vcap = std::max(s->max_limit, max_init_speed) + (double)p.a * (double)p.dt;
+    s->P.L_c = (uint32_t)std::ceil((double)p.veh_len);
+    s->P.L_fx = (int32_t)std::lround((double)p.veh_len * 1024.0);
+    s->P.Z_out = (uint32_t)std::ceil(vcap * (double)p.dt) + 1u;
+    s->P.Z_in = s->P.L_c + s->P.Z_out;
+}
+uint32_t len_min(const manta_sim *s) { return std::max(s->P.Z_out + 1u, s->P.L_c + 1u); }
+
+}  // namespace
+
+extern "C" {
+
+int manta_set_allocator(manta_alloc_fn alloc, manta_free_fn free_, void *ctx)
+{
+    if ((alloc == nullptr) != (free_ == nullptr)) return fail(nullptr, MANTA_ERR_INVALID_ARG, "allocator needs both callbacks");
+    g_alloc = alloc;
+    g_free = free_;
+    g_alloc_ctx = ctx;
+    return MANTA_OK;
+}
+
+const char *manta_last_error(const manta_sim *sim) { return sim ? sim->err.c_str() : g_last_error.c_str(); }
+uint64_t manta_launch_count(const manta_sim *sim) { return sim ? sim->launches : 0; }
+uint64_t manta_device_bytes(const manta_sim *sim) { return sim ? sim->dev_bytes : 0; }
+uint64_t manta_atlas_cells(const manta_sim *sim) { return sim ? sim->n_cells : 0; }
+
+void manta_destroy(manta_sim *sim)
+{
+    if (!sim) return;
+    cudaSetDevice(sim->device);
+    cudaStreamSynchronize(sim->stream);
+    while (!sim->allocs.empty()) dev_free(sim, sim->allocs.back().p);
+    delete sim;
+}
+
+int manta_set_stream(manta_sim *sim, void *cuda_stream)
+{
+    if (!sim) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    sim->stream = (cudaStream_t)cuda_stream;
+    return MANTA_OK;
+}
+
+int manta_create(const manta_network *net, const manta_params *prm, int cuda_device, manta_sim **out)
+{
+    if (!net || !prm || !out) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (prm->size != sizeof(manta_params)) return fail(nullptr, MANTA_ERR_INVALID_ARG, "manta_params.size mismatch");
+    if (!net->row_ptr || !net->head || !net->length_m || !net->lanes || !net->speed_limit || net->n_nodes == 0 ||
+        net->n_edges == 0)
+        return fail(nullptr, MANTA_ERR_INVALID_ARG, "network arrays missing");
+    const manta_params &p = *prm;
+    if (!(p.dt > 0.f) || !(p.a > 0.f) || !(p.b > 0.f) || !(p.T >= 0.f) || !(p.s0 >= 0.f) || !(p.veh_len > 0.f) ||
+        p.lookahead_cells < 1 || p.lookahead_cells > 8192 || p.lookback_cells < 1 || p.lookback_cells > 8192 ||
+        !(p.mlc_scale_m >= 1.f) || !(p.mlc_scale_m <= 10000.f) || !(p.lc_alpha >= 0.f) || !(p.lc_eps_sigma >= 0.f) ||
+        !std::isfinite(p.dlc_gain_thr) || !std::isfinite(p.lc_gap_low) || !std::isfinite(p.lc_gap_high))
+        return fail(nullptr, MANTA_ERR_INVALID_ARG, "parameter out of range");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device < 0 || cuda_device >= n_dev) {
+        cudaGetLastError();
+        return fail(nullptr, MANTA_ERR_CUDA, "no CUDA device %d (there is no CPU fallback)", cuda_device);
+    }
+    manta_sim *s = new manta_sim();
+    s->device = cuda_device;
+    s->prm = p;
+    auto bail = [&](int rc) {
+        std::string e = s->err;
+        manta_destroy(s);
+        g_last_error = e;
+        return rc;
+    };
+    if (cudaSetDevice(cuda_device) != cudaSuccess) return bail(fail(s, MANTA_ERR_CUDA, "cudaSetDevice failed"));
+    cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
+
+    // ---- validate + lay out the atlas (one row of 1 m cells per road lane)
+    const uint32_t N = net->n_nodes, M = net->n_edges;
+    s->n_nodes = N;
+    s->n_edges = M;
+    if (net->row_ptr[0] != 0 || net->row_ptr[N] != M) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "row_ptr does not span the edges"));
+    s->row_ptr.assign(net->row_ptr, net->row_ptr + N + 1);
+    s->head.assign(net->head, net->head + M);
+    s->tail.resize(M);
+    s->lanes.assign(net->lanes, net->lanes + M);
+    s->len_c.resize(M);
+    s->cell_off.resize(M);
+    for (uint32_t u = 0; u < N; u++) {
+        if (s->row_ptr[u + 1] < s->row_ptr[u]) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "row_ptr not monotone at node %u", u));
+        if (s->row_ptr[u + 1] - s->row_ptr[u] > 255u) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "out-degree of node %u > 255", u));
+        for (uint32_t e = s->row_ptr[u]; e < s->row_ptr[u + 1]; e++) s->tail[e] = u;
+    }
+    s->max_limit = 0.0;
+    uint64_t cells = 0;
+    for (uint32_t e = 0; e < M; e++) {
+        const float L = net->length_m[e], lim = net->speed_limit[e];
+        if (!(net->lanes[e] >= 1 && net->lanes[e] <= MANTA_MAX_LANES) || !std::isfinite(L) || !(L > 0.f) ||
+            !std::isfinite(lim) || !(lim > 0.f) || net->head[e] >= N)
+            return bail(fail(s, MANTA_ERR_BAD_NETWORK, "edge %u: bad lanes / length / limit / head", e));
+        const long lc = std::lround((double)L);
+        if (lc > (long)MANTA_MAX_EDGE_CELLS) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "edge %u longer than %u cells", e, MANTA_MAX_EDGE_CELLS));
+        s->len_c[e] = (uint32_t)lc;
+        s->max_limit = std::max(s->max_limit, (double)lim);
+        if (cells > 0xFFFFFFFFull) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "atlas exceeds 2^32 cells"));
+        s->cell_off[e] = (uint32_t)cells;
+        cells += (uint64_t)(((uint32_t)lc + 15u) & ~15u) * net->lanes[e];
+    }
+    if (cells + 256 > 0xFFFFFFFFull) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "atlas exceeds 2^32 cells"));
+    s->n_cells = cells;
+    derive_constants(s, 0.0);
+    for (uint32_t e = 0; e < M; e++)
+        if (s->len_c[e] < len_min(s))
+            return bail(fail(s, MANTA_ERR_BAD_NETWORK, "edge %u has %u cells < LEN_MIN %u (G19)", e, s->len_c[e], len_min(s)));
+
+    // ---- constants of R0, rounded once from double
+    DevP &P = s->P;
+    P.dt = p.dt; P.a = p.a; P.T = p.T; P.s0 = p.s0; P.veh_len = p.veh_len;
+    P.C1 = (float)(1.0 / (2.0 * std::sqrt((double)p.a * (double)p.b)));
+    P.HALF_DT = (float)(0.5 * (double)p.dt);
+    P.VSCALE = (float)((1.0 / 1024.0) / (double)p.dt);
+    P.ADT = (float)((double)p.a * (double)p.dt);
+    P.dlc_thr = p.dlc_gain_thr; P.alpha = p.lc_alpha; P.gap_low = p.lc_gap_low; P.gap_high = p.lc_gap_high;
+    P.eps_sigma = p.lc_eps_sigma;
+    P.H = p.lookahead_cells; P.lookback = p.lookback_cells;
+    P.Lam = std::max<uint32_t>(1u, (uint32_t)std::lround((double)p.mlc_scale_m));
+    P.seed_lo = (uint32_t)p.seed; P.seed_hi = (uint32_t)(p.seed >> 32);
+    P.n_edges = M; P.flags = p.flags;
+
+    // ---- device tables
+    std::vector<uint4> et(M);
+    for (uint32_t e = 0; e < M; e++) {
+        const uint32_t prio = (net->node_ctrl && net->node_ctrl[s->head[e]] == MANTA_PRIORITY) ? 1u : 0u;
+        if (net->node_ctrl && net->node_ctrl[s->head[e]] > 1) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "node_ctrl value > 1"));
+        uint32_t vb;
+        memcpy(&vb, &net->speed_limit[e], 4);
+        et[e] = make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16) | (prio << 27), s->head[e], vb);
+    }
+    std::vector<uint32_t> pm(5 * P.Lam + 1);
+    for (uint32_t d = 0; d <= 5 * P.Lam; d++) {  // Eq. (2), distances in units of Lambda (G6)
+        if (d <= P.Lam)
+            pm[d] = 0xFFFFFFFFu;
+        else {
+            const double xi = (double)d / (double)P.Lam;
+            pm[d] = (uint32_t)std::floor(4294967296.0 * std::exp(-(xi - 1.0) * (xi - 1.0)));
+        }
+    }
+    int rc;
+    uint4 *d_et; uint32_t *d_head, *d_pm, *d_ee; unsigned long long *d_claim; Counters *d_ctr; BlockStats *d_blk;
+    if ((rc = upload(s, &d_et, et.data(), M))) return bail(rc);
+    if ((rc = upload(s, &d_head, s->head.data(), M))) return bail(rc);
+    if ((rc = upload(s, &d_pm, pm.data(), pm.size()))) return bail(rc);
+    if ((rc = alloc_fill(s, &d_ee, M, 0))) return bail(rc);
+    if ((rc = alloc_fill(s, &d_claim, (uint64_t)M * 8 + N, 0xFF))) return bail(rc);
+    if ((rc = alloc_fill(s, &d_ctr, 1, 0))) return bail(rc);
+    s->n_blk_stats = (uint32_t)s->sm_count * 16u;
+    if ((rc = alloc_fill(s, &d_blk, s->n_blk_stats, 0))) return bail(rc);
+    for (int k = 0; k < 2; k++) {
+        if ((rc = alloc_fill(s, &P.occ[k], cells + 256, 0))) return bail(rc);
+        if ((rc = alloc_fill(s, &P.spd[k], cells + 256, 0))) return bail(rc);
+    }
+    P.edge_tab = d_et; P.head = d_head; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
+    P.blk = d_blk;
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(s, MANTA_ERR_CUDA, "upload failed: %s", cudaGetErrorString(cudaGetLastError())));
+    *out = s;
+    return MANTA_OK;
+}
+
+int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, const uint32_t *route_edges,
+                     const float *depart_time_s, const float *init_pos_m, const float *init_speed)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (s->loaded) return fail(s, MANTA_ERR_STATE, "trips already loaded");
+    if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0) return fail(s, MANTA_ERR_INVALID_ARG, "null / empty trips");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const uint64_t total = route_ptr[n_trips];
+    if (route_ptr[0] != 0 || total >= 0xFFFFFFFFull) return fail(s, MANTA_ERR_BAD_ROUTE, "route_ptr must start at 0 and stay below 2^32 entries");
+    // ---- validation (BAD_ROUTE)
+    double max_init = 0.0;
+    for (uint32_t i = 0; i < n_trips; i++) {
+        const uint64_t b = route_ptr[i], e = route_ptr[i + 1];
+        if (e <= b || e > total) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: empty route", i);
+        for (uint64_t k = b; k < e; k++) {
+            if (route_edges[k] >= s->n_edges) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: edge id out of range", i);
+            if (k > b && s->head[route_edges[k - 1]] != s->tail[route_edges[k]])
+                return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: route not connected at position %llu", i, (unsigned long long)(k - b));
+        }
+        const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
+        if (!pre && !(depart_time_s[i] >= 0.0f)) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: negative departure time", i);
+        if (init_speed) {
+            if (!(init_speed[i] >= 0.0f) || !std::isfinite(init_speed[i])) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: bad init_speed", i);
+            if (pre) max_init = std::max(max_init, (double)init_speed[i]);
+        }
+    }
+    const DevP saved = s->P;
+    derive_constants(s, max_init);
+    auto rollback = [&](int rc) { s->P = saved; return rc; };
+    for (uint32_t e = 0; e < s->n_edges; e++)
+        if (s->len_c[e] < len_min(s)) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "edge %u shorter than LEN_MIN for the pre-placed speeds", e));
+    if (s->prm.lookback_cells < s->P.L_c + s->P.Z_out)
+        return rollback(fail(s, MANTA_ERR_INVALID_ARG, "lookback_cells %u < L_c + Z_out = %u (R5)", s->prm.lookback_cells, s->P.L_c + s->P.Z_out));
+
+    // ---- vehicle ids: rank in the stable (depart_step, trip index) order
+    std::vector<uint32_t> dstep(n_trips), trip_of_id(n_trips);
+    for (uint32_t i = 0; i < n_trips; i++) {
+        const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
+        const double ds = std::floor((double)depart_time_s[i] / (double)s->prm.dt);
+        if (!pre && ds >= 4294967295.0) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: departure too late", i));
+        dstep[i] = pre ? 0u : (uint32_t)ds;
+    }
+    std::iota(trip_of_id.begin(), trip_of_id.end(), 0u);
+    std::stable_sort(trip_of_id.begin(), trip_of_id.end(), [&](uint32_t x, uint32_t y) { return dstep[x] < dstep[y]; });
+    std::vector<uint32_t> depart_by_id(n_trips), route_start(n_trips);
+    for (uint32_t id = 0; id < n_trips; id++) {
+        depart_by_id[id] = dstep[trip_of_id[id]];
+        route_start[id] = (uint32_t)route_ptr[trip_of_id[id]];
+    }
+    // ---- pre-placed vehicles (R1, last sentence) and their spacing check
+    std::vector<uint4> init_a0;
+    {
+        std::vector<std::pair<uint64_t, uint32_t>> keyx;
+        for (uint32_t id = 0; id < n_trips; id++) {
+            const uint32_t tr = trip_of_id[id];
+            if (!(init_pos_m && init_pos_m[tr] >= 0.0f)) continue;
+            const uint32_t e = route_edges[route_ptr[tr]];
+            const long x = std::lround((double)init_pos_m[tr] * 1024.0);
+            if (x < 0 || (uint64_t)x >= ((uint64_t)s->len_c[e] << 10)) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: init_pos_m beyond its edge", tr));
+            const float v = init_speed ? init_speed[tr] : 0.0f;
+            uint32_t vb;
+            memcpy(&vb, &v, 4);
+            init_a0.push_back(make_uint4((uint32_t)x, vb, id, route_start[id]));
+            keyx.push_back({((uint64_t)e << 32) | (uint64_t)x, id});
+        }
+        std::sort(keyx.begin(), keyx.end());
+        for (size_t k = 1; k < keyx.size(); k++)
+            if ((keyx[k].first >> 32) == (keyx[k - 1].first >> 32) &&
+                (int64_t)(keyx[k].first & 0xFFFFFFFFull) - (int64_t)(keyx[k - 1].first & 0xFFFFFFFFull) < (int64_t)s->P.L_fx)
+                return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "pre-placed vehicles closer than L on edge %llu", (unsigned long long)(keyx[k].first >> 32)));
+    }
+    // ---- admission FIFOs: waiting trips grouped by first edge, id order inside (G25)
+    std::vector<uint32_t> q_edge, q_ptr, q_ids;
+    {
+        std::vector<uint32_t> cnt(s->n_edges + 1, 0);
+        for (uint32_t id = 0; id < n_trips; id++) {
+            const uint32_t tr = trip_of_id[id];
+            if (init_pos_m && init_pos_m[tr] >= 0.0f) continue;
+            cnt[route_edges[route_ptr[tr]] + 1]++;
+        }
+        for (uint32_t e = 0; e < s->n_edges; e++) cnt[e + 1] += cnt[e];
+        q_ids.resize(cnt[s->n_edges]);
+        std::vector<uint32_t> fill(cnt.begin(), cnt.end() - 1);
+        for (uint32_t id = 0; id < n_trips; id++) {
+            const uint32_t tr = trip_of_id[id];
+            if (init_pos_m && init_pos_m[tr] >= 0.0f) continue;
+            q_ids[fill[route_edges[route_ptr[tr]]]++] = id;
+        }
+        for (uint32_t e = 0; e < s->n_edges; e++)
+            if (cnt[e + 1] > cnt[e]) {
+                q_edge.push_back(e);
+                q_ptr.push_back(cnt[e]);
+            }
+        q_ptr.push_back(cnt[s->n_edges]);
+    }
+    // ---- upload; expand the route store on the device
+    DevP &P = s->P;
+    int rc;
+    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_dep, *d_rs, *d_adm, *d_arr, *d_qe, *d_qp, *d_qi, *d_qh;
+    uint64_t *d_rp = nullptr;
+    uint4 *d_route;
+    if ((rc = upload(s, &d_re, route_edges, total))) return rollback(rc);
+    if ((rc = upload(s, &d_rp, route_ptr, (uint64_t)n_trips + 1))) return rollback(rc);
+    if ((rc = upload(s, &d_rowptr, s->row_ptr.data(), s->row_ptr.size()))) return rollback(rc);
+    d_route = (uint4 *)dev_alloc(s, (total + 1) * sizeof(uint4));
+    if (!d_route) return rollback(fail(s, MANTA_ERR_OOM, "route store allocation failed"));
+    k_expand_routes<<<(unsigned)std::min<uint64_t>((total + 255) / 256, 65535ull * 16), 256, 0, s->stream>>>(P.edge_tab, d_rowptr, d_re, total, d_route);
+    k_mark_last<<<(n_trips + 255) / 256, 256, 0, s->stream>>>(d_rp, n_trips, d_route);
+    CUDA_TRY(s, cudaGetLastError());
+    if ((rc = upload(s, &d_dep, depart_by_id.data(), n_trips))) return rollback(rc);
+    if ((rc = upload(s, &d_rs, route_start.data(), n_trips))) return rollback(rc);
+    if ((rc = upload(s, &s->d_trip_of_id, trip_of_id.data(), n_trips))) return rollback(rc);
+    if ((rc = alloc_fill(s, &d_adm, n_trips, 0xFF))) return rollback(rc);
+    if ((rc = alloc_fill(s, &d_arr, n_trips, 0xFF))) return rollback(rc);
+    if ((rc = upload(s, &d_qe, q_edge.data(), q_edge.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qp, q_ptr.data(), q_ptr.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qi, q_ids.data(), q_ids.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
+    const uint32_t cap = n_trips;
+    for (int k = 0; k < 2; k++) {
+        P.A0[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
+        P.A1[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
+        P.acc[k] = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, (uint64_t)cap * sizeof(float)) : nullptr;
+        if (!P.A0[k] || !P.A1[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+        if (P.acc[k]) CUDA_TRY(s, cudaMemsetAsync(P.acc[k], 0, (uint64_t)cap * sizeof(float), s->stream));
+    }
+    P.N = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
+    if (!P.N) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+    P.route = d_route; P.depart_step = d_dep; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
+    P.q_edge = d_qe; P.q_ptr = d_qp; P.q_ids = d_qi; P.q_head = d_qh;
+    P.n_queues = (uint32_t)q_edge.size();
+    P.cap = cap;
+    const uint32_t n_init = (uint32_t)init_a0.size();
+    if (n_init) {
+        CUDA_TRY(s, cudaMemcpyAsync(P.A0[0], init_a0.data(), (uint64_t)n_init * sizeof(uint4), cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(&P.ctr->n_act[0], &n_init, sizeof(uint32_t), cudaMemcpyHostToDevice, s->stream));
+        k_place_initial<<<(n_init + 255) / 256, 256, 0, s->stream>>>(P, n_init);
+        CUDA_TRY(s, cudaGetLastError());
+    }
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    dev_free(s, d_re);
+    dev_free(s, d_rp);
+    dev_free(s, d_rowptr);
+    s->n_trips = n_trips;
+    s->loaded = true;
+    s->t = 0;
+    const uint32_t max_blocks = std::min<uint32_t>(s->n_blk_stats, (uint32_t)s->sm_count * 8u);
+    s->grid_update = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + 255u) / 256u, max_blocks));
+    s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, max_blocks));
+    return MANTA_OK;
+}
+
+int manta_step_async(manta_sim *s, uint32_t n_steps)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    if ((uint64_t)s->t + n_steps >= 0xFFFFFFFEull) return fail(s, MANTA_ERR_INVALID_ARG, "step counter would overflow");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    for (uint32_t k = 0; k < n_steps; k++) {
+        const uint32_t t = s->t;
+        k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
+        k_update<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
+        k_commit<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
+        s->launches += 3;
+        s->t = t + 1;
+    }
+    CUDA_TRY(s, cudaGetLastError());
+    return MANTA_OK;
+}
+
+int manta_sync(manta_sim *s)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return MANTA_OK;
+}
+
+int manta_step(manta_sim *s, uint32_t n_steps)
+{
+    const int rc = manta_step_async(s, n_steps);
+    if (rc) return rc;
+    return manta_sync(s);
+}
+
+int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_trip_result *trips, manta_summary *sum)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const uint32_t n = s->n_trips;
+    const int cur = (int)(s->t & 1u);
+    Counters c;
+    CUDA_TRY(s, cudaMemcpyAsync(&c, s->P.ctr, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (edge_entries)
+        CUDA_TRY(s, cudaMemcpyAsync(edge_entries, s->P.edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyDeviceToHost, s->stream));
+    if (st || trips || sum) {
+        // scratch: status u8 | lane u8 | tag u8 | route_pos u32 | x u32 | v f32 | acc f32 | results uint2
+        const uint64_t nn = ((uint64_t)n + 15) & ~15ull;
+        uint8_t *buf = (uint8_t *)dev_alloc(s, nn * (3 + 16 + 8));
+        if (!buf) return fail(s, MANTA_ERR_OOM, "readback scratch allocation failed");
+        uint2 *d_res = (uint2 *)buf;
+        uint32_t *d_rpos = (uint32_t *)(buf + nn * 8), *d_x = d_rpos + nn;
+        float *d_v = (float *)(d_x + nn), *d_acc = d_v + nn;
+        uint8_t *d_status = (uint8_t *)(d_acc + nn), *d_lane = d_status + nn, *d_tag = d_lane + nn;
+        CUDA_TRY(s, cudaMemsetAsync(buf, 0, nn * (3 + 16 + 8), s->stream));
+        const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
+        k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
+        k_gather_state<<<g, 256, 0, s->stream>>>(s->P, cur, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
+        CUDA_TRY(s, cudaGetLastError());
+        std::vector<uint8_t> h_status(n);
+        CUDA_TRY(s, cudaMemcpyAsync(h_status.data(), d_status, n, cudaMemcpyDeviceToHost, s->stream));
+        if (st) {
+            if (st->route_pos) CUDA_TRY(s, cudaMemcpyAsync(st->route_pos, d_rpos, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->lane) CUDA_TRY(s, cudaMemcpyAsync(st->lane, d_lane, n, cudaMemcpyDeviceToHost, s->stream));
+            if (st->tag) CUDA_TRY(s, cudaMemcpyAsync(st->tag, d_tag, n, cudaMemcpyDeviceToHost, s->stream));
+            if (st->x_fx) CUDA_TRY(s, cudaMemcpyAsync(st->x_fx, d_x, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->v) CUDA_TRY(s, cudaMemcpyAsync(st->v, d_v, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->acc) CUDA_TRY(s, cudaMemcpyAsync(st->acc, d_acc, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+        }
+        if (trips) CUDA_TRY(s, cudaMemcpyAsync(trips, d_res, (uint64_t)n * 8, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        dev_free(s, buf);
+        if (st && st->status) memcpy(st->status, h_status.data(), n);
+        if (sum) {
+            std::vector<BlockStats> bs(s->n_blk_stats);
+            CUDA_TRY(s, cudaMemcpy(bs.data(), s->P.blk, sizeof(BlockStats) * bs.size(), cudaMemcpyDeviceToHost));
+            memset(sum, 0, sizeof *sum);
+            for (uint32_t i = 0; i < n; i++) {
+                sum->n_waiting += h_status[i] == MANTA_WAITING;
+                sum->n_active += h_status[i] == MANTA_ACTIVE;
+            }
+            sum->t = s->t;
+            sum->n_done = c.n_done;
+            sum->sum_travel_steps = c.sum_travel;
+            sum->vehicle_updates = c.n_updates;
+            for (const BlockStats &b : bs) {
+                sum->lane_changes += b.lane_changes;
+                sum->cells_examined += b.cells_examined;
+                sum->lc_evals += b.lc_evals;
+            }
+        }
+    }
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return MANTA_OK;
+}
+
+int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const int cur = (int)(s->t & 1u);
+    if (occ) CUDA_TRY(s, cudaMemcpyAsync(occ, s->P.occ[cur], s->n_cells * 2, cudaMemcpyDeviceToHost, s->stream));
+    if (spd) CUDA_TRY(s, cudaMemcpyAsync(spd, s->P.spd[cur], s->n_cells * 4, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    for (uint32_t e = 0; e < s->n_edges; e++) {
+        if (cell_off) cell_off[e] = s->cell_off[e];
+        if (pitch) pitch[e] = (s->len_c[e] + 15u) & ~15u;
+    }
+    return MANTA_OK;
+}
+
+}  // extern "C"

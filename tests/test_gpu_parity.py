@@ -1,0 +1,169 @@
+"""GPU parity proper: the CUDA path (through the C ABI) against the oracle, bit for bit, on the same seeded
+inputs.  Integer state, occupancy, cell indices, edge transitions and counters must be identical; fp32 speeds are
+compared by bit pattern (deterministic mode: -fmad=false, same operation order)."""
+import numpy as np
+import pytest
+
+from paper_2007_03614_b200 import workloads as wl
+from tests.helpers import ACTIVE, check_conservation, check_entries, check_no_overlap, states_equal
+
+pytestmark = pytest.mark.gpu
+
+SUMMARY_KEYS = ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps", "vehicle_updates", "lane_changes",
+                "cells_examined", "lc_evals")
+
+
+@pytest.fixture(scope="module")
+def binding():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2007_03614_b200 import binding as b
+    b.load_library()
+    return b
+
+
+def describe(net, trips, o_st, g_st, idx):
+    rp = trips["route_ptr"].astype(np.int64)
+    lines = []
+    for i in idx[:6]:
+        lines.append("trip %d route %s" % (i, trips["route_edges"][rp[i]:rp[i + 1]][:12].tolist()))
+        for name, st in (("oracle", o_st), ("gpu", g_st)):
+            lines.append("   %-6s status %d rpos %d lane %d tag %d x %d v %r adm %d arr %d" % (
+                name, st["status"][i], st["route_pos"][i], st["lane"][i], st["tag"][i], st["x_fx"][i],
+                float(st["v"][i]), st["admit_step"][i], st["arrive_step"][i]))
+    return "\n".join(lines)
+
+
+def compare(net, trips, o, g, label, atlas=False):
+    o_st, g_out = o.state(), g.readback()
+    bad = states_equal(o_st, g_out)
+    if bad:
+        idx = sorted({i for _, ii in bad for i in ii})
+        raise AssertionError("%s: state mismatch %s\n%s" % (label, bad, describe(net, trips, o_st, g_out, idx)))
+    assert np.array_equal(o.edge_entries(), g_out["edge_entries"]), label
+    os_, gs = o.summary(), g_out["summary"]
+    assert [os_[k] for k in SUMMARY_KEYS] == [gs[k] for k in SUMMARY_KEYS], (label, os_, gs)
+    if atlas:
+        oa, ga = o.atlas(), g.readback_atlas()
+        lens = np.round(net["length_m"].astype(np.float64)).astype(np.int64)
+        for e in range(net["n_edges"]):
+            for l in range(int(net["lanes"][e])):
+                ro = int(oa["row_off"][int(oa["first_row"][e]) + l])
+                rg = int(ga["cell_off"][e]) + l * int(ga["pitch"][e])
+                occ_o = oa["occ"][ro:ro + lens[e]]
+                code_o = np.where(occ_o > 0, 1 + oa["frac"][ro:ro + lens[e]].astype(np.int64), 0)
+                assert np.array_equal(code_o, ga["occ"][rg:rg + lens[e]].astype(np.int64)), (label, e, l)
+                m = occ_o > 0
+                assert np.array_equal(oa["spd"][ro:ro + lens[e]][m].view(np.uint32),
+                                      ga["spd"][rg:rg + lens[e]][m].view(np.uint32)), (label, e, l)
+                assert (ga["occ"][rg + lens[e]:rg + int(ga["pitch"][e])] == 0).all()      # padding stays empty
+    return o_st, g_out
+
+
+def run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=0, every=16, atlas_every=0, flags=0):
+    o = oracle_mod.Oracle(net, params, trips)
+    gp = dict(params or {})
+    gp["flags"] = flags
+    g = binding.Sim(net, gp, trips)
+    L_fx = o.derived()["L_fx"]
+    compare(net, trips, o, g, "t=0", atlas=True)
+    t = 0
+    while t < n_steps:
+        k = 1 if t < dense_until else min(every, n_steps - t)
+        o.step(k)
+        g.step(k)
+        t += k
+        o_st, g_out = compare(net, trips, o, g, "t=%d" % t, atlas=bool(atlas_every) and (t % atlas_every == 0 or t < 4))
+    check_no_overlap(net, trips, g_out, L_fx)
+    check_conservation(g_out, len(trips["depart_time_s"]), g_out["summary"])
+    check_entries(g_out, g_out["edge_entries"])
+    n_launch = g.launch_count
+    g.close()
+    return o.summary(), n_launch
+
+
+def test_exports(binding):
+    L = binding.load_library()
+    for name in binding.EXPORTS:
+        assert hasattr(L, name)
+
+
+def test_config0_full_run_bit_exact(oracle_mod, binding):
+    net, trips, params, n_steps = wl.config0()
+    s, n_launch = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=600, every=8, atlas_every=400)
+    assert s["n_done"] == 2000 and s["lane_changes"] > 100
+    assert n_launch > 0
+
+
+def test_config1_ring_bit_exact(oracle_mod, binding):
+    net, trips, params, n_steps = wl.config1()
+    s, _ = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=200, every=64, atlas_every=3200)
+    assert s["n_active"] == 600 and s["vehicle_updates"] == 600 * n_steps
+
+
+@pytest.mark.parametrize("ctrl,lanes", [(wl.GREEN, 3), (wl.PRIORITY, 2), (wl.GREEN, 1)])
+def test_dense_small_grid_every_step(oracle_mod, binding, ctrl, lanes):
+    net = wl.grid_network(nx=4, ny=4, lanes=lanes, ctrl=ctrl)
+    o_, d_ = wl.uniform_od(net, 700, 5)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(700, 0.0, 150.0, 6), n_threads=2)
+    run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1500, dense_until=1500, atlas_every=100)
+
+
+def test_multilane_ring_lane_changes(oracle_mod, binding):
+    net = wl.ring_network(n_edges=4, edge_len=300.0, lanes=3)
+    trips = wl.ring_trips(net, n_veh=150, laps_steps=3000, jitter=1.5, vmax=12.0, seed=11)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 3000, dense_until=300, atlas_every=500)
+    assert s["lane_changes"] > 50
+
+
+def test_config2_shaped_small_bit_exact(oracle_mod, binding):
+    """A 1/64-scale Bay-Area-shaped network (ragged row lengths, 1-5 lanes, short edges, H = 256 spanning
+    several edges) with the 07:00-07:20 demand window."""
+    net, trips, params, _ = wl.config2(scale=1 / 64.0, window=(2 * 3600.0, 2 * 3600.0 + 1200.0), n_threads=4)
+    assert len(trips["depart_time_s"]) > 1500
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 3000, dense_until=100, every=25, atlas_every=1000)
+    assert s["n_done"] > 500 and s["lane_changes"] > 20
+
+
+def test_edge_cases(oracle_mod, binding):
+    # a single trip on a single edge; trips that depart after the horizon; route of one edge
+    net = wl.straight_road(n_edges=2, length_m=50.0, lanes=1)
+    trips = dict(route_ptr=np.array([0, 1, 3, 4], np.uint64), route_edges=np.array([0, 0, 1, 1], np.uint32),
+                 depart_time_s=np.array([0.0, 3.2, 1e6], np.float32), init_pos_m=None, init_speed=None)
+    run_both(oracle_mod, binding, net, trips, None, 120, dense_until=120, atlas_every=1)
+
+
+def test_error_codes(binding):
+    net = wl.straight_road(n_edges=2, length_m=50.0)
+    good = dict(route_ptr=np.array([0, 2], np.uint64), route_edges=np.array([0, 1], np.uint32),
+                depart_time_s=np.zeros(1, np.float32), init_pos_m=None, init_speed=None)
+    bad_net = dict(net)
+    bad_net["lanes"] = np.array([0, 1], np.uint8)
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(bad_net)
+    assert e.value.code == binding.ERR_BAD_NETWORK
+    short = dict(net)
+    short["length_m"] = np.array([3.0, 50.0], np.float32)
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(short)
+    assert e.value.code == binding.ERR_BAD_NETWORK
+    s = binding.Sim(net)
+    with pytest.raises(binding.MantaError) as e:
+        s.step(1)
+    assert e.value.code == binding.ERR_STATE
+    for bad in (dict(good, route_edges=np.array([1, 0], np.uint32)),            # not connected
+                dict(good, route_edges=np.array([0, 7], np.uint32)),            # edge id out of range
+                dict(good, route_ptr=np.array([0, 0], np.uint64)),              # empty route
+                dict(good, depart_time_s=np.array([-1.0], np.float32))):
+        with pytest.raises(binding.MantaError) as e:
+            s.load_trips(bad)
+        assert e.value.code == binding.ERR_BAD_ROUTE
+    s.load_trips(good)
+    with pytest.raises(binding.MantaError) as e:
+        s.load_trips(good)
+    assert e.value.code == binding.ERR_STATE
+    s.step(3)
+    assert s.readback()["summary"]["t"] == 3
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(net, dict(dt=0.0))
+    assert e.value.code == binding.ERR_INVALID_ARG
