@@ -38,9 +38,14 @@ def check_conservation(st, n_trips, summary=None):
 
 
 def check_entries(st, edge_entries, trips=None):
-    """K6 (second half): sum of edge entries == sum over admitted vehicles of (route_pos + 1)."""
+    """K6 (second half): sum of edge entries == sum over admitted vehicles of (route_pos + 1); a DONE vehicle
+    has entered every edge of its route (its route_pos is taken from the route length when trips is given)."""
+    rpos = st["route_pos"].astype(np.int64)
+    if trips is not None:
+        rl = np.diff(trips["route_ptr"].astype(np.int64))
+        rpos = np.where(st["status"] == DONE, rl - 1, rpos)
     adm = st["status"] != WAITING
-    assert int(edge_entries.astype(np.int64).sum()) == int((st["route_pos"][adm].astype(np.int64) + 1).sum())
+    assert int(edge_entries.astype(np.int64).sum()) == int((rpos[adm] + 1).sum())
 
 
 def check_monotone(prev, cur):

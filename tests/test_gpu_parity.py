@@ -76,7 +76,7 @@ def run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=0, ev
         o_st, g_out = compare(net, trips, o, g, "t=%d" % t, atlas=bool(atlas_every) and (t % atlas_every == 0 or t < 4))
     check_no_overlap(net, trips, g_out, L_fx)
     check_conservation(g_out, len(trips["depart_time_s"]), g_out["summary"])
-    check_entries(g_out, g_out["edge_entries"])
+    check_entries(g_out, g_out["edge_entries"], trips)
     n_launch = g.launch_count
     g.close()
     return o.summary(), n_launch
