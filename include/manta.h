@@ -138,6 +138,11 @@ int manta_step(manta_sim *sim, uint32_t n_steps);
 int manta_step_async(manta_sim *sim, uint32_t n_steps);
 int manta_sync(manta_sim *sim);
 
+/* Same as manta_step, with CUDA events recorded on the simulation's stream around every phase; adds the device
+ * time of the admission, update and commit phases (milliseconds, summed over the n_steps) to phase_ms[0..2].
+ * For measurement only (the events cost a little); results are identical to manta_step. */
+int manta_step_timed(manta_sim *sim, uint32_t n_steps, double phase_ms[3]);
+
 /* Copies results to host buffers (each may be NULL): per-trip state, cumulative per-edge entry counts
  * ([n_edges]), per-trip admit/arrive steps ([n_trips]), and the summary counters. */
 int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,

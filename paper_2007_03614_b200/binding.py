@@ -19,6 +19,7 @@ NONE = 0xFFFFFFFF
 FLAG_SCALAR_SCAN, FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 1, 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
+           "manta_step_timed",
            "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error")
 
@@ -79,6 +80,7 @@ def load_library():
     for f in ("manta_step", "manta_step_async"):
         getattr(L, f).argtypes = [C.c_void_p, C.c_uint32]
     L.manta_sync.argtypes = [C.c_void_p]
+    L.manta_step_timed.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(C.c_double * 3)]
     L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
     L.manta_atlas_cells.argtypes = [C.c_void_p]
     L.manta_atlas_cells.restype = C.c_uint64
@@ -174,6 +176,12 @@ class Sim:
 
     def step_async(self, n=1):
         self._check(load_library().manta_step_async(self.h, int(n)))
+
+    def step_timed(self, n=1):
+        """manta_step with per-phase CUDA-event timing; returns [admit_ms, update_ms, commit_ms] summed over n."""
+        ms = (C.c_double * 3)(0.0, 0.0, 0.0)
+        self._check(load_library().manta_step_timed(self.h, int(n), C.byref(ms)))
+        return [float(x) for x in ms]
 
     def sync(self):
         self._check(load_library().manta_sync(self.h))

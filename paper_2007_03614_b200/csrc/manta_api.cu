@@ -254,6 +254,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     P.Lam = std::max<uint32_t>(1u, (uint32_t)std::lround((double)p.mlc_scale_m));
     P.seed_lo = (uint32_t)p.seed; P.seed_hi = (uint32_t)(p.seed >> 32);
     P.n_edges = M; P.flags = p.flags;
+    if (p.lookahead_cells > 960u || p.lookback_cells > 960u) P.flags |= MANTA_FLAG_SCALAR_SCAN;   // chunk 'rel' field is 10 bits
 
     // ---- device tables
     std::vector<uint4> et(M);
@@ -463,6 +464,42 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
         s->t = t + 1;
     }
     CUDA_TRY(s, cudaGetLastError());
+    return MANTA_OK;
+}
+
+int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
+{
+    if (!s || !phase_ms) return fail(s, MANTA_ERR_INVALID_ARG, "null argument");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const uint32_t CH = 128;
+    std::vector<cudaEvent_t> ev(4 * CH);
+    for (auto &e : ev) CUDA_TRY(s, cudaEventCreate(&e));
+    for (uint32_t done = 0; done < n_steps;) {
+        const uint32_t m = std::min(CH, n_steps - done);
+        for (uint32_t k = 0; k < m; k++) {
+            const uint32_t t = s->t;
+            cudaEventRecord(ev[4 * k + 0], s->stream);
+            k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
+            cudaEventRecord(ev[4 * k + 1], s->stream);
+            k_update<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
+            cudaEventRecord(ev[4 * k + 2], s->stream);
+            k_commit<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
+            cudaEventRecord(ev[4 * k + 3], s->stream);
+            s->launches += 3;
+            s->t = t + 1;
+        }
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        for (uint32_t k = 0; k < m; k++)
+            for (int ph = 0; ph < 3; ph++) {
+                float ms = 0.f;
+                CUDA_TRY(s, cudaEventElapsedTime(&ms, ev[4 * k + ph], ev[4 * k + ph + 1]));
+                phase_ms[ph] += (double)ms;
+            }
+        done += m;
+    }
+    for (auto &e : ev) cudaEventDestroy(e);
     return MANTA_OK;
 }
 

@@ -59,125 +59,151 @@ __device__ __forceinline__ Lead leader_scalar(const DevP &P, const uint16_t *occ
 }
 
 // ------------------------------------------------------------------------------------------------ R3-R8
-// Everything after the own-lane leader is known: IDM (Eq. 1), mandatory tag (Eq. 2), lane change with gap
-// acceptance (Eq. 3, 4), ballistic integration with hard clamp, edge-end classification and claim.
-__device__ __forceinline__ void finish_update(const DevP &P, uint32_t t, const uint16_t *occ, const float *spd,
-                                              uint32_t slot, const uint4 &s0v, const uint4 &s1v, const Lead &ld,
-                                              float *acc_out, unsigned long long &n_lc, unsigned long long &n_lc_eval)
-{
-    const int32_t x = (int32_t)s0v.x;
-    const float v = __uint_as_float(s0v.y);
-    const uint32_t id = s0v.z, cursor = s0v.w;
-    const uint32_t cell_off = s1v.x, geom = s1v.y;
-    const float v0 = __uint_as_float(s1v.w);
-    const uint32_t len_c = GEOM_LEN(geom), n = GEOM_LANES(geom), l = GEOM_LANE(geom);
-    const bool last = GEOM_LAST(geom) != 0u;
-    const int32_t len_fx = (int32_t)(len_c << 10);
-    const uint32_t c = (uint32_t)x >> 10;
-    const uint32_t pitch = pitch_of(len_c);
+// Per-vehicle context carried from the leader search to the end of the update.
+struct Veh {
+    int32_t x;
+    float v, v0;
+    uint32_t id, cursor, cell_off, geom, eid;
+    uint32_t len_c, n, l, c, pitch;
+    bool last;
+    // after pre_lc
+    float acc_cur;
+    int32_t bound;
+    uint32_t tag, lt;
+    bool mand, disc_pre, need_lc;
+};
 
+__device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &s1v)
+{
+    V.x = (int32_t)s0v.x;
+    V.v = __uint_as_float(s0v.y);
+    V.id = s0v.z;
+    V.cursor = s0v.w;
+    V.cell_off = s1v.x;
+    V.geom = s1v.y;
+    V.eid = s1v.z;
+    V.v0 = __uint_as_float(s1v.w);
+    V.len_c = GEOM_LEN(V.geom);
+    V.n = GEOM_LANES(V.geom);
+    V.l = GEOM_LANE(V.geom);
+    V.last = GEOM_LAST(V.geom) != 0u;
+    V.c = (uint32_t)V.x >> 10;
+    V.pitch = pitch_of(V.len_c);
+}
+
+// R3 against the own-lane leader, R4 (mandatory tag of Eq. 2, lane-change desire pre-tests).
+__device__ __forceinline__ void pre_lc(const DevP &P, uint32_t t, Veh &V, const Lead &ld)
+{
     float s = 0.0f;
-    int32_t bound = 0x7FFFFFFF;
+    V.bound = 0x7FFFFFFF;
     if (ld.found) {
-        float sf = (float)(ld.lead_abs - x);
+        float sf = (float)(ld.lead_abs - V.x);
         sf = sf * 0.0009765625f;
         s = sf - P.veh_len;
-        bound = ld.lead_abs - P.L_fx;
+        V.bound = ld.lead_abs - P.L_fx;
     }
-    const float acc_cur = idm_acc(P, v, v0, ld.found, s, ld.v_lead);
-
+    V.acc_cur = idm_acc(P, V.v, V.v0, ld.found, s, ld.v_lead);
     // R4: mandatory tag, Eq. (2)
-    uint32_t tag = GEOM_TAG(geom);
-    if (tag == 0u && !last && n >= 2u) {
-        uint32_t dcell = len_c - c;
+    uint32_t tag = GEOM_TAG(V.geom);
+    if (tag == 0u && !V.last && V.n >= 2u) {
+        const uint32_t dcell = V.len_c - V.c;
         if (dcell <= P.Lam)
             tag = 1u;
         else if (dcell <= 5u * P.Lam) {
-            uint32_t u0 = rng32(P, id, t, 0u);
+            const uint32_t u0 = rng32(P, V.id, t, 0u);
             if (u0 < P.P_mlc[dcell]) tag = 1u;
         }
     }
-    const uint32_t lo = GEOM_LO(geom), hi = GEOM_HI(geom);
+    V.tag = tag;
+    const uint32_t lo = GEOM_LO(V.geom), hi = GEOM_HI(V.geom);
     const int dir = (t & 1u) ? -1 : 1;  // G11
-    const int lt_s = (int)l + dir;
-    uint32_t l_new = l;
-    float acc = acc_cur;
-    const bool possible = lt_s >= 0 && lt_s < (int)n && c >= P.Z_in && c + P.Z_out < len_c;
+    const int lt_s = (int)V.l + dir;
+    V.mand = false;
+    V.disc_pre = false;
+    V.lt = 0u;
+    const bool possible = lt_s >= 0 && lt_s < (int)V.n && V.c >= P.Z_in && V.c + P.Z_out < V.len_c;
     if (possible) {
         const uint32_t lt = (uint32_t)lt_s;
-        const bool l_in = (l >= lo && l <= hi), lt_in = (lt >= lo && lt <= hi);
-        const bool mand = tag == 1u && !l_in && ((l < lo && dir > 0) || (l > hi && dir < 0));
-        bool disc_pre = false;
+        V.lt = lt;
+        const bool l_in = (V.l >= lo && V.l <= hi), lt_in = (lt >= lo && lt <= hi);
+        V.mand = tag == 1u && !l_in && ((V.l < lo && dir > 0) || (V.l > hi && dir < 0));
         if (!(tag == 1u && !lt_in) && ld.found) {  // G9: impeded in the own lane
-            float rr = v / v0;
+            float rr = V.v / V.v0;
             float rr2 = rr * rr;
             float fr = rr2 * rr2;
             float af = 1.0f - fr;
             af = P.a * af;
-            float g = af - acc_cur;
-            disc_pre = g > P.dlc_thr;
+            float g = af - V.acc_cur;
+            V.disc_pre = g > P.dlc_thr;
         }
-        if (mand || disc_pre) {
-            n_lc_eval += 1ull;
-            // R5: lead / lag in the target lane
-            const uint32_t rowt = cell_off + lt * pitch;
-            uint32_t ja = 0, ca = 0, jb = 0, cb = 0;
-            const bool has_a = scan_fwd(occ, rowt, c, min(len_c, c + P.H), ja, ca);
-            const bool has_b = scan_bwd(occ, rowt, c > P.lookback ? c - P.lookback : 0u, c, jb, cb);
-            int32_t x_a = 0, x_b = 0;
-            float v_a = 0.0f, v_b = 0.0f, gap_lead = 0.0f, gap_lag = 0.0f;
+    }
+    V.need_lc = V.mand || V.disc_pre;
+}
+
+// R5 gaps, R6 gap acceptance (Eq. 3, 4), R7 integration and clamp, R8 edge-end classification and claim.
+// (has_a, ja, ca, v_a) / (has_b, jb, cb, v_b): lead / lag found in the target lane (cell index, cell code, speed);
+// ignored unless V.need_lc.
+__device__ __forceinline__ void post_lc(const DevP &P, uint32_t t, const Veh &V, uint32_t slot, bool has_a, uint32_t ja,
+                                        uint32_t ca, float v_a, bool has_b, uint32_t jb, uint32_t cb, float v_b,
+                                        float *acc_out, unsigned long long &n_lc)
+{
+    const int32_t x = V.x;
+    const float v = V.v;
+    uint32_t l_new = V.l;
+    float acc = V.acc_cur;
+    int32_t bound = V.bound;
+    if (V.need_lc) {
+        int32_t x_a = 0, x_b = 0;
+        float gap_lead = 0.0f, gap_lag = 0.0f;
+        if (has_a) {
+            x_a = (int32_t)((ja << 10) | (ca - 1u));
+            float gf = (float)(x_a - x);
+            gf = gf * 0.0009765625f;
+            gap_lead = gf - P.veh_len;
+        }
+        if (has_b) {
+            x_b = (int32_t)((jb << 10) | (cb - 1u));
+            float gf = (float)(x - x_b);
+            gf = gf * 0.0009765625f;
+            gap_lag = gf - P.veh_len;
+        }
+        const float acc_tgt = idm_acc(P, v, V.v0, has_a, gap_lead, v_a);
+        const float gain = acc_tgt - V.acc_cur;
+        const bool want = V.mand || (V.disc_pre && gain > P.dlc_thr);
+        if (want) {
+            // R6: gap acceptance, Eq. (3), (4)
+            const float g0 = (v < 11.176f) ? P.gap_low : P.gap_high;
+            bool ok = true;
             if (has_a) {
-                x_a = (int32_t)((ja << 10) | (ca - 1u));
-                v_a = spd[(size_t)rowt + ja];
-                float gf = (float)(x_a - x);
-                gf = gf * 0.0009765625f;
-                gap_lead = gf - P.veh_len;
+                float t1 = P.alpha * v;
+                float t2 = v - v_a;
+                t2 = P.alpha * t2;
+                float g = g0 + t1;
+                g = g + t2;
+                g = fmaxf(g0, g);
+                g = g + eps_draw(P, V.id, t, 1u);
+                g = fmaxf(g, 0.0f);
+                if (!(gap_lead >= g)) ok = false;
             }
             if (has_b) {
-                x_b = (int32_t)((jb << 10) | (cb - 1u));
-                v_b = spd[(size_t)rowt + jb];
-                float gf = (float)(x - x_b);
-                gf = gf * 0.0009765625f;
-                gap_lag = gf - P.veh_len;
+                float t1 = P.alpha * v;
+                float t2 = v - v_b;
+                t2 = P.alpha * t2;
+                float g = g0 + t1;
+                g = g + t2;
+                g = fmaxf(g0, g);
+                g = g + eps_draw(P, V.id, t, 4u);
+                float fl = v_b + P.ADT;  // hard safety floor
+                fl = fl * P.dt;
+                fl = fl + 0.01f;
+                g = fmaxf(g, fl);
+                if (!(gap_lag >= g)) ok = false;
             }
-            const float acc_tgt = idm_acc(P, v, v0, has_a, gap_lead, v_a);
-            const float gain = acc_tgt - acc_cur;
-            const bool want = mand || (disc_pre && gain > P.dlc_thr);
-            if (want) {
-                // R6: gap acceptance, Eq. (3), (4)
-                const float g0 = (v < 11.176f) ? P.gap_low : P.gap_high;
-                bool ok = true;
-                if (has_a) {
-                    float t1 = P.alpha * v;
-                    float t2 = v - v_a;
-                    t2 = P.alpha * t2;
-                    float g = g0 + t1;
-                    g = g + t2;
-                    g = fmaxf(g0, g);
-                    g = g + eps_draw(P, id, t, 1u);
-                    g = fmaxf(g, 0.0f);
-                    if (!(gap_lead >= g)) ok = false;
-                }
-                if (has_b) {
-                    float t1 = P.alpha * v;
-                    float t2 = v - v_b;
-                    t2 = P.alpha * t2;
-                    float g = g0 + t1;
-                    g = g + t2;
-                    g = fmaxf(g0, g);
-                    g = g + eps_draw(P, id, t, 4u);
-                    float fl = v_b + P.ADT;  // hard safety floor
-                    fl = fl * P.dt;
-                    fl = fl + 0.01f;
-                    g = fmaxf(g, fl);
-                    if (!(gap_lag >= g)) ok = false;
-                }
-                if (ok) {
-                    l_new = lt;
-                    acc = fminf(acc_cur, acc_tgt);
-                    if (has_a) bound = min(bound, x_a - P.L_fx);
-                    n_lc += 1ull;
-                }
+            if (ok) {
+                l_new = V.lt;
+                acc = fminf(V.acc_cur, acc_tgt);
+                if (has_a) bound = min(bound, x_a - P.L_fx);
+                n_lc += 1ull;
             }
         }
     }
@@ -197,25 +223,143 @@ __device__ __forceinline__ void finish_update(const DevP &P, uint32_t t, const u
     }
     if (acc_out) acc_out[slot] = acc;
     // R8
+    const int32_t len_fx = (int32_t)(V.len_c << 10);
     uint32_t kind, word = 0u, nx;
     if (xn < len_fx) {
         kind = KIND_STAY;
         nx = (uint32_t)xn;
-    } else if (last) {
+    } else if (V.last) {
         kind = KIND_DONE;  // G18
         nx = 0u;
     } else {
-        const uint4 rn = P.route[cursor + 1u];
+        const uint4 rn = P.route[V.cursor + 1u];
         const uint32_t lplus = min(l_new, GEOM_LANES(rn.y) - 1u);
-        word = GEOM_PRIO(geom) ? (P.n_edges * 8u + P.head[s1v.z])   // PRIORITY: the node
-                               : (rn.z * 8u + lplus);               // GREEN: the lane entry
+        word = GEOM_PRIO(V.geom) ? (P.n_edges * 8u + P.head[V.eid])  // PRIORITY: the node
+                                 : (rn.z * 8u + lplus);              // GREEN: the lane entry
         kind = KIND_CAND;
         nx = (uint32_t)(xn - len_fx);
         // smallest id wins; the key carries ~t in the high word so claim words never need a reset
-        const unsigned long long key = ((unsigned long long)(0xFFFFFFFFu - t) << 32) | (unsigned long long)id;
+        const unsigned long long key = ((unsigned long long)(0xFFFFFFFFu - t) << 32) | (unsigned long long)V.id;
         atomicMin(&P.claim[word], key);
     }
-    P.N[slot] = make_uint4(nx, __float_as_uint(vn), kind | (l_new << 2) | (tag << 5), word);
+    P.N[slot] = make_uint4(nx, __float_as_uint(vn), kind | (l_new << 2) | (V.tag << 5), word);
+}
+
+// Scalar version of the whole update of one vehicle (MANTA_FLAG_SCALAR_SCAN, and the fallback of the cooperative
+// path for vehicles whose window does not fit its chunk list).
+__device__ __forceinline__ void lc_scans_scalar(const DevP &P, const uint16_t *occ, const float *spd, const Veh &V,
+                                                bool &has_a, uint32_t &ja, uint32_t &ca, float &v_a, bool &has_b,
+                                                uint32_t &jb, uint32_t &cb, float &v_b)
+{
+    // R5: lead / lag in the target lane
+    const uint32_t rowt = V.cell_off + V.lt * V.pitch;
+    has_a = scan_fwd(occ, rowt, V.c, min(V.len_c, V.c + P.H), ja, ca);
+    has_b = scan_bwd(occ, rowt, V.c > P.lookback ? V.c - P.lookback : 0u, V.c, jb, cb);
+    v_a = has_a ? spd[(size_t)rowt + ja] : 0.0f;
+    v_b = has_b ? spd[(size_t)rowt + jb] : 0.0f;
+}
+
+// ------------------------------------------------------------------------------------------------ R2/R5 cooperative
+// Warp-cooperative look-ahead.  Each lane owns one vehicle and writes the atlas windows it has to search as a list
+// of CHUNKS (64 cells = 128 bytes = one cache line, 8-cell aligned inside its row) into the warp's shared-memory
+// scratch.  The warp then serves the lists in rounds: in round r, the four 8-lane groups each issue chunk r of up
+// to eight owners as one 16-byte load per lane (8 independent, fully coalesced 128-byte requests in flight per
+// lane), then find the first (or last) occupied cell with ballot + ffs.  Lanes outside a chunk's valid range are
+// predicated off, so no sector outside the window is fetched.
+#define MANTA_MAXCH 12
+#define MANTA_CH_STRIDE 13
+struct WarpScratch {
+    uint2 ch[32 * MANTA_CH_STRIDE];  // chunk lists: x = absolute cell index of the chunk, y = rel | lo << 10 | hi << 16
+    uint2 res[32];                   // per owner: x = absolute cell index of the hit, y = rel_dist << 16 | cell code
+    uint32_t nch[32];
+};
+
+// chunks of cells [start, end) of the row at absolute cell `row`, ascending.  `bias` = (distance in cells from the
+// owner's reference to the row's cell 0) so that rel = bias + base.  Returns the new list length (ovf on overflow).
+__device__ __forceinline__ uint32_t emit_fwd(uint2 *list, uint32_t k, uint32_t row, uint32_t start, uint32_t end, int bias,
+                                             bool &ovf)
+{
+    for (uint32_t base = start & ~7u; base < end; base += 64u) {
+        if (k >= MANTA_MAXCH) {
+            ovf = true;
+            return k;
+        }
+        const uint32_t lo = start > base ? start - base : 0u;
+        const uint32_t hi = min(end - base, 64u);
+        list[k++] = make_uint2(row + base, (uint32_t)(bias + (int)base) | (lo << 10) | (hi << 16));
+    }
+    return k;
+}
+// chunks of cells [start, end) descending (nearest first) for the backward (lag) search; rel = c - base
+__device__ __forceinline__ uint32_t emit_bwd(uint2 *list, uint32_t k, uint32_t row, uint32_t start, uint32_t end, uint32_t c,
+                                             bool &ovf)
+{
+    if (end <= start) return k;
+    for (int base = (int)((end - 1u) & ~63u) ; base + 64 > (int)start; base -= 64) {
+        if (k >= MANTA_MAXCH) {
+            ovf = true;
+            return k;
+        }
+        const uint32_t b = (uint32_t)base;
+        const uint32_t lo = (int)start > base ? start - b : 0u;
+        const uint32_t hi = min(end - b, 64u);
+        list[k++] = make_uint2(row + b, (c - b) | (lo << 10) | (hi << 16));
+    }
+    return k;
+}
+
+template <bool BACKWARD>
+__device__ __forceinline__ void coop_scan(const uint16_t *occ, WarpScratch &ws, uint32_t lane)
+{
+    const uint32_t q = lane >> 3, j = lane & 7u, my = j * 8u;
+    uint32_t pend = 0u, maxr = 0u;
+#pragma unroll
+    for (uint32_t p = 0; p < 8u; p++) {
+        const uint32_t nc = ws.nch[p * 4u + q];
+        if (nc) pend |= 1u << p;
+        maxr = max(maxr, nc);
+    }
+    maxr = __reduce_max_sync(0xFFFFFFFFu, maxr);
+    for (uint32_t r = 0; r < maxr; r++) {
+        if (!__any_sync(0xFFFFFFFFu, pend != 0u)) break;
+        uint4 w[8];
+#pragma unroll
+        for (uint32_t p = 0; p < 8u; p++) {
+            const uint32_t o = p * 4u + q;
+            w[p] = make_uint4(0u, 0u, 0u, 0u);
+            if (((pend >> p) & 1u) && r < ws.nch[o]) {
+                const uint2 d = ws.ch[o * MANTA_CH_STRIDE + r];
+                const uint32_t lo = (d.y >> 10) & 63u, hi = (d.y >> 16) & 127u;
+                if (my + 8u > lo && my < hi) w[p] = *reinterpret_cast<const uint4 *>(occ + (size_t)d.x + my);
+            }
+        }
+#pragma unroll
+        for (uint32_t p = 0; p < 8u; p++) {
+            const uint32_t o = p * 4u + q;
+            uint32_t m = nzmask8(w[p]);
+            uint2 d = make_uint2(0u, 0u);
+            if (m) {
+                d = ws.ch[o * MANTA_CH_STRIDE + r];
+                const uint32_t lo = (d.y >> 10) & 63u, hi = (d.y >> 16) & 127u;
+                if (lo > my) m &= 0xFFu << (lo - my);
+                if (hi < my + 8u) m &= (1u << (hi - my)) - 1u;
+            }
+            const uint32_t bal = __ballot_sync(0xFFFFFFFFu, m != 0u);
+            const uint32_t gb = (bal >> (q * 8u)) & 0xFFu;
+            if (gb) {
+                const uint32_t jj = BACKWARD ? (31u - (uint32_t)__clz((int)gb)) : ((uint32_t)__ffs((int)gb) - 1u);
+                if (j == jj) {
+                    const uint32_t i = BACKWARD ? (31u - (uint32_t)__clz((int)m)) : ((uint32_t)__ffs((int)m) - 1u);
+                    const uint32_t off = my + i, rel = d.y & 1023u;
+                    ws.res[o] = make_uint2(d.x + off, ((BACKWARD ? rel - off : rel + off) << 16) | code_at(w[p], i));
+                }
+                pend &= ~(1u << p);
+            } else if (((pend >> p) & 1u) && r + 1u >= ws.nch[o]) {
+                pend &= ~(1u << p);
+            }
+        }
+    }
+    __syncwarp();
 }
 
 // ------------------------------------------------------------------------------------------------ P0: R1
@@ -255,22 +399,145 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
 }
 
 // ------------------------------------------------------------------------------------------------ P1: R2-R8
-__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize,
-                                             unsigned long long &n_lc, unsigned long long &n_cells,
-                                             unsigned long long &n_eval)
+// Scalar variant: one thread does everything for its vehicle (A/B baseline, MANTA_FLAG_SCALAR_SCAN).
+__device__ __forceinline__ void update_phase_scalar(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize,
+                                                    unsigned long long &n_lc, unsigned long long &n_cells,
+                                                    unsigned long long &n_eval)
 {
     const int cur = (int)(t & 1u);
     const uint16_t *occ = P.occ[cur];
     const float *spd = P.spd[cur];
     const uint32_t n = P.ctr->n_act[cur];
-    const uint4 *A0 = P.A0[cur];
-    const uint4 *A1 = P.A1[cur];
     float *acc_out = P.acc[cur];
     for (uint32_t i = gtid; i < n; i += gsize) {
-        const uint4 s0v = A0[i];
-        const uint4 s1v = A1[i];
-        const Lead ld = leader_scalar(P, occ, spd, s0v.w, s1v.x, s1v.y, GEOM_LANE(s1v.y), s0v.x >> 10, n_cells);
-        finish_update(P, t, occ, spd, i, s0v, s1v, ld, acc_out, n_lc, n_eval);
+        Veh V;
+        veh_load(V, P.A0[cur][i], P.A1[cur][i]);
+        const Lead ld = leader_scalar(P, occ, spd, V.cursor, V.cell_off, V.geom, V.l, V.c, n_cells);
+        pre_lc(P, t, V, ld);
+        bool has_a = false, has_b = false;
+        uint32_t ja = 0, ca = 0, jb = 0, cb = 0;
+        float v_a = 0.0f, v_b = 0.0f;
+        if (V.need_lc) {
+            n_eval += 1ull;
+            lc_scans_scalar(P, occ, spd, V, has_a, ja, ca, v_a, has_b, jb, cb, v_b);
+        }
+        post_lc(P, t, V, i, has_a, ja, ca, v_a, has_b, jb, cb, v_b, acc_out, n_lc);
+    }
+}
+
+// Warp-cooperative variant (default): lane = vehicle; the atlas windows of the 32 vehicles of a warp are searched
+// by coop_scan.  Must be entered by whole warps.
+__device__ __forceinline__ void update_phase_coop(const DevP &P, uint32_t t, WarpScratch &ws, uint32_t warp_gid,
+                                                  uint32_t n_warps_total, unsigned long long &n_lc,
+                                                  unsigned long long &n_cells, unsigned long long &n_eval)
+{
+    const int cur = (int)(t & 1u);
+    const uint16_t *occ = P.occ[cur];
+    const float *spd = P.spd[cur];
+    const uint32_t n = P.ctr->n_act[cur];
+    float *acc_out = P.acc[cur];
+    const uint32_t lane = threadIdx.x & 31u;
+    uint2 *mylist = &ws.ch[lane * MANTA_CH_STRIDE];
+    for (uint32_t base = warp_gid * 32u; base < n; base += n_warps_total * 32u) {
+        const uint32_t i = base + lane;
+        const bool valid = i < n;
+        Veh V;
+        Lead ld;
+        ld.found = false;
+        ld.lead_abs = 0;
+        ld.v_lead = 0.0f;
+        bool ovf = false;
+        uint32_t k = 0u, win_total = 0u;
+        V.need_lc = false;
+        if (valid) {
+            veh_load(V, P.A0[cur][i], P.A1[cur][i]);
+            // R2: the look-ahead window as chunk list: own row from c+1, then on along the route
+            uint32_t len = V.len_c, row = V.cell_off + V.l * V.pitch, start = V.c + 1u, rem = P.H, dist0 = 0u, l = V.l;
+            uint32_t cursor = V.cursor;
+            bool last = V.last;
+            for (;;) {
+                const uint32_t end = min(len, start + rem);
+                if (start < end) {
+                    k = emit_fwd(mylist, k, row, start, end, (int)dist0 - (int)V.c + 8, ovf);
+                    win_total += end - start;
+                    rem -= end - start;
+                }
+                if (ovf || rem == 0u || last) break;
+                cursor += 1u;
+                const uint4 rr = P.route[cursor];
+                dist0 += len;
+                len = GEOM_LEN(rr.y);
+                l = min(l, GEOM_LANES(rr.y) - 1u);
+                row = rr.x + l * pitch_of(len);
+                start = 0u;
+                last = GEOM_LAST(rr.y) != 0u;
+            }
+        }
+        ws.nch[lane] = (valid && !ovf) ? k : 0u;
+        ws.res[lane] = make_uint2(0u, 0u);
+        __syncwarp();
+        coop_scan<false>(occ, ws, lane);
+        if (valid) {
+            if (ovf) {
+                ld = leader_scalar(P, occ, spd, V.cursor, V.cell_off, V.geom, V.l, V.c, n_cells);
+            } else {
+                const uint2 r = ws.res[lane];
+                if (r.y & 0xFFFFu) {
+                    const uint32_t dist = V.c + (r.y >> 16) - 8u;   // cells from the own edge's tail to the leader
+                    ld.found = true;
+                    ld.lead_abs = (int32_t)((dist << 10) | ((r.y & 0xFFFFu) - 1u));
+                    ld.v_lead = spd[r.x];
+                    n_cells += (unsigned long long)(dist - V.c);
+                } else {
+                    n_cells += (unsigned long long)win_total;
+                }
+            }
+            pre_lc(P, t, V, ld);
+        }
+        const bool need = valid && V.need_lc;
+        bool has_a = false, has_b = false;
+        uint32_t ja = 0, ca = 0, jb = 0, cb = 0;
+        float v_a = 0.0f, v_b = 0.0f;
+        if (__any_sync(0xFFFFFFFFu, need)) {
+            // R5: lead (forward from c) and lag (backward from c-1) in the target lane, same machinery
+            const uint32_t rowt = V.cell_off + V.lt * V.pitch;
+            bool ovf2 = false;
+            k = 0u;
+            if (need) k = emit_fwd(mylist, 0u, rowt, V.c, min(V.len_c, V.c + P.H), 8 - (int)V.c, ovf2);
+            ws.nch[lane] = (need && !ovf2) ? k : 0u;
+            ws.res[lane] = make_uint2(0u, 0u);
+            __syncwarp();
+            coop_scan<false>(occ, ws, lane);
+            if (need && !ovf2) {
+                const uint2 r = ws.res[lane];
+                if (r.y & 0xFFFFu) {
+                    has_a = true;
+                    ja = V.c + (r.y >> 16) - 8u;
+                    ca = r.y & 0xFFFFu;
+                    v_a = spd[r.x];
+                }
+            }
+            k = 0u;
+            if (need) k = emit_bwd(mylist, 0u, rowt, V.c > P.lookback ? V.c - P.lookback : 0u, V.c, V.c, ovf2);
+            ws.nch[lane] = (need && !ovf2) ? k : 0u;
+            ws.res[lane] = make_uint2(0u, 0u);
+            __syncwarp();
+            coop_scan<true>(occ, ws, lane);
+            if (need && !ovf2) {
+                const uint2 r = ws.res[lane];
+                if (r.y & 0xFFFFu) {
+                    has_b = true;
+                    jb = V.c - (r.y >> 16);
+                    cb = r.y & 0xFFFFu;
+                    v_b = spd[r.x];
+                }
+            }
+            if (need && ovf2) lc_scans_scalar(P, occ, spd, V, has_a, ja, ca, v_a, has_b, jb, cb, v_b);
+        }
+        if (valid) {
+            if (need) n_eval += 1ull;
+            post_lc(P, t, V, i, has_a, ja, ca, v_a, has_b, jb, cb, v_b, acc_out, n_lc);
+        }
     }
 }
 
@@ -394,12 +661,16 @@ __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 __global__ void __launch_bounds__(256) k_update(const DevP P, uint32_t t)
 {
     __shared__ unsigned long long s_stats[3];
+    __shared__ WarpScratch s_ws[8];
     if (threadIdx.x < 3u) s_stats[threadIdx.x] = 0ull;
     __syncthreads();
     unsigned long long n_lc = 0ull, n_cells = 0ull, n_eval = 0ull;
     const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
     if (gtid == 0u) P.ctr->n_updates += (unsigned long long)P.ctr->n_act[t & 1u];
-    update_phase(P, t, gtid, gridDim.x * blockDim.x, n_lc, n_cells, n_eval);
+    if (P.flags & 1u)   // MANTA_FLAG_SCALAR_SCAN
+        update_phase_scalar(P, t, gtid, gridDim.x * blockDim.x, n_lc, n_cells, n_eval);
+    else
+        update_phase_coop(P, t, s_ws[threadIdx.x >> 5], gtid >> 5, (gridDim.x * blockDim.x) >> 5, n_lc, n_cells, n_eval);
     flush_stats(P, n_lc, n_cells, n_eval, s_stats);
 }
 

@@ -296,7 +296,7 @@ def uniform_od(net, n_trips, seed=SEED_DEMAND):
 
 
 def gravity_od(net, n_trips, seed=SEED_DEMAND, n_origins=16384, dist_median=4300.0, dist_sigma=1.0,
-               n_centres=12, centre_share=0.3):
+               n_centres=12, centre_share=0.0):
     """Gravity-style OD on a coordinate-carrying network: origins drawn from a weighted set of origin nodes
     (the paper samples nodes inside 1454 TAZs); destination at a lognormal crow-fly distance
     (tuned so routed lengths have median ~6.5 km / mean ~11 km) in a uniform direction, or,
@@ -379,8 +379,13 @@ def depart_bimodal(n_trips, seed=SEED_DEMAND + 1, t_open=5 * 3600.0, t_close=12 
     return out.astype(np.float32)
 
 
-def make_trips(net, origin, dest, depart_time_s, n_threads=None):
-    rp, re_ = route_trips(net, origin, dest, n_threads=n_threads)
+def make_trips(net, origin, dest, depart_time_s, n_threads=None, weight="length"):
+    """Routes are shortest paths by edge LENGTH ("the length of the road link in meters ... is used
+    as the weight of the edge"), fixed for the whole run; weight="time" gives free-flow time."""
+    w = net["length_m"].astype(np.float64)
+    if weight == "time":
+        w = w / net["speed_limit"].astype(np.float64)
+    rp, re_ = route_trips(net, origin, dest, weight=w, n_threads=n_threads)
     return dict(route_ptr=rp, route_edges=re_, depart_time_s=np.asarray(depart_time_s, np.float32),
                 init_pos_m=None, init_speed=None)
 
@@ -397,7 +402,8 @@ def config1(n_veh=600, n_steps=14400):
     return net, ring_trips(net, n_veh=n_veh, laps_steps=n_steps), dict(lookahead_cells=128), n_steps
 
 
-def config2(scale=1.0, n_trips=None, seed=SEED_DEMAND, net=None, window=None, n_threads=None):
+def config2(scale=1.0, n_trips=None, seed=SEED_DEMAND, net=None, window=None, n_threads=None, weight="time",
+            centre_share=0.0):
     """Bay-Area-shaped run.  scale < 1 shrinks the lattice side and the trip count together (parity cases);
     window=(t0, t1) keeps only trips departing in [t0, t1) seconds after 05:00, shifted to start at 0."""
     if net is None:
@@ -406,8 +412,8 @@ def config2(scale=1.0, n_trips=None, seed=SEED_DEMAND, net=None, window=None, n_
     if n_trips is None:
         n_trips = int(round(3_200_000 * scale))
     dep = depart_bimodal(n_trips, seed + 1)
-    o, d = gravity_od(net, n_trips, seed, n_origins=max(64, int(16384 * scale)))
+    o, d = gravity_od(net, n_trips, seed, n_origins=max(64, int(16384 * scale)), centre_share=centre_share)
     if window is not None:
         sel = (dep >= window[0]) & (dep < window[1])
         o, d, dep = o[sel], d[sel], dep[sel] - np.float32(window[0])
-    return net, make_trips(net, o, d, dep, n_threads=n_threads), dict(lookahead_cells=256), 50400
+    return net, make_trips(net, o, d, dep, n_threads=n_threads, weight=weight), dict(lookahead_cells=256), 50400

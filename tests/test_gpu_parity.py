@@ -88,9 +88,14 @@ def test_exports(binding):
         assert hasattr(L, name)
 
 
-def test_config0_full_run_bit_exact(oracle_mod, binding):
+FLAGS = [0, 1]   # default (warp-cooperative scan) and MANTA_FLAG_SCALAR_SCAN
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_config0_full_run_bit_exact(oracle_mod, binding, flags):
     net, trips, params, n_steps = wl.config0()
-    s, n_launch = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=600, every=8, atlas_every=400)
+    s, n_launch = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=600, every=8, atlas_every=400,
+                           flags=flags)
     assert s["n_done"] == 2000 and s["lane_changes"] > 100
     assert n_launch > 0
 
@@ -101,27 +106,33 @@ def test_config1_ring_bit_exact(oracle_mod, binding):
     assert s["n_active"] == 600 and s["vehicle_updates"] == 600 * n_steps
 
 
+@pytest.mark.parametrize("flags", FLAGS)
 @pytest.mark.parametrize("ctrl,lanes", [(wl.GREEN, 3), (wl.PRIORITY, 2), (wl.GREEN, 1)])
-def test_dense_small_grid_every_step(oracle_mod, binding, ctrl, lanes):
+def test_dense_small_grid_every_step(oracle_mod, binding, ctrl, lanes, flags):
     net = wl.grid_network(nx=4, ny=4, lanes=lanes, ctrl=ctrl)
     o_, d_ = wl.uniform_od(net, 700, 5)
     trips = wl.make_trips(net, o_, d_, wl.depart_uniform(700, 0.0, 150.0, 6), n_threads=2)
-    run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1500, dense_until=1500, atlas_every=100)
+    run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1500, dense_until=1500, atlas_every=100,
+             flags=flags)
 
 
-def test_multilane_ring_lane_changes(oracle_mod, binding):
+@pytest.mark.parametrize("flags", FLAGS)
+def test_multilane_ring_lane_changes(oracle_mod, binding, flags):
     net = wl.ring_network(n_edges=4, edge_len=300.0, lanes=3)
     trips = wl.ring_trips(net, n_veh=150, laps_steps=3000, jitter=1.5, vmax=12.0, seed=11)
-    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 3000, dense_until=300, atlas_every=500)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 3000, dense_until=300, atlas_every=500,
+                    flags=flags)
     assert s["lane_changes"] > 50
 
 
-def test_config2_shaped_small_bit_exact(oracle_mod, binding):
+@pytest.mark.parametrize("flags", FLAGS)
+def test_config2_shaped_small_bit_exact(oracle_mod, binding, flags):
     """A 1/64-scale Bay-Area-shaped network (ragged row lengths, 1-5 lanes, short edges, H = 256 spanning
     several edges) with the 07:00-07:20 demand window."""
     net, trips, params, _ = wl.config2(scale=1 / 64.0, window=(2 * 3600.0, 2 * 3600.0 + 1200.0), n_threads=4)
     assert len(trips["depart_time_s"]) > 1500
-    s, _ = run_both(oracle_mod, binding, net, trips, params, 3000, dense_until=100, every=25, atlas_every=1000)
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 3000, dense_until=100, every=25, atlas_every=1000,
+                    flags=flags)
     assert s["n_done"] > 500 and s["lane_changes"] > 20
 
 
