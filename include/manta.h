@@ -48,8 +48,7 @@ extern "C" {
 #define MANTA_MAX_EDGE_CELLS 65535u
 
 /* manta_params.flags */
-#define MANTA_FLAG_SCALAR_SCAN 1u      /* per-thread look-ahead instead of the warp-cooperative scan (A/B evidence) */
-#define MANTA_FLAG_MULTI_KERNEL 2u     /* three launches per step instead of the persistent cooperative kernel */
+#define MANTA_FLAG_MULTI_KERNEL 2u     /* three launches per timestep instead of the persistent cooperative kernel */
 #define MANTA_FLAG_RECORD_ACC 4u       /* keep each vehicle's last acceleration for manta_state.acc (tests)  */
 
 typedef struct manta_sim manta_sim; /* opaque; owned by the library; one simulation on one device */
@@ -149,7 +148,8 @@ int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, m
                    manta_summary *summary);
 
 /* Logical atlas of the current step for tests: occ[i] = 0 (empty) or 1 + frac10 per padded cell, spd[i] the
- * occupant's speed; row (e, lane) starts at cell_off[e] + lane * pitch[e].  Sizes via manta_atlas_cells. */
+ * occupant's speed; row (e, lane) starts at cell_off[e] + lane * pitch[e].  Sizes via manta_atlas_cells.  (On the
+ * device the atlas is a 1-bit occupancy plane plus an 8-byte payload plane; this call expands it.) */
 uint64_t manta_atlas_cells(const manta_sim *sim);
 int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch);
 

@@ -16,7 +16,7 @@ OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STAT
 GREEN, PRIORITY = 0, 1
 WAITING, ACTIVE, DONE = 0, 1, 2
 NONE = 0xFFFFFFFF
-FLAG_SCALAR_SCAN, FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 1, 2, 4
+FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_timed",

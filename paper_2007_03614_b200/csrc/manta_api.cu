@@ -51,8 +51,9 @@ struct manta_sim {
     uint32_t *d_trip_of_id = nullptr;
     uint32_t t = 0;
     int sm_count = 148;
-    int grid_update = 1, grid_admit = 1;
+    int grid_update = 1, grid_admit = 1, grid_cross = 1, grid_persist = 0;
     uint32_t n_blk_stats = 0;
+    uint32_t n_active_hint = 0;   // active count seen by the last readback (sizes the cross-phase launch)
 };
 
 namespace {
@@ -182,6 +183,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         return fail(nullptr, MANTA_ERR_INVALID_ARG, "network arrays missing");
     const manta_params &p = *prm;
     if (!(p.dt > 0.f) || !(p.a > 0.f) || !(p.b > 0.f) || !(p.T >= 0.f) || !(p.s0 >= 0.f) || !(p.veh_len > 0.f) ||
+        !(p.veh_len <= 62.f) ||   // the entry window [0, L_c] of R1 is tested in one 64-cell word
         p.lookahead_cells < 1 || p.lookahead_cells > 8192 || p.lookback_cells < 1 || p.lookback_cells > 8192 ||
         !(p.mlc_scale_m >= 1.f) || !(p.mlc_scale_m <= 10000.f) || !(p.lc_alpha >= 0.f) || !(p.lc_eps_sigma >= 0.f) ||
         !std::isfinite(p.dlc_gain_thr) || !std::isfinite(p.lc_gap_low) || !std::isfinite(p.lc_gap_high))
@@ -232,7 +234,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         s->max_limit = std::max(s->max_limit, (double)lim);
         if (cells > 0xFFFFFFFFull) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "atlas exceeds 2^32 cells"));
         s->cell_off[e] = (uint32_t)cells;
-        cells += (uint64_t)(((uint32_t)lc + 15u) & ~15u) * net->lanes[e];
+        cells += (uint64_t)(((uint32_t)lc + 63u) & ~63u) * net->lanes[e];
     }
     if (cells + 256 > 0xFFFFFFFFull) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "atlas exceeds 2^32 cells"));
     s->n_cells = cells;
@@ -254,7 +256,6 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     P.Lam = std::max<uint32_t>(1u, (uint32_t)std::lround((double)p.mlc_scale_m));
     P.seed_lo = (uint32_t)p.seed; P.seed_hi = (uint32_t)(p.seed >> 32);
     P.n_edges = M; P.flags = p.flags;
-    if (p.lookahead_cells > 960u || p.lookback_cells > 960u) P.flags |= MANTA_FLAG_SCALAR_SCAN;   // chunk 'rel' field is 10 bits
 
     // ---- device tables
     std::vector<uint4> et(M);
@@ -275,7 +276,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         }
     }
     int rc;
-    uint4 *d_et; uint32_t *d_head, *d_pm, *d_ee; unsigned long long *d_claim; Counters *d_ctr; BlockStats *d_blk;
+    uint4 *d_et; uint32_t *d_head, *d_pm, *d_ee; u64 *d_claim; Counters *d_ctr; BlockStats *d_blk;
     if ((rc = upload(s, &d_et, et.data(), M))) return bail(rc);
     if ((rc = upload(s, &d_head, s->head.data(), M))) return bail(rc);
     if ((rc = upload(s, &d_pm, pm.data(), pm.size()))) return bail(rc);
@@ -284,10 +285,10 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     if ((rc = alloc_fill(s, &d_ctr, 1, 0))) return bail(rc);
     s->n_blk_stats = (uint32_t)s->sm_count * 16u;
     if ((rc = alloc_fill(s, &d_blk, s->n_blk_stats, 0))) return bail(rc);
-    for (int k = 0; k < 2; k++) {
-        if ((rc = alloc_fill(s, &P.occ[k], cells + 256, 0))) return bail(rc);
-        if ((rc = alloc_fill(s, &P.spd[k], cells + 256, 0))) return bail(rc);
-    }
+    for (int k = 0; k < 3; k++)
+        if ((rc = alloc_fill(s, &P.bits[k], cells / 64 + 8, 0))) return bail(rc);
+    for (int k = 0; k < 2; k++)
+        if ((rc = alloc_fill(s, &P.pay[k], cells + 64, 0))) return bail(rc);
     P.edge_tab = d_et; P.head = d_head; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
     P.blk = d_blk;
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(s, MANTA_ERR_CUDA, "upload failed: %s", cudaGetErrorString(cudaGetLastError())));
@@ -301,7 +302,8 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
     if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
     if (s->loaded) return fail(s, MANTA_ERR_STATE, "trips already loaded");
-    if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0) return fail(s, MANTA_ERR_INVALID_ARG, "null / empty trips");
+    if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0 || n_trips >= 0x7FFFFFFFu)
+        return fail(s, MANTA_ERR_INVALID_ARG, "null / empty / too many trips");
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint64_t total = route_ptr[n_trips];
     if (route_ptr[0] != 0 || total >= 0xFFFFFFFFull) return fail(s, MANTA_ERR_BAD_ROUTE, "route_ptr must start at 0 and stay below 2^32 entries");
@@ -416,22 +418,23 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
     const uint32_t cap = n_trips;
     for (int k = 0; k < 2; k++) {
-        P.A0[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
-        P.A1[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
+        P.S0[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
+        P.S1[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
         P.acc[k] = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, (uint64_t)cap * sizeof(float)) : nullptr;
-        if (!P.A0[k] || !P.A1[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+        if (!P.S0[k] || !P.S1[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
         if (P.acc[k]) CUDA_TRY(s, cudaMemsetAsync(P.acc[k], 0, (uint64_t)cap * sizeof(float), s->stream));
     }
-    P.N = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
-    if (!P.N) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+    P.xlist = (uint2 *)dev_alloc(s, (uint64_t)cap * sizeof(uint2));
+    if (!P.xlist) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
     P.route = d_route; P.depart_step = d_dep; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
     P.q_edge = d_qe; P.q_ptr = d_qp; P.q_ids = d_qi; P.q_head = d_qh;
     P.n_queues = (uint32_t)q_edge.size();
     P.cap = cap;
     const uint32_t n_init = (uint32_t)init_a0.size();
     if (n_init) {
-        CUDA_TRY(s, cudaMemcpyAsync(P.A0[0], init_a0.data(), (uint64_t)n_init * sizeof(uint4), cudaMemcpyHostToDevice, s->stream));
-        CUDA_TRY(s, cudaMemcpyAsync(&P.ctr->n_act[0], &n_init, sizeof(uint32_t), cudaMemcpyHostToDevice, s->stream));
+        const u64 fill0 = n_init;
+        CUDA_TRY(s, cudaMemcpyAsync(P.S0[0], init_a0.data(), (uint64_t)n_init * sizeof(uint4), cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(&P.ctr->fill[0], &fill0, sizeof(u64), cudaMemcpyHostToDevice, s->stream));
         k_place_initial<<<(n_init + 255) / 256, 256, 0, s->stream>>>(P, n_init);
         CUDA_TRY(s, cudaGetLastError());
     }
@@ -442,26 +445,64 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
-    const uint32_t max_blocks = std::min<uint32_t>(s->n_blk_stats, (uint32_t)s->sm_count * 8u);
-    s->grid_update = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + 255u) / 256u, max_blocks));
-    s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, max_blocks));
+    // launch geometry: grid-stride kernels sized to what is resident at once; the persistent kernel needs all of
+    // its blocks co-resident (cooperative launch)
+    int occ = 0, coop = 0;
+    CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent, MANTA_NT, 0));
+    CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
+    s->grid_persist = (coop && occ > 0) ? std::min<int>(s->sm_count * occ, (int)s->n_blk_stats) : 0;
+    const uint32_t max_upd = std::min<uint32_t>(s->n_blk_stats, (uint32_t)s->sm_count * 2u);
+    s->grid_update = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + MANTA_NT - 1u) / MANTA_NT, max_upd));
+    s->grid_cross = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + 255u) / 256u, (uint32_t)s->sm_count * 2u));
+    s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, (uint32_t)s->sm_count * 8u));
     return MANTA_OK;
 }
 
-int manta_step_async(manta_sim *s, uint32_t n_steps)
+namespace {
+
+int check_ready(manta_sim *s, uint32_t n_steps)
 {
     if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
     if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
     if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
     if ((uint64_t)s->t + n_steps >= 0xFFFFFFFEull) return fail(s, MANTA_ERR_INVALID_ARG, "step counter would overflow");
+    return MANTA_OK;
+}
+
+// three launches per timestep (MANTA_FLAG_MULTI_KERNEL, manta_step_timed, devices without cooperative launch)
+void launch_step_multi(manta_sim *s, uint32_t t, cudaEvent_t *ev)
+{
+    if (ev) cudaEventRecord(ev[0], s->stream);
+    k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
+    if (ev) cudaEventRecord(ev[1], s->stream);
+    k_update<<<s->grid_update, MANTA_NT, 0, s->stream>>>(s->P, t);
+    if (ev) cudaEventRecord(ev[2], s->stream);
+    k_cross<<<s->grid_cross, 256, 0, s->stream>>>(s->P, t);
+    if (ev) cudaEventRecord(ev[3], s->stream);
+    s->launches += 3;
+}
+
+}  // namespace
+
+int manta_step_async(manta_sim *s, uint32_t n_steps)
+{
+    int rc = check_ready(s, n_steps);
+    if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
-    for (uint32_t k = 0; k < n_steps; k++) {
-        const uint32_t t = s->t;
-        k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
-        k_update<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
-        k_commit<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
-        s->launches += 3;
-        s->t = t + 1;
+    if ((s->prm.flags & MANTA_FLAG_MULTI_KERNEL) || s->grid_persist == 0) {
+        for (uint32_t k = 0; k < n_steps; k++) launch_step_multi(s, s->t++, nullptr);
+    } else {
+        // one cooperative launch per chunk of timesteps; the grid barrier words restart from zero every launch
+        for (uint32_t done = 0; done < n_steps;) {
+            uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s->t;
+            CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 2 * sizeof(unsigned int), s->stream));
+            void *args[] = {(void *)&s->P, (void *)&t0, (void *)&m};
+            CUDA_TRY(s, cudaLaunchCooperativeKernel((const void *)k_persistent, dim3((unsigned)s->grid_persist), dim3(MANTA_NT),
+                                                    args, 0, s->stream));
+            s->launches += 1;
+            s->t += m;
+            done += m;
+        }
     }
     CUDA_TRY(s, cudaGetLastError());
     return MANTA_OK;
@@ -469,27 +510,16 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
 
 int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
 {
-    if (!s || !phase_ms) return fail(s, MANTA_ERR_INVALID_ARG, "null argument");
-    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
-    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    if (!phase_ms) return fail(s, MANTA_ERR_INVALID_ARG, "null argument");
+    int rc = check_ready(s, n_steps);
+    if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint32_t CH = 128;
     std::vector<cudaEvent_t> ev(4 * CH);
     for (auto &e : ev) CUDA_TRY(s, cudaEventCreate(&e));
     for (uint32_t done = 0; done < n_steps;) {
         const uint32_t m = std::min(CH, n_steps - done);
-        for (uint32_t k = 0; k < m; k++) {
-            const uint32_t t = s->t;
-            cudaEventRecord(ev[4 * k + 0], s->stream);
-            k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
-            cudaEventRecord(ev[4 * k + 1], s->stream);
-            k_update<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
-            cudaEventRecord(ev[4 * k + 2], s->stream);
-            k_commit<<<s->grid_update, 256, 0, s->stream>>>(s->P, t);
-            cudaEventRecord(ev[4 * k + 3], s->stream);
-            s->launches += 3;
-            s->t = t + 1;
-        }
+        for (uint32_t k = 0; k < m; k++) launch_step_multi(s, s->t++, &ev[4 * k]);
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
         for (uint32_t k = 0; k < m; k++)
             for (int ph = 0; ph < 3; ph++) {
@@ -508,6 +538,15 @@ int manta_sync(manta_sim *s)
     if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
     CUDA_TRY(s, cudaSetDevice(s->device));
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (s->loaded && s->grid_persist) {
+        unsigned int ab = 0;
+        CUDA_TRY(s, cudaMemcpyAsync(&ab, &s->P.ctr->abort, sizeof ab, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        if (ab) {
+            s->sticky_cuda = true;
+            return fail(s, MANTA_ERR_CUDA, "grid barrier of the persistent step kernel timed out");
+        }
+    }
     return MANTA_OK;
 }
 
@@ -587,13 +626,24 @@ int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell
     if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
     if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
     CUDA_TRY(s, cudaSetDevice(s->device));
-    const int cur = (int)(s->t & 1u);
-    if (occ) CUDA_TRY(s, cudaMemcpyAsync(occ, s->P.occ[cur], s->n_cells * 2, cudaMemcpyDeviceToHost, s->stream));
-    if (spd) CUDA_TRY(s, cudaMemcpyAsync(spd, s->P.spd[cur], s->n_cells * 4, cudaMemcpyDeviceToHost, s->stream));
-    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (occ || spd) {
+        // the logical atlas is rebuilt from the occupancy bits and the payload plane of the current step
+        const uint64_t n = s->n_cells;
+        uint8_t *buf = (uint8_t *)dev_alloc(s, n * 6 + 64);
+        if (!buf) return fail(s, MANTA_ERR_OOM, "atlas export scratch allocation failed");
+        float *d_spd = (float *)buf;
+        uint16_t *d_occ = (uint16_t *)(buf + n * 4);
+        k_export_atlas<<<(unsigned)std::min<uint64_t>((n + 255) / 256, 65535ull), 256, 0, s->stream>>>(
+            s->P.bits[s->t % 3u], s->P.pay[s->t & 1u], n, d_occ, d_spd);
+        CUDA_TRY(s, cudaGetLastError());
+        if (occ) CUDA_TRY(s, cudaMemcpyAsync(occ, d_occ, n * 2, cudaMemcpyDeviceToHost, s->stream));
+        if (spd) CUDA_TRY(s, cudaMemcpyAsync(spd, d_spd, n * 4, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        dev_free(s, buf);
+    }
     for (uint32_t e = 0; e < s->n_edges; e++) {
         if (cell_off) cell_off[e] = s->cell_off[e];
-        if (pitch) pitch[e] = (s->len_c[e] + 15u) & ~15u;
+        if (pitch) pitch[e] = (s->len_c[e] + 63u) & ~63u;
     }
     return MANTA_OK;
 }

@@ -9,24 +9,34 @@
 
 namespace manta {
 
+typedef unsigned long long u64;
+
 // ---------------------------------------------------------------------------------------------------------
 // Layout in HBM
 //
-// Atlas: plane occ[2] of u16 per 1 m cell (0 = empty, 1 + frac10 of the occupant's Q22.10
-// position) and plane spd[2] of fp32 (occupant's speed); buffer t&1 is read in step t, buffer (t+1)&1 written.
-// Row (edge e, lane l) starts at cell  cell_off[e] + l * pitch(e),  pitch = len_c rounded up to 16 cells, so
-// every row starts on a 32-byte sector and 16-byte vector loads never straddle rows.
+// Traffic atlas (one cell per metre of lane, at most one vehicle per cell, the cell records the
+// occupant's velocity), stored as two SoA planes over the same cell index:
+//   bits[3]  OCCUPANCY plane, 1 bit per 1 m cell, packed 64 cells per u64 word.  Buffer t % 3 holds the marks of
+//            time t: step t reads buffer t % 3, sets the time-(t+1) marks in buffer (t+1) % 3 and clears its own
+//            time-(t-1) marks in buffer (t+2) % 3, so a buffer is all-zero again when it is next written and no
+//            phase both reads and writes one buffer.  A 256-cell look-ahead is 4-5 words (one or two sectors).
+//   pay[2]   PAYLOAD plane, 8 bytes per cell: { frac10 of the occupant's Q22.10 position, its fp32 speed bits }.
+//            Buffer t & 1 is valid for the cells whose bit is set in bits[t % 3]; never cleared.
+// Row (edge e, lane l) starts at cell  cell_off[e] + l * pitch(e),  pitch = len_c rounded up to 64 cells, so every
+// row starts on a word boundary and no word is shared by two rows.
 //
 // Route store: one 16-byte RouteRec per route entry (edge attributes inlined, so following a route costs one
-// gather instead of route -> edge table):
+// gather instead of route -> edge table); consecutive entries of a trip are consecutive in memory:
 //   w0 cell_off   w1 geom   w2 edge id   w3 speed limit v0 (fp32 bits)
 // geom bits: 0-15 len_c | 16-19 lanes | 20-22 lo | 23-25 hi | 26 last | 27 head-node PRIORITY | 28-30 lane | 31 tag
-// (lane / tag are only meaningful in a vehicle's private copy of its current RouteRec).
+// (lane / tag are only meaningful in a vehicle's private copy).
 //
-// Active vehicles: compact double-buffered arrays of two uint4 per vehicle (32 bytes, one sector):
-//   A0 = { x_fx, v bits, vehicle id, route cursor (absolute RouteRec index) }     A1 = current RouteRec copy
-// plus a 16-byte tentative next state N written by the update phase and consumed by the commit phase:
-//   N  = { x', v' bits, meta (kind | lane' << 2 | tag' << 5), claim word index }
+// Active vehicles: compact double-buffered arrays of two uint4 per vehicle (32 bytes, one sector); the update
+// phase reads buffer t & 1 and writes the survivors, compacted, to buffer (t+1) & 1:
+//   S0 = { x_fx, v bits, vehicle id, route cursor (absolute RouteRec index) }
+//   S1 = { cell_off, geom (+ lane, tag), absolute cell of the time-(t-1) mark or NONE, v0 bits }
+// Cross list: 8-byte entries made by the update phase for the few vehicles that need the second phase
+// (edge-end candidates, whose claim must be resolved, and arrivals, whose time-t mark must be cleared).
 // ---------------------------------------------------------------------------------------------------------
 
 #define GEOM_LEN(g) ((g) & 0xFFFFu)
@@ -38,20 +48,21 @@ namespace manta {
 #define GEOM_LANE(g) (((g) >> 28) & 7u)
 #define GEOM_TAG(g) ((g) >> 31)
 #define GEOM_STATIC_MASK 0x0FFFFFFFu
+#define CELL_NONE 0xFFFFFFFFu
+#define XL_DONE 0x80000000u
 
 enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
 
 struct Counters {
-    unsigned int n_act[2];               // active-array fill of buffer 0 / 1
-    unsigned int pad[2];
-    unsigned long long n_done, sum_travel, n_updates;
+    u64 fill[2];                         // low 32 bits: fill of active buffer k; high 32: cross-list entries made while filling it
+    u64 n_done, sum_travel, n_updates;
     unsigned int bar_count, bar_gen;     // grid barrier of the persistent kernel
-    unsigned int t_dev, pad2;
+    unsigned int abort, pad;
 };
 
 // per-block private statistics (no atomics on the hot path; summed at readback)
 struct BlockStats {
-    unsigned long long lane_changes, cells_examined, lc_evals, pad;
+    u64 lane_changes, cells_examined, lc_evals, pad;
 };
 
 struct DevP {
@@ -66,14 +77,14 @@ struct DevP {
     const uint4 *edge_tab;       // per edge: {cell_off, geom (len | lanes | PRIORITY bit), head node, v0 bits}
     const uint32_t *head;        // head node per edge (PRIORITY claims only)
     // atlas
-    uint16_t *occ[2];
-    float *spd[2];
+    u64 *bits[3];
+    uint2 *pay[2];
     // routes
     const uint4 *route;
     // vehicles
-    uint4 *A0[2];
-    uint4 *A1[2];
-    uint4 *N;
+    uint4 *S0[2];
+    uint4 *S1[2];
+    uint2 *xlist;                // cross list: {XL_DONE, cell to clear} or {position in the next buffer, claim word}
     float *acc[2];               // optional (MANTA_FLAG_RECORD_ACC): acceleration applied in the last step
     // per vehicle id
     const uint32_t *depart_step;
@@ -86,14 +97,14 @@ struct DevP {
     const uint32_t *q_ids;
     uint32_t *q_head;
     // claims, counters, tables
-    unsigned long long *claim;   // [n_edges * 8 + n_nodes]
+    u64 *claim;                  // [n_edges * 8 + n_nodes]
     uint32_t *edge_entries;
     const uint32_t *P_mlc;       // [5 * Lam + 1]
     Counters *ctr;
     BlockStats *blk;
 };
 
-__device__ __forceinline__ uint32_t pitch_of(uint32_t len_c) { return (len_c + 15u) & ~15u; }
+__device__ __forceinline__ uint32_t pitch_of(uint32_t len_c) { return (len_c + 63u) & ~63u; }
 
 // ------------------------------------------------------------------------------------------- G22: rng(id, t, k)
 __device__ __forceinline__ uint32_t mix32(uint32_t h)
@@ -154,61 +165,53 @@ __device__ __forceinline__ float idm_acc(const DevP &P, float v, float v0, bool 
 }
 
 // ------------------------------------------------------------------------------------------- atlas row scans
-// 8 cells (16 bytes) per load; rows are 16-cell aligned so an 8-aligned group never leaves the row's padding.
-__device__ __forceinline__ uint32_t nzmask8(const uint4 &w)
+// "Looking up the status of neighboring cells" on the occupancy plane: 64 cells per load, the word
+// after the current one is requested before the current one is examined.
+__device__ __forceinline__ u64 bits_below(uint32_t n) { return n >= 64u ? ~0ull : ((1ull << n) - 1ull); }  // n in 1..64
+
+// first occupied cell j in [start, end) of the row whose cell 0 is absolute cell `row`; requires start < end
+__device__ __forceinline__ bool first_set(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
 {
-    uint32_t m = 0;
-    m |= (w.x & 0xFFFFu) ? 1u : 0u;
-    m |= (w.x >> 16) ? 2u : 0u;
-    m |= (w.y & 0xFFFFu) ? 4u : 0u;
-    m |= (w.y >> 16) ? 8u : 0u;
-    m |= (w.z & 0xFFFFu) ? 16u : 0u;
-    m |= (w.z >> 16) ? 32u : 0u;
-    m |= (w.w & 0xFFFFu) ? 64u : 0u;
-    m |= (w.w >> 16) ? 128u : 0u;
-    return m;
-}
-__device__ __forceinline__ uint32_t code_at(const uint4 &w, uint32_t i)
-{
-    uint32_t word = (i & 4u) ? ((i & 2u) ? w.w : w.z) : ((i & 2u) ? w.y : w.x);
-    return (i & 1u) ? (word >> 16) : (word & 0xFFFFu);
-}
-// first occupied cell j in [start, end) of the row starting at absolute cell `row`; returns false if none
-__device__ __forceinline__ bool scan_fwd(const uint16_t *occ, uint32_t row, uint32_t start, uint32_t end, uint32_t &j,
-                                         uint32_t &code)
-{
-    for (uint32_t base = start & ~7u; base < end; base += 8u) {
-        uint4 w = *reinterpret_cast<const uint4 *>(occ + (size_t)row + base);
-        uint32_t m = nzmask8(w);
-        if (start > base) m &= 0xFFu << (start - base);
-        if (end - base < 8u) m &= (1u << (end - base)) - 1u;
+    const u64 *p = B + (row >> 6);
+    uint32_t w = start >> 6;
+    const uint32_t wl = (end - 1u) >> 6;
+    u64 m = p[w];
+    u64 m_next = (w < wl) ? p[w + 1u] : 0ull;
+    m &= ~0ull << (start & 63u);
+    for (;;) {
+        if (w == wl) m &= bits_below(end - (w << 6));
         if (m) {
-            uint32_t i = (uint32_t)__ffs((int)m) - 1u;
-            j = base + i;
-            code = code_at(w, i);
+            j = (w << 6) + (uint32_t)__ffsll((long long)m) - 1u;
             return true;
         }
+        if (w == wl) return false;
+        ++w;
+        m = m_next;
+        m_next = (w < wl) ? p[w + 1u] : 0ull;
     }
-    return false;
 }
-// last occupied cell j in [start, end)
-__device__ __forceinline__ bool scan_bwd(const uint16_t *occ, uint32_t row, uint32_t start, uint32_t end, uint32_t &j,
-                                         uint32_t &code)
+// last occupied cell j in [start, end); requires start < end
+__device__ __forceinline__ bool last_set(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
 {
-    if (end <= start) return false;
-    for (int base = (int)((end - 1u) & ~7u); base + 8 > (int)start; base -= 8) {
-        uint4 w = *reinterpret_cast<const uint4 *>(occ + (size_t)row + (uint32_t)base);
-        uint32_t m = nzmask8(w);
-        if ((int)start > base) m &= 0xFFu << (start - (uint32_t)base);
-        if (end - (uint32_t)base < 8u) m &= (1u << (end - (uint32_t)base)) - 1u;
+    const u64 *p = B + (row >> 6);
+    uint32_t w = (end - 1u) >> 6;
+    const uint32_t w0 = start >> 6;
+    u64 m = p[w];
+    u64 m_next = (w > w0) ? p[w - 1u] : 0ull;
+    m &= bits_below(end - (w << 6));
+    for (;;) {
+        if (w == w0) m &= ~0ull << (start & 63u);
         if (m) {
-            uint32_t i = 31u - (uint32_t)__clz((int)m);
-            j = (uint32_t)base + i;
-            code = code_at(w, i);
+            j = (w << 6) + 63u - (uint32_t)__clzll((long long)m);
             return true;
         }
+        if (w == w0) return false;
+        --w;
+        m = m_next;
+        m_next = (w > w0) ? p[w - 1u] : 0ull;
     }
-    return false;
 }
+__device__ __forceinline__ void mark_set(u64 *B, uint32_t cell) { atomicOr(&B[cell >> 6], 1ull << (cell & 63u)); }
+__device__ __forceinline__ void mark_clear(u64 *B, uint32_t cell) { atomicAnd(&B[cell >> 6], ~(1ull << (cell & 63u))); }
 
 }  // namespace manta

@@ -88,7 +88,7 @@ def test_exports(binding):
         assert hasattr(L, name)
 
 
-FLAGS = [0, 1]   # default (warp-cooperative scan) and MANTA_FLAG_SCALAR_SCAN
+FLAGS = [0, 2]   # default (one persistent cooperative kernel per manta_step) and MANTA_FLAG_MULTI_KERNEL
 
 
 @pytest.mark.parametrize("flags", FLAGS)
