@@ -116,6 +116,16 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def algorithmic_bytes(hbar, flc, lookback):
+    """Algorithmic bytes per vehicle-update of the 1-bit-occupancy layout.
+    update phase: state read 32 + compacted state write 32, next route record 16, own-lane occupancy bits
+    hbar / 8, leader payload 8, new mark (8-byte word) 8 + payload 8, clearing of the old mark 8; a lane-change
+    evaluation adds the target row's bits ahead and behind plus two payloads.  The whole step adds the cross
+    list entry and the second state pass of the ~2 % of vehicles at an edge end (folded in as 2 B)."""
+    upd = 32.0 + 32.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0 + flc * ((hbar + lookback) / 8.0 + 16.0)
+    return upd, upd + 2.0
+
+
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
     """Bounded sample of the same workload for the CPU oracle: the first n_sample_trips trips departing at or
     after start_step, their departures shifted so the earliest leaves at t = 0; run n_steps timesteps."""
@@ -257,8 +267,7 @@ def main():
     hbar = d["cells_examined"] / max(1, d["vehicle_updates"])
     flc = d["lc_evals"] / max(1, d["vehicle_updates"])
     # algorithmic bytes per vehicle-update: whole step, and the update phase alone
-    bytes_step = 80.0 + 2.0 * hbar * (1.0 + flc) + 136.0 * flc
-    bytes_update = 52.0 + 2.0 * hbar * (1.0 + flc) + 136.0 * flc
+    bytes_update, bytes_step = algorithmic_bytes(hbar, flc, params.get("lookback_cells", 64))
     peak, peak_src = measured_peak()
     upd_per_launch = d["vehicle_updates"] / Kp
     t_update = ph[1] / Kp * 1e-3
