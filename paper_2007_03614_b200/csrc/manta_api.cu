@@ -51,9 +51,9 @@ struct manta_sim {
     uint32_t *d_trip_of_id = nullptr;
     uint32_t t = 0;
     int sm_count = 148;
-    int grid_update = 1, grid_admit = 1, grid_cross = 1, grid_persist = 0;
+    int grid_step = 1, grid_admit = 1, grid_persist = 0;   // blocks of the segment kernels / admission / persistent kernel
+    bool w256 = true;             // look-ahead <= 256 cells and look-back <= 128: whole-window scans
     uint32_t n_blk_stats = 0;
-    uint32_t n_active_hint = 0;   // active count seen by the last readback (sizes the cross-phase launch)
 };
 
 namespace {
@@ -276,20 +276,19 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         }
     }
     int rc;
-    uint4 *d_et; uint32_t *d_head, *d_pm, *d_ee; u64 *d_claim; Counters *d_ctr; BlockStats *d_blk;
+    uint4 *d_et; uint32_t *d_pm, *d_ee; u64 *d_claim; Counters *d_ctr; BlockStats *d_blk;
     if ((rc = upload(s, &d_et, et.data(), M))) return bail(rc);
-    if ((rc = upload(s, &d_head, s->head.data(), M))) return bail(rc);
     if ((rc = upload(s, &d_pm, pm.data(), pm.size()))) return bail(rc);
     if ((rc = alloc_fill(s, &d_ee, M, 0))) return bail(rc);
     if ((rc = alloc_fill(s, &d_claim, (uint64_t)M * 8 + N, 0xFF))) return bail(rc);
     if ((rc = alloc_fill(s, &d_ctr, 1, 0))) return bail(rc);
     s->n_blk_stats = (uint32_t)s->sm_count * 16u;
     if ((rc = alloc_fill(s, &d_blk, s->n_blk_stats, 0))) return bail(rc);
-    for (int k = 0; k < 3; k++)
+    for (int k = 0; k < 2; k++)
         if ((rc = alloc_fill(s, &P.bits[k], cells / 64 + 8, 0))) return bail(rc);
     for (int k = 0; k < 2; k++)
         if ((rc = alloc_fill(s, &P.pay[k], cells + 64, 0))) return bail(rc);
-    P.edge_tab = d_et; P.head = d_head; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
+    P.edge_tab = d_et; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
     P.blk = d_blk;
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(s, MANTA_ERR_CUDA, "upload failed: %s", cudaGetErrorString(cudaGetLastError())));
     *out = s;
@@ -370,7 +369,9 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
                 return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "pre-placed vehicles closer than L on edge %llu", (unsigned long long)(keyx[k].first >> 32)));
     }
     // ---- admission FIFOs: waiting trips grouped by first edge, id order inside (G25)
-    std::vector<uint32_t> q_edge, q_ptr, q_ids;
+    // q_ent = {vehicle id, depart_step, route_start, depart_step of the next entry of the same queue or NONE}
+    std::vector<uint32_t> q_edge, q_ptr, q_next;
+    std::vector<uint4> q_ent, q_row;
     {
         std::vector<uint32_t> cnt(s->n_edges + 1, 0);
         for (uint32_t id = 0; id < n_trips; id++) {
@@ -379,64 +380,91 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
             cnt[route_edges[route_ptr[tr]] + 1]++;
         }
         for (uint32_t e = 0; e < s->n_edges; e++) cnt[e + 1] += cnt[e];
-        q_ids.resize(cnt[s->n_edges]);
+        q_ent.resize((size_t)cnt[s->n_edges] + 1);
         std::vector<uint32_t> fill(cnt.begin(), cnt.end() - 1);
         for (uint32_t id = 0; id < n_trips; id++) {
             const uint32_t tr = trip_of_id[id];
             if (init_pos_m && init_pos_m[tr] >= 0.0f) continue;
-            q_ids[fill[route_edges[route_ptr[tr]]]++] = id;
+            q_ent[fill[route_edges[route_ptr[tr]]]++] = make_uint4(id, depart_by_id[id], route_start[id], MANTA_NONE);
         }
         for (uint32_t e = 0; e < s->n_edges; e++)
             if (cnt[e + 1] > cnt[e]) {
                 q_edge.push_back(e);
                 q_ptr.push_back(cnt[e]);
+                q_next.push_back(q_ent[cnt[e]].y);
+                for (uint32_t k = cnt[e]; k + 1 < cnt[e + 1]; k++) q_ent[k].w = q_ent[k + 1].y;
             }
         q_ptr.push_back(cnt[s->n_edges]);
     }
-    // ---- upload; expand the route store on the device
+    // ---- launch geometry and vehicle segments.  A segment is processed by one block per phase; the persistent
+    // kernel needs all of its blocks co-resident (cooperative launch), so n_seg = that grid.
+    s->w256 = s->prm.lookahead_cells <= 256u && s->prm.lookback_cells <= 128u;
+    {
+        int occ = 0, coop = 0;
+        if (s->w256)
+            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<true>, MANTA_NT, 0));
+        else
+            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<false>, MANTA_NT, 0));
+        CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
+        s->grid_persist = (coop && occ > 0) ? std::min<int>(s->sm_count * occ, (int)s->n_blk_stats) : 0;
+        s->grid_step = s->grid_persist ? s->grid_persist : std::min<int>(s->sm_count * 2, (int)s->n_blk_stats);
+    }
     DevP &P = s->P;
+    P.n_seg = (uint32_t)s->grid_step;
+    P.seg_cap = (n_trips + P.n_seg - 1u) / P.n_seg + 64u;
+    const uint64_t cap = (uint64_t)P.n_seg * P.seg_cap;
+    if (cap >= 0xFFFFFFFFull) return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
+    // ---- upload; expand the route store on the device
     int rc;
-    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_dep, *d_rs, *d_adm, *d_arr, *d_qe, *d_qp, *d_qi, *d_qh;
+    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qh, *d_qn;
     uint64_t *d_rp = nullptr;
-    uint4 *d_route;
+    uint4 *d_route, *d_qent, *d_qrow;
+    for (size_t k = 0; k < q_edge.size(); k++) {
+        const uint32_t e = q_edge[k];
+        q_row.push_back(make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16), e, 0u));
+    }
     if ((rc = upload(s, &d_re, route_edges, total))) return rollback(rc);
     if ((rc = upload(s, &d_rp, route_ptr, (uint64_t)n_trips + 1))) return rollback(rc);
     if ((rc = upload(s, &d_rowptr, s->row_ptr.data(), s->row_ptr.size()))) return rollback(rc);
-    d_route = (uint4 *)dev_alloc(s, (total + 1) * sizeof(uint4));
+    d_route = (uint4 *)dev_alloc(s, (total + 8) * sizeof(uint4));   // + 8: the look-ahead requests four records ahead
     if (!d_route) return rollback(fail(s, MANTA_ERR_OOM, "route store allocation failed"));
+    CUDA_TRY(s, cudaMemsetAsync(d_route + total, 0, 8 * sizeof(uint4), s->stream));
     k_expand_routes<<<(unsigned)std::min<uint64_t>((total + 255) / 256, 65535ull * 16), 256, 0, s->stream>>>(P.edge_tab, d_rowptr, d_re, total, d_route);
     k_mark_last<<<(n_trips + 255) / 256, 256, 0, s->stream>>>(d_rp, n_trips, d_route);
     CUDA_TRY(s, cudaGetLastError());
-    if ((rc = upload(s, &d_dep, depart_by_id.data(), n_trips))) return rollback(rc);
     if ((rc = upload(s, &d_rs, route_start.data(), n_trips))) return rollback(rc);
     if ((rc = upload(s, &s->d_trip_of_id, trip_of_id.data(), n_trips))) return rollback(rc);
     if ((rc = alloc_fill(s, &d_adm, n_trips, 0xFF))) return rollback(rc);
     if ((rc = alloc_fill(s, &d_arr, n_trips, 0xFF))) return rollback(rc);
-    if ((rc = upload(s, &d_qe, q_edge.data(), q_edge.size()))) return rollback(rc);
-    if ((rc = upload(s, &d_qp, q_ptr.data(), q_ptr.size()))) return rollback(rc);
-    if ((rc = upload(s, &d_qi, q_ids.data(), q_ids.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qrow, q_row.data(), q_row.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qent, q_ent.data(), q_ent.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
-    const uint32_t cap = n_trips;
+    if ((rc = upload(s, &d_qn, q_next.data(), q_next.size()))) return rollback(rc);
     for (int k = 0; k < 2; k++) {
-        P.S0[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
-        P.S1[k] = (uint4 *)dev_alloc(s, (uint64_t)cap * sizeof(uint4));
-        P.acc[k] = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, (uint64_t)cap * sizeof(float)) : nullptr;
+        P.S0[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
+        P.S1[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
+        P.acc[k] = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, cap * sizeof(float)) : nullptr;
         if (!P.S0[k] || !P.S1[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
-        if (P.acc[k]) CUDA_TRY(s, cudaMemsetAsync(P.acc[k], 0, (uint64_t)cap * sizeof(float), s->stream));
+        if (P.acc[k]) CUDA_TRY(s, cudaMemsetAsync(P.acc[k], 0, cap * sizeof(float), s->stream));
+        if ((rc = alloc_fill(s, &P.seg_cnt[k], P.n_seg, 0))) return rollback(rc);
     }
-    P.xlist = (uint2 *)dev_alloc(s, (uint64_t)cap * sizeof(uint2));
+    if ((rc = alloc_fill(s, &P.seg_xn, P.n_seg, 0))) return rollback(rc);
+    P.xlist = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
     if (!P.xlist) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
-    P.route = d_route; P.depart_step = d_dep; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
-    P.q_edge = d_qe; P.q_ptr = d_qp; P.q_ids = d_qi; P.q_head = d_qh;
+    P.route = d_route; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
+    P.q_row = d_qrow; P.q_ent = d_qent; P.q_head = d_qh; P.q_next = d_qn; P.q_ptr = nullptr;
     P.n_queues = (uint32_t)q_edge.size();
-    P.cap = cap;
     const uint32_t n_init = (uint32_t)init_a0.size();
     if (n_init) {
-        const u64 fill0 = n_init;
-        CUDA_TRY(s, cudaMemcpyAsync(P.S0[0], init_a0.data(), (uint64_t)n_init * sizeof(uint4), cudaMemcpyHostToDevice, s->stream));
-        CUDA_TRY(s, cudaMemcpyAsync(&P.ctr->fill[0], &fill0, sizeof(u64), cudaMemcpyHostToDevice, s->stream));
-        k_place_initial<<<(n_init + 255) / 256, 256, 0, s->stream>>>(P, n_init);
+        uint4 *d_init;
+        if ((rc = upload(s, &d_init, init_a0.data(), n_init))) return rollback(rc);
+        std::vector<uint32_t> cnt0(P.n_seg);
+        for (uint32_t k = 0; k < P.n_seg; k++) cnt0[k] = n_init / P.n_seg + (k < n_init % P.n_seg ? 1u : 0u);
+        CUDA_TRY(s, cudaMemcpyAsync(P.seg_cnt[0], cnt0.data(), (uint64_t)P.n_seg * 4, cudaMemcpyHostToDevice, s->stream));
+        k_place_initial<<<(n_init + 255) / 256, 256, 0, s->stream>>>(P, d_init, n_init);
         CUDA_TRY(s, cudaGetLastError());
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        dev_free(s, d_init);
     }
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     dev_free(s, d_re);
@@ -445,15 +473,6 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
-    // launch geometry: grid-stride kernels sized to what is resident at once; the persistent kernel needs all of
-    // its blocks co-resident (cooperative launch)
-    int occ = 0, coop = 0;
-    CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent, MANTA_NT, 0));
-    CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
-    s->grid_persist = (coop && occ > 0) ? std::min<int>(s->sm_count * occ, (int)s->n_blk_stats) : 0;
-    const uint32_t max_upd = std::min<uint32_t>(s->n_blk_stats, (uint32_t)s->sm_count * 2u);
-    s->grid_update = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + MANTA_NT - 1u) / MANTA_NT, max_upd));
-    s->grid_cross = (int)std::max<uint32_t>(1u, std::min<uint32_t>((cap + 255u) / 256u, (uint32_t)s->sm_count * 2u));
     s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, (uint32_t)s->sm_count * 8u));
     return MANTA_OK;
 }
@@ -475,9 +494,12 @@ void launch_step_multi(manta_sim *s, uint32_t t, cudaEvent_t *ev)
     if (ev) cudaEventRecord(ev[0], s->stream);
     k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
     if (ev) cudaEventRecord(ev[1], s->stream);
-    k_update<<<s->grid_update, MANTA_NT, 0, s->stream>>>(s->P, t);
+    if (s->w256)
+        k_update<true><<<s->grid_step, MANTA_NT, 0, s->stream>>>(s->P, t);
+    else
+        k_update<false><<<s->grid_step, MANTA_NT, 0, s->stream>>>(s->P, t);
     if (ev) cudaEventRecord(ev[2], s->stream);
-    k_cross<<<s->grid_cross, 256, 0, s->stream>>>(s->P, t);
+    k_cross<<<s->grid_step, 256, 0, s->stream>>>(s->P, t);
     if (ev) cudaEventRecord(ev[3], s->stream);
     s->launches += 3;
 }
@@ -497,8 +519,8 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
             uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s->t;
             CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 2 * sizeof(unsigned int), s->stream));
             void *args[] = {(void *)&s->P, (void *)&t0, (void *)&m};
-            CUDA_TRY(s, cudaLaunchCooperativeKernel((const void *)k_persistent, dim3((unsigned)s->grid_persist), dim3(MANTA_NT),
-                                                    args, 0, s->stream));
+            const void *fn = s->w256 ? (const void *)k_persistent<true> : (const void *)k_persistent<false>;
+            CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3((unsigned)s->grid_persist), dim3(MANTA_NT), args, 0, s->stream));
             s->launches += 1;
             s->t += m;
             done += m;
@@ -565,9 +587,6 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint32_t n = s->n_trips;
     const int cur = (int)(s->t & 1u);
-    Counters c;
-    CUDA_TRY(s, cudaMemcpyAsync(&c, s->P.ctr, sizeof c, cudaMemcpyDeviceToHost, s->stream));
-    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     if (edge_entries)
         CUDA_TRY(s, cudaMemcpyAsync(edge_entries, s->P.edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyDeviceToHost, s->stream));
     if (st || trips || sum) {
@@ -582,7 +601,7 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
         CUDA_TRY(s, cudaMemsetAsync(buf, 0, nn * (3 + 16 + 8), s->stream));
         const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
         k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
-        k_gather_state<<<g, 256, 0, s->stream>>>(s->P, cur, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
+        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, cur, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
         CUDA_TRY(s, cudaGetLastError());
         std::vector<uint8_t> h_status(n);
         CUDA_TRY(s, cudaMemcpyAsync(h_status.data(), d_status, n, cudaMemcpyDeviceToHost, s->stream));
@@ -607,13 +626,13 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
                 sum->n_active += h_status[i] == MANTA_ACTIVE;
             }
             sum->t = s->t;
-            sum->n_done = c.n_done;
-            sum->sum_travel_steps = c.sum_travel;
-            sum->vehicle_updates = c.n_updates;
             for (const BlockStats &b : bs) {
                 sum->lane_changes += b.lane_changes;
                 sum->cells_examined += b.cells_examined;
                 sum->lc_evals += b.lc_evals;
+                sum->n_done += b.n_done;
+                sum->sum_travel_steps += b.sum_travel;
+                sum->vehicle_updates += b.n_updates;
             }
         }
     }
@@ -634,7 +653,7 @@ int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell
         float *d_spd = (float *)buf;
         uint16_t *d_occ = (uint16_t *)(buf + n * 4);
         k_export_atlas<<<(unsigned)std::min<uint64_t>((n + 255) / 256, 65535ull), 256, 0, s->stream>>>(
-            s->P.bits[s->t % 3u], s->P.pay[s->t & 1u], n, d_occ, d_spd);
+            s->P.bits[s->t & 1u], s->P.pay[s->t & 1u], n, d_occ, d_spd);
         CUDA_TRY(s, cudaGetLastError());
         if (occ) CUDA_TRY(s, cudaMemcpyAsync(occ, d_occ, n * 2, cudaMemcpyDeviceToHost, s->stream));
         if (spd) CUDA_TRY(s, cudaMemcpyAsync(spd, d_spd, n * 4, cudaMemcpyDeviceToHost, s->stream));

@@ -16,27 +16,33 @@ typedef unsigned long long u64;
 //
 // Traffic atlas (one cell per metre of lane, at most one vehicle per cell, the cell records the
 // occupant's velocity), stored as two SoA planes over the same cell index:
-//   bits[3]  OCCUPANCY plane, 1 bit per 1 m cell, packed 64 cells per u64 word.  Buffer t % 3 holds the marks of
-//            time t: step t reads buffer t % 3, sets the time-(t+1) marks in buffer (t+1) % 3 and clears its own
-//            time-(t-1) marks in buffer (t+2) % 3, so a buffer is all-zero again when it is next written and no
-//            phase both reads and writes one buffer.  A 256-cell look-ahead is 4-5 words (one or two sectors).
+//   bits[2]  OCCUPANCY plane, 1 bit per 1 m cell, packed 64 cells per u64 word.  Buffer t & 1 holds the marks of
+//            time t.  Step t reads buffer t & 1 and turns buffer (t+1) & 1 -- which still holds the marks of time
+//            t-1 -- into the marks of time t+1 with XOR toggles: every vehicle toggles its own time-(t-1) mark off
+//            and its time-(t+1) mark on.  XOR commutes, so a cell that one vehicle leaves and another enters in
+//            the same step ends up set whatever the order, and a vehicle whose old and new mark share a word
+//            issues ONE atomic (none at all if it did not change cell).  No phase reads and writes one buffer.
+//            A 256-cell look-ahead is 4-5 words (one or two sectors).
 //   pay[2]   PAYLOAD plane, 8 bytes per cell: { frac10 of the occupant's Q22.10 position, its fp32 speed bits }.
-//            Buffer t & 1 is valid for the cells whose bit is set in bits[t % 3]; never cleared.
+//            Buffer t & 1 is valid for the cells whose bit is set in bits[t & 1]; never cleared.
 // Row (edge e, lane l) starts at cell  cell_off[e] + l * pitch(e),  pitch = len_c rounded up to 64 cells, so every
 // row starts on a word boundary and no word is shared by two rows.
 //
 // Route store: one 16-byte RouteRec per route entry (edge attributes inlined, so following a route costs one
-// gather instead of route -> edge table); consecutive entries of a trip are consecutive in memory:
+// gather instead of route -> edge table); consecutive entries of a trip are consecutive in memory, so the next
+// four records of a vehicle are one or two sectors:
 //   w0 cell_off   w1 geom   w2 edge id   w3 speed limit v0 (fp32 bits)
 // geom bits: 0-15 len_c | 16-19 lanes | 20-22 lo | 23-25 hi | 26 last | 27 head-node PRIORITY | 28-30 lane | 31 tag
 // (lane / tag are only meaningful in a vehicle's private copy).
 //
-// Active vehicles: compact double-buffered arrays of two uint4 per vehicle (32 bytes, one sector); the update
-// phase reads buffer t & 1 and writes the survivors, compacted, to buffer (t+1) & 1:
+// Active vehicles: n_seg SEGMENTS of seg_cap slots, two uint4 per vehicle (32 bytes, one sector), double-buffered.
+// A segment is processed by one thread block per phase, so survivor compaction needs only shared-memory atomics:
+// the update phase reads segment s of buffer t & 1 and writes its survivors, compacted, to segment s of buffer
+// (t+1) & 1.  A vehicle stays in the segment it was admitted to (admission picks the emptier of two segments).
 //   S0 = { x_fx, v bits, vehicle id, route cursor (absolute RouteRec index) }
 //   S1 = { cell_off, geom (+ lane, tag), absolute cell of the time-(t-1) mark or NONE, v0 bits }
-// Cross list: 8-byte entries made by the update phase for the few vehicles that need the second phase
-// (edge-end candidates, whose claim must be resolved, and arrivals, whose time-t mark must be cleared).
+// Cross list (per segment): 16-byte entries made by the update phase for the few vehicles that need the second
+// phase (edge-end candidates, whose claim must be resolved, and arrivals, whose time-t mark must be cleared).
 // ---------------------------------------------------------------------------------------------------------
 
 #define GEOM_LEN(g) ((g) & 0xFFFFu)
@@ -54,15 +60,22 @@ typedef unsigned long long u64;
 enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
 
 struct Counters {
-    u64 fill[2];                         // low 32 bits: fill of active buffer k; high 32: cross-list entries made while filling it
-    u64 n_done, sum_travel, n_updates;
     unsigned int bar_count, bar_gen;     // grid barrier of the persistent kernel
     unsigned int abort, pad;
 };
 
-// per-block private statistics (no atomics on the hot path; summed at readback)
+// per-block private statistics and result counters (no global atomics on the hot path; summed at readback)
 struct BlockStats {
-    u64 lane_changes, cells_examined, lc_evals, pad;
+    u64 lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel, pad0, pad1;
+};
+
+// entry of the lane-change queue in shared memory (update phase, second pass)
+struct LcEntry {
+    uint4 s0, s1;
+    int32_t lead_abs;       // own-lane leader (R2) found by the first pass
+    uint32_t v_lead_bits;
+    uint32_t found;
+    uint32_t pad;
 };
 
 struct DevP {
@@ -72,30 +85,32 @@ struct DevP {
     uint32_t H, lookback, L_c, Z_out, Z_in, Lam;
     int32_t L_fx;
     uint32_t seed_lo, seed_hi;
-    uint32_t n_edges, n_queues, flags, cap;
+    uint32_t n_edges, n_queues, flags;
+    uint32_t n_seg, seg_cap;     // active-vehicle segments
     // network
     const uint4 *edge_tab;       // per edge: {cell_off, geom (len | lanes | PRIORITY bit), head node, v0 bits}
-    const uint32_t *head;        // head node per edge (PRIORITY claims only)
     // atlas
-    u64 *bits[3];
+    u64 *bits[2];
     uint2 *pay[2];
     // routes
     const uint4 *route;
-    // vehicles
+    // vehicles: segment s occupies slots [s * seg_cap, s * seg_cap + seg_cnt[k][s]) of buffer k
     uint4 *S0[2];
     uint4 *S1[2];
-    uint2 *xlist;                // cross list: {XL_DONE, cell to clear} or {position in the next buffer, claim word}
+    uint32_t *seg_cnt[2];
+    uint4 *xlist;                // cross list of segment s at [s * seg_cap, ...): {slot | XL_DONE, claim word | cell, cursor, id}
+    uint32_t *seg_xn;            // cross-list entries of each segment (written by the update phase)
     float *acc[2];               // optional (MANTA_FLAG_RECORD_ACC): acceleration applied in the last step
     // per vehicle id
-    const uint32_t *depart_step;
     const uint32_t *route_start;
     uint32_t *admit_step;
     uint32_t *arrive_step;
-    // admission queues: one FIFO per origin edge (reading G25)
-    const uint32_t *q_edge;
-    const uint32_t *q_ptr;
-    const uint32_t *q_ids;
-    uint32_t *q_head;
+    // admission queues: one FIFO per origin edge (reading G25), entries in vehicle-id order
+    const uint4 *q_row;          // [n_queues] edge_tab record of the origin edge
+    const uint32_t *q_ptr;       // [n_queues + 1]
+    const uint4 *q_ent;          // [waiting trips] {vehicle id, depart_step, route_start, edge id}
+    uint32_t *q_head;            // [n_queues]
+    uint32_t *q_next;            // [n_queues] depart_step of the head entry (NONE when the queue is exhausted)
     // claims, counters, tables
     u64 *claim;                  // [n_edges * 8 + n_nodes]
     uint32_t *edge_entries;
@@ -211,7 +226,62 @@ __device__ __forceinline__ bool last_set(const u64 *B, uint32_t row, uint32_t st
         m_next = (w > w0) ? p[w - 1u] : 0ull;
     }
 }
-__device__ __forceinline__ void mark_set(u64 *B, uint32_t cell) { atomicOr(&B[cell >> 6], 1ull << (cell & 63u)); }
-__device__ __forceinline__ void mark_clear(u64 *B, uint32_t cell) { atomicAnd(&B[cell >> 6], ~(1ull << (cell & 63u))); }
+// Marks are XOR toggles (see the layout comment): setting a clear bit and clearing a set bit are the same operation.
+__device__ __forceinline__ void mark_toggle(u64 *B, uint32_t cell) { atomicXor(&B[cell >> 6], 1ull << (cell & 63u)); }
+// a vehicle's old mark off and new mark on, merged into one atomic when both fall in one word
+__device__ __forceinline__ void mark_move(u64 *B, uint32_t cell_old, uint32_t cell_new)
+{
+    const u64 m_old = 1ull << (cell_old & 63u), m_new = 1ull << (cell_new & 63u);
+    if ((cell_old >> 6) == (cell_new >> 6)) {
+        const u64 m = m_old ^ m_new;
+        if (m) atomicXor(&B[cell_new >> 6], m);
+    } else {
+        atomicXor(&B[cell_old >> 6], m_old);
+        atomicXor(&B[cell_new >> 6], m_new);
+    }
+}
+
+// first occupied cell j in [start, end) of a row, for windows of at most 256 cells (H <= 256): the up-to-five words
+// are requested together, then examined.  Requires start < end <= start + 256.
+__device__ __forceinline__ bool first_set_w(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
+{
+    const u64 *p = B + (row >> 6);
+    const uint32_t w0 = start >> 6, wl = (end - 1u) >> 6;
+    u64 m[5];
+#pragma unroll
+    for (uint32_t i = 0; i < 5u; i++) m[i] = (w0 + i <= wl) ? p[w0 + i] : 0ull;
+    m[0] &= ~0ull << (start & 63u);
+    const u64 tail = bits_below(end - (wl << 6));
+#pragma unroll
+    for (uint32_t i = 0; i < 5u; i++) {
+        if (w0 + i == wl) m[i] &= tail;
+        if (m[i]) {
+            j = ((w0 + i) << 6) + (uint32_t)__ffsll((long long)m[i]) - 1u;
+            return true;
+        }
+    }
+    return false;
+}
+// last occupied cell j in [start, end), windows of at most 128 cells (lookback <= 128): up to three words at once
+__device__ __forceinline__ bool last_set_w(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
+{
+    const u64 *p = B + (row >> 6);
+    const uint32_t w0 = start >> 6, wl = (end - 1u) >> 6;
+    u64 m[3];
+#pragma unroll
+    for (uint32_t i = 0; i < 3u; i++) m[i] = (wl >= w0 + i) ? p[wl - i] : 0ull;
+    m[0] &= bits_below(end - (wl << 6));
+    const u64 head = ~0ull << (start & 63u);
+#pragma unroll
+    for (uint32_t i = 0; i < 3u; i++) {
+        if (wl - i == w0) m[i] &= head;
+        if (m[i]) {
+            j = ((wl - i) << 6) + 63u - (uint32_t)__clzll((long long)m[i]);
+            return true;
+        }
+        if (wl - i == w0) return false;
+    }
+    return false;
+}
 
 }  // namespace manta

@@ -1,10 +1,16 @@
 // manta_kernels.cuh -- the three phases of one MANTA timestep as device functions, plus their kernels.
 //
-//   A admit   (R1)      : one thread per origin-edge FIFO; releases the head trip if its entry window is free
-//   U update  (R2-R9)   : one thread per active vehicle; reads the time-t atlas, and for the vehicles that stay on
-//                         their edge (the great majority) finishes the step: next state to the compacted next
-//                         buffer, time-(t+1) mark, clearing of the time-(t-1) mark.  Edge-end candidates post a
-//                         min-id claim and an entry of the cross list; arrivals post an entry too.
+//   A admit   (R1)      : one thread per origin-edge FIFO; idle queues cost one coalesced load (q_next); a due head
+//                         trip is released if its entry window is free
+//   U update  (R2-R9)   : one thread block per vehicle segment, one thread per active vehicle.  First pass: leader
+//                         search on the time-t occupancy words (the next four route records are requested up
+//                         front, the words of a row are requested together), IDM, lane-change pre-tests.  Vehicles
+//                         that must look at the adjacent lane (~6 %) are parked in a shared-memory queue and handled
+//                         by a dense second pass, so they do not hold their warps.  Vehicles that stay on their
+//                         edge (the great majority) finish the step here: next state to the compacted next buffer
+//                         of the segment (warp ballot + one shared-memory atomic per warp), time-(t+1) mark and
+//                         payload, time-(t-1) mark toggled off.  Edge-end candidates post a min-id claim and a
+//                         cross-list entry; arrivals post a cross-list entry.
 //   X cross   (R8, R9)  : one thread per cross-list entry: resolves the claim (winner moves to its next route
 //                         edge, loser holds at the stop line), writes its mark; clears the marks of arrivals.
 //
@@ -15,7 +21,9 @@
 
 namespace manta {
 
-#define MANTA_NT 512   // threads per block of the step kernels
+#define MANTA_NT 512      // threads per block of the step kernels
+#define MANTA_QCAP 256    // lane-change queue entries per block (overflow is handled in line)
+#define MANTA_MAX_LANES_DEV 8u
 
 struct Lead {
     bool found;
@@ -42,6 +50,14 @@ struct Outcome {
     float vn, acc;
 };
 
+// shared memory of the update phase
+struct UpdateSmem {
+    u64 stats[6];                 // lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel (kernel lifetime)
+    uint32_t out, xn, qn, flag;   // per segment: survivors written, cross-list entries, queued lane-change evaluations
+    LcEntry q[MANTA_QCAP];
+};
+enum { ST_LC = 0, ST_CELLS = 1, ST_EVAL = 2, ST_UPD = 3, ST_DONE = 4, ST_TRAVEL = 5 };
+
 __device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &s1v)
 {
     V.x = (int32_t)s0v.x;
@@ -60,45 +76,72 @@ __device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &
     V.pitch = pitch_of(V.len_c);
 }
 
+template <bool W256>
+__device__ __forceinline__ bool scan_fwd(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
+{
+    if (W256) return first_set_w(B, row, start, end, j);
+    return first_set(B, row, start, end, j);
+}
+template <bool W256>
+__device__ __forceinline__ bool scan_bwd(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
+{
+    if (W256) return last_set_w(B, row, start, end, j);
+    return last_set(B, row, start, end, j);
+}
+
 // ------------------------------------------------------------------------------------------------ R2
 // Leader search along the own lane and on along the route ("looking up the status of neighboring
-// cells"; G16).  The next route record is requested before the current row's words are examined, so the chain of
-// dependent loads is: state -> {own-row words, next record} -> next row's words -> leader payload.
-__device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const uint2 *pay, const Veh &V, u64 &examined)
+// cells"; G16).  The {cell_off, geom} halves of the next four route records are requested before the own row is
+// examined (they are consecutive in memory), so a hop costs one round trip for the next row's words and the chain
+// of dependent loads is: state -> {own-row words, records} -> next row's words ... -> leader payload.  Records past
+// the trip's last one belong to another trip: they may be loaded but are never used (the walk stops at `last`).
+template <bool W256>
+__device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const uint2 *pay, const Veh &V, uint32_t &examined)
 {
     Lead L;
     L.found = false;
     L.lead_abs = 0;
     L.v_lead = 0.0f;
     uint32_t len = V.len_c, row = V.cell_off + V.l * V.pitch, start = V.c + 1u, rem = P.H, dist_base = 0u, l = V.l;
-    uint32_t cursor = V.cursor;
     bool last = V.last;
-    uint4 rn = make_uint4(0u, 0u, 0u, 0u);
-    if (!last) rn = P.route[cursor + 1u];
+    const uint4 *rp = P.route + V.cursor;
+    uint2 r1 = make_uint2(0u, 0u), r2 = r1, r3 = r1, r4 = r1;
+    if (!last) {
+        r1 = *reinterpret_cast<const uint2 *>(rp + 1);
+        r2 = *reinterpret_cast<const uint2 *>(rp + 2);
+        r3 = *reinterpret_cast<const uint2 *>(rp + 3);
+        r4 = *reinterpret_cast<const uint2 *>(rp + 4);
+    }
+    uint32_t hop = 0u;
     for (;;) {
         const uint32_t end = min(len, start + rem);
         if (start < end) {
             uint32_t j;
-            if (first_set(B, row, start, end, j)) {
+            if (scan_fwd<W256>(B, row, start, end, j)) {
                 const uint2 pc = pay[(size_t)row + j];
-                examined += (u64)(j - start + 1u);
+                examined += j - start + 1u;
                 L.found = true;
                 L.lead_abs = (int32_t)(((dist_base + j) << 10) | pc.x);
                 L.v_lead = __uint_as_float(pc.y);
                 return L;
             }
-            examined += (u64)(end - start);
+            examined += end - start;
             rem -= end - start;
         }
         if (rem == 0u || last) return L;
-        cursor += 1u;
+        hop += 1u;
+        uint2 rn;
+        if (hop == 1u) rn = r1;
+        else if (hop == 2u) rn = r2;
+        else if (hop == 3u) rn = r3;
+        else if (hop == 4u) rn = r4;
+        else rn = *reinterpret_cast<const uint2 *>(rp + hop);
         dist_base += len;
         len = GEOM_LEN(rn.y);
         l = min(l, GEOM_LANES(rn.y) - 1u);
         row = rn.x + l * pitch_of(len);
         start = 0u;
         last = GEOM_LAST(rn.y) != 0u;
-        if (!last) rn = P.route[cursor + 1u];
     }
 }
 
@@ -155,7 +198,7 @@ __device__ __forceinline__ void pre_lc(const DevP &P, uint32_t t, Veh &V, const 
 // (has_a, x_a, v_a) / (has_b, x_b, v_b): lead / lag found in the target lane (Q22.10 position, speed); ignored
 // unless V.need_lc.
 __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh &V, bool has_a, int32_t x_a, float v_a,
-                                           bool has_b, int32_t x_b, float v_b, u64 &n_lc)
+                                           bool has_b, int32_t x_b, float v_b, uint32_t &n_lc)
 {
     const int32_t x = V.x;
     const float v = V.v;
@@ -210,7 +253,7 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
                 l_new = V.lt;
                 acc = fminf(V.acc_cur, acc_tgt);
                 if (has_a) bound = min(bound, x_a - P.L_fx);
-                n_lc += 1ull;
+                n_lc += 1u;
             }
         }
     }
@@ -242,10 +285,12 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
         O.kind = KIND_DONE;  // G18
         O.nx = 0u;
     } else {
-        const uint4 rn = P.route[V.cursor + 1u];
-        const uint32_t lplus = min(l_new, GEOM_LANES(rn.y) - 1u);
-        O.word = GEOM_PRIO(V.geom) ? (P.n_edges * 8u + P.head[P.route[V.cursor].z])  // PRIORITY: the node
-                                   : (rn.z * 8u + lplus);                             // GREEN: the lane entry
+        if (GEOM_PRIO(V.geom)) {   // PRIORITY: the claim word is the head node of this edge
+            O.word = P.n_edges * 8u + P.edge_tab[P.route[V.cursor].z].z;
+        } else {                   // GREEN: the lane entry (e+, l+)
+            const uint4 rn = P.route[V.cursor + 1u];
+            O.word = rn.z * 8u + min(l_new, GEOM_LANES(rn.y) - 1u);
+        }
         O.kind = KIND_CAND;
         O.nx = (uint32_t)(xn - len_fx);
         // smallest id wins; the key carries ~t in the high word so claim words never need a reset
@@ -255,242 +300,307 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
     return O;
 }
 
-// The whole R2-R8 arithmetic of one vehicle (reads only the time-t atlas).
-__device__ __forceinline__ Outcome update_vehicle(const DevP &P, uint32_t t, const u64 *B, const uint2 *pay, Veh &V, u64 &n_lc,
-                                                  u64 &n_cells, u64 &n_eval)
+// R5: lead (first occupied cell >= c, within the edge) and lag (last occupied cell < c) in the target lane, then
+// the rest of the update.
+template <bool W256>
+__device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_t t, const u64 *B, const uint2 *pay, const Veh &V,
+                                                          uint32_t &n_lc)
 {
-    const Lead ld = leader_search(P, B, pay, V, n_cells);
-    pre_lc(P, t, V, ld);
-    bool has_a = false, has_b = false;
+    const uint32_t rowt = V.cell_off + V.lt * V.pitch;
+    uint32_t ja = 0u, jb = 0u;
+    const uint32_t b0 = V.c > P.lookback ? V.c - P.lookback : 0u;
+    const bool has_a = scan_fwd<W256>(B, rowt, V.c, min(V.len_c, V.c + P.H), ja);
+    const bool has_b = V.c > b0 && scan_bwd<W256>(B, rowt, b0, V.c, jb);
     int32_t x_a = 0, x_b = 0;
     float v_a = 0.0f, v_b = 0.0f;
-    if (V.need_lc) {
-        // R5: lead (first occupied cell >= c, within the edge) and lag (last occupied cell < c) in the target lane
-        n_eval += 1ull;
-        const uint32_t rowt = V.cell_off + V.lt * V.pitch;
-        uint32_t ja = 0u, jb = 0u;
-        has_a = first_set(B, rowt, V.c, min(V.len_c, V.c + P.H), ja);
-        const uint32_t b0 = V.c > P.lookback ? V.c - P.lookback : 0u;
-        has_b = V.c > b0 && last_set(B, rowt, b0, V.c, jb);
-        if (has_a) {
-            const uint2 pc = pay[(size_t)rowt + ja];
-            x_a = (int32_t)((ja << 10) | pc.x);
-            v_a = __uint_as_float(pc.y);
-        }
-        if (has_b) {
-            const uint2 pc = pay[(size_t)rowt + jb];
-            x_b = (int32_t)((jb << 10) | pc.x);
-            v_b = __uint_as_float(pc.y);
-        }
+    uint2 pa = make_uint2(0u, 0u), pb = pa;
+    if (has_a) pa = pay[(size_t)rowt + ja];
+    if (has_b) pb = pay[(size_t)rowt + jb];
+    if (has_a) {
+        x_a = (int32_t)((ja << 10) | pa.x);
+        v_a = __uint_as_float(pa.y);
+    }
+    if (has_b) {
+        x_b = (int32_t)((jb << 10) | pb.x);
+        v_b = __uint_as_float(pb.y);
     }
     return post_lc(P, t, V, has_a, x_a, v_a, has_b, x_b, v_b, n_lc);
 }
 
+// R9 for one warp's vehicles: survivors compacted into the segment's next buffer (warp ballot + one shared-memory
+// atomic), time-(t+1) mark and payload for stayers, time-(t-1) mark toggled off, cross-list entries.  Must be
+// called by all 32 lanes; `have` says whether this lane carries a vehicle.
+__device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, bool have, const Veh &V,
+                                          const Outcome &O)
+{
+    const int nxt = (int)((t & 1u) ^ 1u);
+    u64 *Bn = P.bits[nxt];
+    const uint32_t lane_id = threadIdx.x & 31u;
+    const bool alive = have && O.kind != KIND_DONE, listed = have && O.kind != KIND_STAY;
+    const uint32_t bal_a = __ballot_sync(0xFFFFFFFFu, alive), bal_x = __ballot_sync(0xFFFFFFFFu, listed);
+    uint32_t base_a = 0u, base_x = 0u;
+    if (lane_id == 0u) {
+        if (bal_a) base_a = atomicAdd(&sm.out, (uint32_t)__popc(bal_a));
+        if (bal_x) base_x = atomicAdd(&sm.xn, (uint32_t)__popc(bal_x));
+    }
+    base_a = __shfl_sync(0xFFFFFFFFu, base_a, 0);
+    base_x = __shfl_sync(0xFFFFFFFFu, base_x, 0);
+    if (!have) return;
+    const uint32_t lt_mask = (1u << lane_id) - 1u;
+    const uint32_t pos = base_a + __popc(bal_a & lt_mask);
+    const uint32_t xpos = seg_base + base_x + __popc(bal_x & lt_mask);
+    const uint32_t cur_abs = V.cell_off + V.l * V.pitch + V.c;
+    const uint32_t geom_n = (V.geom & GEOM_STATIC_MASK) | (O.l_new << 28) | (V.tag << 31);
+    if (O.kind == KIND_STAY) {
+        const uint32_t cell = V.cell_off + O.l_new * V.pitch + (O.nx >> 10);
+        if (V.prev != CELL_NONE)
+            mark_move(Bn, V.prev, cell);
+        else
+            mark_toggle(Bn, cell);
+        P.pay[nxt][cell] = make_uint2(O.nx & 1023u, __float_as_uint(O.vn));
+    } else {
+        if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
+        if (O.kind == KIND_DONE) {
+            P.xlist[xpos] = make_uint4(XL_DONE, cur_abs, 0u, 0u);
+            P.arrive_step[V.id] = t + 1u;
+            atomicAdd(&sm.stats[ST_DONE], 1ull);
+            atomicAdd(&sm.stats[ST_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
+        } else {
+            P.xlist[xpos] = make_uint4(pos, O.word, V.cursor, V.id);
+        }
+    }
+    if (alive) {  // candidates: tentative winner state; the cross phase decides
+        P.S0[nxt][seg_base + pos] = make_uint4(O.nx, __float_as_uint(O.vn), V.id, V.cursor);
+        P.S1[nxt][seg_base + pos] = make_uint4(V.cell_off, geom_n, cur_abs, __float_as_uint(V.v0));
+        if (P.acc[nxt]) P.acc[nxt][seg_base + pos] = O.acc;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ A: R1
-// Departure admission (G17, G25).  Thread k owns the FIFO of origin edge q_edge[k]; trips in it are
-// in vehicle-id (= departure) order, so the head is the smallest waiting id on that edge.
+// Departure admission (G17, G25).  Thread k owns the FIFO of one origin edge; trips in it are in
+// vehicle-id (= departure) order, so the head is the smallest waiting id on that edge.
 __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize)
 {
     const int cur = (int)(t & 1u);
-    u64 *B = P.bits[t % 3u];
+    u64 *B = P.bits[cur];
     uint2 *pay = P.pay[cur];
     const u64 window = bits_below(P.L_c + 1u);
     for (uint32_t k = gtid; k < P.n_queues; k += gsize) {
+        if (P.q_next[k] > t) continue;                 // idle (or exhausted: NONE) queue
         const uint32_t h = P.q_head[k];
-        if (h >= P.q_ptr[k + 1u]) continue;
-        const uint32_t id = P.q_ids[h];
-        if (P.depart_step[id] > t) continue;
-        const uint32_t e = P.q_edge[k];
-        const uint4 er = P.edge_tab[e];
+        const uint4 er = P.q_row[k];
+        const uint4 ent = P.q_ent[h];                  // {id, depart_step, route_start, depart_step of the next entry}
         const uint32_t len = GEOM_LEN(er.y), lanes = GEOM_LANES(er.y), pitch = pitch_of(len);
-        for (uint32_t l = 0; l < lanes; l++) {
-            const uint32_t row = er.x + l * pitch;
-            if (B[row >> 6] & window) continue;   // window [0, L_c] not free
-            const uint32_t slot = (uint32_t)atomicAdd(&P.ctr->fill[cur], 1ull);
-            const uint32_t cursor = P.route_start[id];
-            const uint4 rr = P.route[cursor];
-            P.S0[cur][slot] = make_uint4(0u, 0u, id, cursor);
-            P.S1[cur][slot] = make_uint4(rr.x, (rr.y & GEOM_STATIC_MASK) | (l << 28), CELL_NONE, rr.w);
-            if (P.acc[cur]) P.acc[cur][slot] = 0.0f;
-            mark_set(B, row);                    // cell 0, frac10 = 0, v = 0: visible to this step's update
-            pay[(size_t)row] = make_uint2(0u, 0u);
-            P.admit_step[id] = t;
-            atomicAdd(&P.edge_entries[e], 1u);
-            P.q_head[k] = h + 1u;
-            break;
+        u64 w[MANTA_MAX_LANES_DEV];
+#pragma unroll
+        for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++) w[l] = l < lanes ? B[(er.x + l * pitch) >> 6] : ~0ull;
+        uint32_t l_sel = 0xFFFFFFFFu;
+#pragma unroll
+        for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++)
+            if (l_sel == 0xFFFFFFFFu && !(w[l] & window)) l_sel = l;   // first lane whose window [0, L_c] is free
+        if (l_sel == 0xFFFFFFFFu) continue;
+        const uint32_t id = ent.x, cursor = ent.z;
+        const uint4 rr = P.route[cursor];
+        // the emptier of two pseudo-random segments (keeps the segments balanced as trips come and go)
+        uint32_t hsh = mix32(k * 0x9E3779B9u + t);
+        uint32_t sa = hsh % P.n_seg, sb = (sa + 1u + (hsh >> 16) % max(P.n_seg - 1u, 1u)) % P.n_seg;
+        uint32_t seg = P.seg_cnt[cur][sb] < P.seg_cnt[cur][sa] ? sb : sa;
+        uint32_t slot;
+        for (;;) {
+            slot = atomicAdd(&P.seg_cnt[cur][seg], 1u);
+            if (slot < P.seg_cap) break;
+            atomicSub(&P.seg_cnt[cur][seg], 1u);       // full: the total capacity covers every trip, so another has room
+            seg = seg + 1u == P.n_seg ? 0u : seg + 1u;
         }
+        const uint32_t row = er.x + l_sel * pitch;
+        const size_t at = (size_t)seg * P.seg_cap + slot;
+        P.S0[cur][at] = make_uint4(0u, 0u, id, cursor);
+        P.S1[cur][at] = make_uint4(rr.x, (rr.y & GEOM_STATIC_MASK) | (l_sel << 28), CELL_NONE, rr.w);
+        if (P.acc[cur]) P.acc[cur][at] = 0.0f;
+        mark_toggle(B, row);                           // cell 0, frac10 = 0, v = 0: visible to this step's update
+        pay[(size_t)row] = make_uint2(0u, 0u);
+        P.admit_step[id] = t;
+        atomicAdd(&P.edge_entries[rr.z], 1u);
+        P.q_head[k] = h + 1u;
+        P.q_next[k] = ent.w;
     }
 }
 
 // ------------------------------------------------------------------------------------------------ U: R2-R9
-// Must be called by ALL threads of the block (contains __syncthreads).  s_scan: 2 * 32 + 2 words of shared memory.
-__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, uint32_t *s_scan, u64 &n_lc, u64 &n_cells, u64 &n_eval)
+// Must be called by ALL threads of the block (contains __syncthreads).
+template <bool W256>
+__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm)
 {
     const int cur = (int)(t & 1u), nxt = cur ^ 1;
-    const u64 *B = P.bits[t % 3u];
-    u64 *Bn = P.bits[(t + 1u) % 3u];
-    u64 *Bp = P.bits[(t + 2u) % 3u];
+    const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
-    uint2 *payn = P.pay[nxt];
-    const uint32_t n = (uint32_t)P.ctr->fill[cur];
-    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
-    const uint32_t gsize = gridDim.x * blockDim.x;
-    for (uint32_t base = blockIdx.x * blockDim.x; base < n; base += gsize) {
-        const uint32_t i = base + threadIdx.x;
-        bool alive = false, listed = false;
-        uint4 o0 = make_uint4(0, 0, 0, 0), o1 = make_uint4(0, 0, 0, 0);
-        uint2 xl = make_uint2(0u, 0u);
-        float acc_v = 0.0f;
-        if (i < n) {
-            Veh V;
-            veh_load(V, P.S0[cur][i], P.S1[cur][i]);
-            if (V.prev != CELL_NONE) mark_clear(Bp, V.prev);          // the time-(t-1) mark
-            const uint32_t cur_abs = V.cell_off + V.l * V.pitch + V.c;
-            const Outcome O = update_vehicle(P, t, B, pay, V, n_lc, n_cells, n_eval);
-            acc_v = O.acc;
-            const uint32_t geom_n = (V.geom & GEOM_STATIC_MASK) | (O.l_new << 28) | (V.tag << 31);
-            if (O.kind == KIND_STAY) {
-                alive = true;
-                const uint32_t cell = V.cell_off + O.l_new * V.pitch + (O.nx >> 10);
-                mark_set(Bn, cell);                                    // R9: the time-(t+1) mark
-                payn[cell] = make_uint2(O.nx & 1023u, __float_as_uint(O.vn));
-                o0 = make_uint4(O.nx, __float_as_uint(O.vn), V.id, V.cursor);
-                o1 = make_uint4(V.cell_off, geom_n, cur_abs, __float_as_uint(V.v0));
-            } else if (O.kind == KIND_DONE) {
-                listed = true;
-                xl = make_uint2(XL_DONE, cur_abs);
-                P.arrive_step[V.id] = t + 1u;
-                atomicAdd(&P.ctr->n_done, 1ull);
-                atomicAdd(&P.ctr->sum_travel, (u64)(t + 1u - P.admit_step[V.id]));
-            } else {  // candidate: tentative winner state; the cross phase decides
-                alive = true;
-                listed = true;
-                xl.y = O.word;
-                o0 = make_uint4(O.nx, __float_as_uint(O.vn), V.id, V.cursor);
-                o1 = make_uint4(V.cell_off, geom_n, cur_abs, __float_as_uint(V.v0));
-            }
-        }
-        // compaction of the survivors and of the cross list: warp ballots + block prefix sum, one atomic per block
-        const uint32_t bal_a = __ballot_sync(0xFFFFFFFFu, alive), bal_x = __ballot_sync(0xFFFFFFFFu, listed);
-        if (lane_id == 0u) {
-            s_scan[warp_id] = __popc(bal_a);
-            s_scan[32u + warp_id] = __popc(bal_x);
+    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+        const uint32_t n = P.seg_cnt[cur][seg];
+        const uint32_t seg_base = seg * P.seg_cap;
+        if (threadIdx.x == 0u) {
+            sm.out = 0u;
+            sm.xn = 0u;
+            sm.qn = 0u;
         }
         __syncthreads();
-        if (warp_id == 0u) {
-            const uint32_t ca = lane_id < n_warps ? s_scan[lane_id] : 0u, cx = lane_id < n_warps ? s_scan[32u + lane_id] : 0u;
-            uint32_t ia = ca, ix = cx;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t ya = __shfl_up_sync(0xFFFFFFFFu, ia, d), yx = __shfl_up_sync(0xFFFFFFFFu, ix, d);
-                if ((int)lane_id >= d) {
-                    ia += ya;
-                    ix += yx;
+        uint32_t n_cells = 0u, n_lc = 0u;
+        // ---- first pass: everything but the adjacent-lane look-up
+        for (uint32_t base = warp_id * 32u; base < n; base += blockDim.x) {
+            const uint32_t i = base + lane_id;
+            const bool have = i < n;
+            bool finish = have;
+            Veh V;
+            Outcome O;
+            O.kind = KIND_STAY;
+            Lead ld;
+            uint4 s0v = make_uint4(0u, 0u, 0u, 0u), s1v = s0v;
+            if (have) {
+                s0v = P.S0[cur][seg_base + i];
+                s1v = P.S1[cur][seg_base + i];
+                veh_load(V, s0v, s1v);
+                ld = leader_search<W256>(P, B, pay, V, n_cells);
+                pre_lc(P, t, V, ld);
+            }
+            const bool want_q = have && V.need_lc;
+            const uint32_t bal_q = __ballot_sync(0xFFFFFFFFu, want_q);
+            if (bal_q) {
+                uint32_t qb = 0u;
+                if (lane_id == 0u) {
+                    qb = atomicAdd(&sm.qn, (uint32_t)__popc(bal_q));
+                    atomicAdd(&sm.stats[ST_EVAL], (u64)__popc(bal_q));
+                }
+                qb = __shfl_sync(0xFFFFFFFFu, qb, 0);
+                if (want_q) {
+                    const uint32_t qi = qb + __popc(bal_q & ((1u << lane_id) - 1u));
+                    if (qi < MANTA_QCAP) {
+                        LcEntry e;
+                        e.s0 = s0v;
+                        e.s1 = s1v;
+                        e.lead_abs = ld.lead_abs;
+                        e.v_lead_bits = __float_as_uint(ld.v_lead);
+                        e.found = ld.found ? 1u : 0u;
+                        e.pad = 0u;
+                        sm.q[qi] = e;
+                        finish = false;
+                    } else {
+                        O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);   // queue full: in line
+                    }
                 }
             }
-            const uint32_t ta = __shfl_sync(0xFFFFFFFFu, ia, 31), tx = __shfl_sync(0xFFFFFFFFu, ix, 31);
-            u64 g = 0ull;
-            if (lane_id == 0u && (ta | tx)) g = atomicAdd(&P.ctr->fill[nxt], (u64)ta | ((u64)tx << 32));
-            g = __shfl_sync(0xFFFFFFFFu, g, 0);
-            if (lane_id < n_warps) {
-                s_scan[lane_id] = (uint32_t)g + ia - ca;
-                s_scan[32u + lane_id] = (uint32_t)(g >> 32) + ix - cx;
+            if (have && !V.need_lc) O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f, n_lc);
+            write_out(P, t, sm, seg_base, finish, V, O);
+        }
+        __syncthreads();
+        // ---- second pass: the queued lane-change evaluations, densely packed
+        const uint32_t nq = min(sm.qn, (uint32_t)MANTA_QCAP);
+        for (uint32_t base = warp_id * 32u; base < nq; base += blockDim.x) {
+            const uint32_t k = base + lane_id;
+            const bool have = k < nq;
+            Veh V;
+            Outcome O;
+            O.kind = KIND_STAY;
+            if (have) {
+                const LcEntry e = sm.q[k];
+                veh_load(V, e.s0, e.s1);
+                Lead ld;
+                ld.found = e.found != 0u;
+                ld.lead_abs = e.lead_abs;
+                ld.v_lead = __uint_as_float(e.v_lead_bits);
+                pre_lc(P, t, V, ld);
+                O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);
             }
+            write_out(P, t, sm, seg_base, have, V, O);
+        }
+        // ---- per-segment bookkeeping
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
+            n_lc += __shfl_down_sync(0xFFFFFFFFu, n_lc, d);
+        }
+        if (lane_id == 0u) {
+            if (n_cells) atomicAdd(&sm.stats[ST_CELLS], (u64)n_cells);
+            if (n_lc) atomicAdd(&sm.stats[ST_LC], (u64)n_lc);
         }
         __syncthreads();
-        if (alive) {
-            const uint32_t pos = s_scan[warp_id] + __popc(bal_a & ((1u << lane_id) - 1u));
-            P.S0[nxt][pos] = o0;
-            P.S1[nxt][pos] = o1;
-            if (P.acc[nxt]) P.acc[nxt][pos] = acc_v;
-            xl.x = pos;
+        if (threadIdx.x == 0u) {
+            P.seg_cnt[nxt][seg] = sm.out;
+            P.seg_xn[seg] = sm.xn;
+            sm.stats[ST_UPD] += (u64)n;
         }
-        if (listed) P.xlist[s_scan[32u + warp_id] + __popc(bal_x & ((1u << lane_id) - 1u))] = xl;
-        __syncthreads();
     }
 }
 
 // ------------------------------------------------------------------------------------------------ X: R8, R9
-__device__ __forceinline__ void cross_phase(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize)
+__device__ __forceinline__ void cross_phase(const DevP &P, uint32_t t)
 {
-    const int nxt = (int)((t & 1u) ^ 1u);
-    u64 *Bc = P.bits[t % 3u];
-    u64 *Bn = P.bits[(t + 1u) % 3u];
+    const int cur = (int)(t & 1u), nxt = cur ^ 1;
+    u64 *Bc = P.bits[cur];
+    u64 *Bn = P.bits[nxt];
     uint2 *payn = P.pay[nxt];
-    const uint32_t n = (uint32_t)(P.ctr->fill[nxt] >> 32);
-    for (uint32_t k = gtid; k < n; k += gsize) {
-        const uint2 xl = P.xlist[k];
-        if (xl.x == XL_DONE) {
-            mark_clear(Bc, xl.y);     // an arrival leaves no time-(t+1) state to clear its time-t mark later
-            continue;
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+        const uint32_t n = P.seg_xn[seg];
+        const size_t seg_base = (size_t)seg * P.seg_cap;
+        for (uint32_t k = threadIdx.x; k < n; k += blockDim.x) {
+            const uint4 xl = P.xlist[seg_base + k];     // {slot | XL_DONE, claim word | cell, cursor, id}
+            if (xl.x == XL_DONE) {
+                mark_toggle(Bc, xl.y);    // an arrival leaves no time-(t+1) state to clear its time-t mark later
+                continue;
+            }
+            uint4 s0 = P.S0[nxt][seg_base + xl.x];
+            uint4 s1 = P.S1[nxt][seg_base + xl.x];
+            const u64 won = P.claim[xl.y];
+            const uint4 rn = P.route[xl.z + 1u];
+            const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)xl.w;
+            if (won == key) {             // winner crosses (R8)
+                const uint32_t lplus = min(GEOM_LANE(s1.y), GEOM_LANES(rn.y) - 1u);
+                s0.w += 1u;
+                s1 = make_uint4(rn.x, (rn.y & GEOM_STATIC_MASK) | (lplus << 28), s1.z, rn.w);
+                atomicAdd(&P.edge_entries[rn.z], 1u);
+            } else {                      // loser holds at the stop line (G15)
+                s0.x = (GEOM_LEN(s1.y) << 10) - 1u;
+                s0.y = 0u;
+            }
+            P.S0[nxt][seg_base + xl.x] = s0;
+            P.S1[nxt][seg_base + xl.x] = s1;
+            const uint32_t cell = s1.x + GEOM_LANE(s1.y) * pitch_of(GEOM_LEN(s1.y)) + (s0.x >> 10);
+            mark_toggle(Bn, cell);
+            payn[cell] = make_uint2(s0.x & 1023u, s0.y);
         }
-        uint4 s0 = P.S0[nxt][xl.x];
-        uint4 s1 = P.S1[nxt][xl.x];
-        const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)s0.z;
-        if (P.claim[xl.y] == key) {   // winner crosses (R8)
-            const uint4 rn = P.route[s0.w + 1u];
-            const uint32_t lplus = min(GEOM_LANE(s1.y), GEOM_LANES(rn.y) - 1u);
-            s0.w += 1u;
-            s1 = make_uint4(rn.x, (rn.y & GEOM_STATIC_MASK) | (lplus << 28), s1.z, rn.w);
-            atomicAdd(&P.edge_entries[rn.z], 1u);
-        } else {                      // loser holds at the stop line (G15)
-            s0.x = (GEOM_LEN(s1.y) << 10) - 1u;
-            s0.y = 0u;
-        }
-        P.S0[nxt][xl.x] = s0;
-        P.S1[nxt][xl.x] = s1;
-        const uint32_t cell = s1.x + GEOM_LANE(s1.y) * pitch_of(GEOM_LEN(s1.y)) + (s0.x >> 10);
-        mark_set(Bn, cell);
-        payn[cell] = make_uint2(s0.x & 1023u, s0.y);
     }
 }
 
-__device__ __forceinline__ void flush_stats(const DevP &P, u64 n_lc, u64 n_cells, u64 n_eval, u64 *s_stats /*[3]*/)
+__device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm)
 {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        n_lc += __shfl_down_sync(0xFFFFFFFFu, n_lc, d);
-        n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
-        n_eval += __shfl_down_sync(0xFFFFFFFFu, n_eval, d);
-    }
-    if ((threadIdx.x & 31u) == 0u) {
-        if (n_lc) atomicAdd(&s_stats[0], n_lc);
-        if (n_cells) atomicAdd(&s_stats[1], n_cells);
-        if (n_eval) atomicAdd(&s_stats[2], n_eval);
-    }
     __syncthreads();
     if (threadIdx.x == 0u) {
         BlockStats *b = &P.blk[blockIdx.x];
-        b->lane_changes += s_stats[0];
-        b->cells_examined += s_stats[1];
-        b->lc_evals += s_stats[2];
+        b->lane_changes += sm.stats[ST_LC];
+        b->cells_examined += sm.stats[ST_CELLS];
+        b->lc_evals += sm.stats[ST_EVAL];
+        b->n_updates += sm.stats[ST_UPD];
+        b->n_done += sm.stats[ST_DONE];
+        b->sum_travel += sm.stats[ST_TRAVEL];
     }
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
 __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 {
-    const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (gtid == 0u) P.ctr->fill[(t & 1u) ^ 1u] = 0ull;   // the buffer (and cross list) this step's update will fill
-    admit_phase(P, t, gtid, gridDim.x * blockDim.x);
+    admit_phase(P, t, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
+template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, 2) k_update(const DevP P, uint32_t t)
 {
-    __shared__ u64 s_stats[3];
-    __shared__ uint32_t s_scan[64];
-    if (threadIdx.x < 3u) s_stats[threadIdx.x] = 0ull;
+    __shared__ UpdateSmem sm;
+    if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
     __syncthreads();
-    u64 n_lc = 0ull, n_cells = 0ull, n_eval = 0ull;
-    if (blockIdx.x == 0u && threadIdx.x == 0u) P.ctr->n_updates += P.ctr->fill[t & 1u] & 0xFFFFFFFFull;
-    update_phase(P, t, s_scan, n_lc, n_cells, n_eval);
-    flush_stats(P, n_lc, n_cells, n_eval, s_stats);
+    update_phase<W256>(P, t, sm);
+    flush_stats(P, sm);
 }
 
-__global__ void __launch_bounds__(256) k_cross(const DevP P, uint32_t t)
-{
-    cross_phase(P, t, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
-}
+__global__ void __launch_bounds__(256) k_cross(const DevP P, uint32_t t) { cross_phase(P, t); }
 
 // Grid-wide barrier of the persistent kernel: arrival counter + generation word, release / acquire at gpu scope
 // (the fences also invalidate L1, so plain loads after the barrier see the other SMs' writes).  A spin that lasts
@@ -528,26 +638,22 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
 }
 
 // One cooperative launch = n_steps timesteps; the host is not involved between steps.
+template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, 2) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps)
 {
-    __shared__ u64 s_stats[3];
-    __shared__ uint32_t s_scan[64];
-    __shared__ uint32_t s_flag;
-    if (threadIdx.x < 3u) s_stats[threadIdx.x] = 0ull;
-    u64 n_lc = 0ull, n_cells = 0ull, n_eval = 0ull;
+    __shared__ UpdateSmem sm;
+    if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
     unsigned gen = 0u;
     const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
     for (uint32_t t = t0; t < t0 + n_steps; t++) {
-        if (gtid == 0u) P.ctr->fill[(t & 1u) ^ 1u] = 0ull;
         admit_phase(P, t, gtid, gsize);
-        if (!grid_barrier(P.ctr, gen, &s_flag)) return;
-        if (gtid == 0u) P.ctr->n_updates += P.ctr->fill[t & 1u] & 0xFFFFFFFFull;
-        update_phase(P, t, s_scan, n_lc, n_cells, n_eval);
-        if (!grid_barrier(P.ctr, gen, &s_flag)) return;
-        cross_phase(P, t, gtid, gsize);
-        if (!grid_barrier(P.ctr, gen, &s_flag)) return;
+        if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+        update_phase<W256>(P, t, sm);
+        if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+        cross_phase(P, t);
+        if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     }
-    flush_stats(P, n_lc, n_cells, n_eval, s_stats);
+    flush_stats(P, sm);
 }
 
 // ------------------------------------------------------------------------------------------------ set-up kernels
@@ -584,36 +690,42 @@ __global__ void k_mark_last(const uint64_t *route_ptr, uint32_t n_trips, uint4 *
         route[k] = r;
     }
 }
-// Pre-placed vehicles (R1, last sentence): fill S1 from the route store, mark atlas_0, count the entry.
-__global__ void k_place_initial(const DevP P, uint32_t n_init)
+// Pre-placed vehicles (R1, last sentence): vehicle i of the list goes to segment i % n_seg; fill S1 from the route
+// store, mark atlas_0, count the entry.
+__global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init)
 {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_init; i += gridDim.x * blockDim.x) {
-        const uint4 s0v = P.S0[0][i];
+        const uint4 s0v = init[i];
         const uint4 rr = P.route[s0v.w];
-        P.S1[0][i] = make_uint4(rr.x, rr.y & GEOM_STATIC_MASK, CELL_NONE, rr.w);  // lane 0, tag 0, no earlier mark
+        const size_t at = (size_t)(i % P.n_seg) * P.seg_cap + i / P.n_seg;
+        P.S0[0][at] = s0v;
+        P.S1[0][at] = make_uint4(rr.x, rr.y & GEOM_STATIC_MASK, CELL_NONE, rr.w);  // lane 0, tag 0, no earlier mark
         const uint32_t cell = rr.x + (s0v.x >> 10);
-        mark_set(P.bits[0], cell);
+        mark_toggle(P.bits[0], cell);
         P.pay[0][cell] = make_uint2(s0v.x & 1023u, s0v.y);
         P.admit_step[s0v.z] = 0u;
         atomicAdd(&P.edge_entries[rr.z], 1u);
     }
 }
-// Readback: scatter the active array into per-trip arrays (caller order).
+// Readback: scatter the active segments into per-trip arrays (caller order).
 __global__ void k_gather_state(const DevP P, int cur, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
                                uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc)
 {
-    const uint32_t n = (uint32_t)P.ctr->fill[cur];
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const uint4 s0v = P.S0[cur][i];
-        const uint4 s1v = P.S1[cur][i];
-        const uint32_t tr = trip_of_id[s0v.z];
-        status[tr] = 1u;
-        route_pos[tr] = s0v.w - P.route_start[s0v.z];
-        lane[tr] = (uint8_t)GEOM_LANE(s1v.y);
-        tag[tr] = (uint8_t)GEOM_TAG(s1v.y);
-        x_fx[tr] = s0v.x;
-        v[tr] = __uint_as_float(s0v.y);
-        acc[tr] = P.acc[cur] ? P.acc[cur][i] : 0.0f;
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+        const uint32_t n = P.seg_cnt[cur][seg];
+        const size_t seg_base = (size_t)seg * P.seg_cap;
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            const uint4 s0v = P.S0[cur][seg_base + i];
+            const uint4 s1v = P.S1[cur][seg_base + i];
+            const uint32_t tr = trip_of_id[s0v.z];
+            status[tr] = 1u;
+            route_pos[tr] = s0v.w - P.route_start[s0v.z];
+            lane[tr] = (uint8_t)GEOM_LANE(s1v.y);
+            tag[tr] = (uint8_t)GEOM_TAG(s1v.y);
+            x_fx[tr] = s0v.x;
+            v[tr] = __uint_as_float(s0v.y);
+            acc[tr] = P.acc[cur] ? P.acc[cur][seg_base + i] : 0.0f;
+        }
     }
 }
 __global__ void k_status_from_steps(uint32_t n_trips, const uint32_t *trip_of_id, const uint32_t *admit_step,
