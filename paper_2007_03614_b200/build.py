@@ -30,7 +30,7 @@ def build_cuda(force=False, verbose=False):
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in DEPS)):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + ["-o", LIB] + SOURCES + ["-lcudart"]
+    cmd = [nvcc()] + NVCC_FLAGS + os.environ.get("MANTA_NVCC_EXTRA", "").split() + ["-o", LIB] + SOURCES + ["-lcudart"]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -21,8 +21,14 @@
 
 namespace manta {
 
+#ifndef MANTA_NT
 #define MANTA_NT 512      // threads per block of the step kernels
-#define MANTA_QCAP 256    // lane-change queue entries per block (overflow is handled in line)
+#endif
+#ifndef MANTA_MINB
+#define MANTA_MINB 1      // blocks per SM the step kernels are compiled for
+#endif
+#define MANTA_NW (MANTA_NT / 32)
+#define MANTA_QCAP 64     // lane-change queue entries per warp (drained whenever 32 or more are waiting)
 #define MANTA_MAX_LANES_DEV 8u
 
 struct Lead {
@@ -38,6 +44,7 @@ struct Veh {
     uint32_t id, cursor, cell_off, geom, prev;
     uint32_t len_c, n, l, c, pitch;
     bool last;
+    uint4 rn;           // next route record (valid unless last)
     // after pre_lc
     float acc_cur;
     int32_t bound;
@@ -53,8 +60,8 @@ struct Outcome {
 // shared memory of the update phase
 struct UpdateSmem {
     u64 stats[6];                 // lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel (kernel lifetime)
-    uint32_t out, xn, qn, flag;   // per segment: survivors written, cross-list entries, queued lane-change evaluations
-    LcEntry q[MANTA_QCAP];
+    uint32_t out, xn, flag, pad;  // per segment: survivors written, cross-list entries; barrier flag
+    uint4 q[MANTA_NW][MANTA_QCAP]; // per-warp queues of lane-change evaluations: {slot, lead_abs, v_lead bits, found}
 };
 enum { ST_LC = 0, ST_CELLS = 1, ST_EVAL = 2, ST_UPD = 3, ST_DONE = 4, ST_TRAVEL = 5 };
 
@@ -91,51 +98,41 @@ __device__ __forceinline__ bool scan_bwd(const u64 *B, uint32_t row, uint32_t st
 
 // ------------------------------------------------------------------------------------------------ R2
 // Leader search along the own lane and on along the route ("looking up the status of neighboring
-// cells"; G16).  The {cell_off, geom} halves of the next four route records are requested before the own row is
-// examined (they are consecutive in memory), so a hop costs one round trip for the next row's words and the chain
-// of dependent loads is: state -> {own-row words, records} -> next row's words ... -> leader payload.  Records past
-// the trip's last one belong to another trip: they may be loaded but are never used (the walk stops at `last`).
+// cells"; G16).  Result: the leader's absolute atlas cell and its distance in cells from the tail of the
+// follower's edge; the caller fetches the payload once, after the search, for the whole warp.
+struct Hit {
+    bool found;
+    uint32_t cell, dist;
+};
+
+// Generic walk (any H): one row after the other, records fetched as the walk reaches them.  Starts at `hop`
+// records past the vehicle's cursor, in row `row` of length `len` at cell `start`.
 template <bool W256>
-__device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const uint2 *pay, const Veh &V, uint32_t &examined)
+__device__ __forceinline__ Hit walk_rows(const DevP &P, const u64 *B, const uint4 *rp, uint32_t hop, uint32_t row, uint32_t len,
+                                         uint32_t start, uint32_t l, uint32_t rem, uint32_t dist_base, bool last,
+                                         uint32_t &examined)
 {
-    Lead L;
-    L.found = false;
-    L.lead_abs = 0;
-    L.v_lead = 0.0f;
-    uint32_t len = V.len_c, row = V.cell_off + V.l * V.pitch, start = V.c + 1u, rem = P.H, dist_base = 0u, l = V.l;
-    bool last = V.last;
-    const uint4 *rp = P.route + V.cursor;
-    uint2 r1 = make_uint2(0u, 0u), r2 = r1, r3 = r1, r4 = r1;
-    if (!last) {
-        r1 = *reinterpret_cast<const uint2 *>(rp + 1);
-        r2 = *reinterpret_cast<const uint2 *>(rp + 2);
-        r3 = *reinterpret_cast<const uint2 *>(rp + 3);
-        r4 = *reinterpret_cast<const uint2 *>(rp + 4);
-    }
-    uint32_t hop = 0u;
+    Hit h;
+    h.found = false;
+    h.cell = 0u;
+    h.dist = 0u;
     for (;;) {
         const uint32_t end = min(len, start + rem);
         if (start < end) {
             uint32_t j;
             if (scan_fwd<W256>(B, row, start, end, j)) {
-                const uint2 pc = pay[(size_t)row + j];
                 examined += j - start + 1u;
-                L.found = true;
-                L.lead_abs = (int32_t)(((dist_base + j) << 10) | pc.x);
-                L.v_lead = __uint_as_float(pc.y);
-                return L;
+                h.found = true;
+                h.cell = row + j;
+                h.dist = dist_base + j;
+                return h;
             }
             examined += end - start;
             rem -= end - start;
         }
-        if (rem == 0u || last) return L;
+        if (rem == 0u || last) return h;
         hop += 1u;
-        uint2 rn;
-        if (hop == 1u) rn = r1;
-        else if (hop == 2u) rn = r2;
-        else if (hop == 3u) rn = r3;
-        else if (hop == 4u) rn = r4;
-        else rn = *reinterpret_cast<const uint2 *>(rp + hop);
+        const uint2 rn = *reinterpret_cast<const uint2 *>(rp + hop);
         dist_base += len;
         len = GEOM_LEN(rn.y);
         l = min(l, GEOM_LANES(rn.y) - 1u);
@@ -143,6 +140,122 @@ __device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const
         start = 0u;
         last = GEOM_LAST(rn.y) != 0u;
     }
+}
+
+// H <= 256.  Three rounds of loads at most for nearly every vehicle: (1) the words of the own row together with
+// the next four route records (consecutive in memory); (2) the first two words of each of the next four rows,
+// all requested together; (3) the leader's payload (by the caller).  Longer walks (a row with more than 128
+// cells to examine after the own one, more than four hops) continue with dependent loads.  Records past the
+// trip's last one belong to another trip: they may be loaded but are never used (the walk stops at `last`).
+__device__ __forceinline__ Hit leader_cells_w(const DevP &P, const u64 *B, Veh &V, uint32_t &examined)
+{
+    Hit h;
+    h.found = false;
+    h.cell = 0u;
+    h.dist = 0u;
+    const uint4 *rp = P.route + V.cursor;
+    uint2 rr[4];
+    V.rn = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int k = 0; k < 4; k++) rr[k] = make_uint2(0u, 0u);
+    if (!V.last) {
+        V.rn = rp[1];
+        rr[1] = *reinterpret_cast<const uint2 *>(rp + 2);
+        rr[2] = *reinterpret_cast<const uint2 *>(rp + 3);
+        rr[3] = *reinterpret_cast<const uint2 *>(rp + 4);
+    }
+    uint32_t rem = P.H;
+    const uint32_t row0 = V.cell_off + V.l * V.pitch;
+    {   // own row
+        const uint32_t start = V.c + 1u, end = min(V.len_c, start + rem);
+        if (start < end) {
+            uint32_t j;
+            if (first_set_w(B, row0, start, end, j)) {
+                examined += j - start + 1u;
+                h.found = true;
+                h.cell = row0 + j;
+                h.dist = j;
+                return h;
+            }
+            examined += end - start;
+            rem -= end - start;
+        }
+    }
+    if (rem == 0u || V.last) return h;
+    rr[0] = make_uint2(V.rn.x, V.rn.y);
+    uint32_t rowk[4], nk[4], lenk[4];
+    u64 wa[4], wb[4];
+    bool valid = true;
+    uint32_t lk = V.l;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const uint32_t g = rr[k].y;
+        lenk[k] = GEOM_LEN(g);
+        lk = min(lk, GEOM_LANES(g) - 1u);
+        rowk[k] = rr[k].x + lk * pitch_of(lenk[k]);
+        nk[k] = valid ? min(lenk[k], rem) : 0u;
+        wa[k] = nk[k] ? B[rowk[k] >> 6] : 0ull;
+        wb[k] = nk[k] > 64u ? B[(rowk[k] >> 6) + 1u] : 0ull;
+        rem -= nk[k];
+        valid = valid && GEOM_LAST(g) == 0u && rem > 0u;
+    }
+    uint32_t dist_base = V.len_c;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        if (nk[k] && !h.found) {
+            const u64 ma = wa[k] & bits_below(min(nk[k], 64u));
+            uint32_t j = 0u;
+            bool f = false;
+            if (ma) {
+                j = (uint32_t)__ffsll((long long)ma) - 1u;
+                f = true;
+            } else if (nk[k] > 64u) {
+                const u64 mb = wb[k] & bits_below(min(nk[k] - 64u, 64u));
+                if (mb) {
+                    j = 64u + (uint32_t)__ffsll((long long)mb) - 1u;
+                    f = true;
+                } else if (nk[k] > 128u) {
+                    f = first_set_w(B, rowk[k], 128u, nk[k], j);
+                }
+            }
+            if (f) {
+                examined += j + 1u;
+                h.found = true;
+                h.cell = rowk[k] + j;
+                h.dist = dist_base + j;
+            } else {
+                examined += nk[k];
+            }
+        }
+        dist_base += lenk[k];
+    }
+    if (h.found || !valid) return h;
+    // more than four hops: go on from the end of the fourth row (start = len: nothing left to examine in it)
+    return walk_rows<true>(P, B, rp, 4u, rowk[3], lenk[3], lenk[3], lk, rem, dist_base - lenk[3], false, examined);
+}
+
+template <bool W256>
+__device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const uint2 *pay, Veh &V, uint32_t &examined)
+{
+    Hit h;
+    if (W256) {
+        h = leader_cells_w(P, B, V, examined);
+    } else {
+        V.rn = make_uint4(0u, 0u, 0u, 0u);
+        if (!V.last) V.rn = P.route[V.cursor + 1u];
+        h = walk_rows<false>(P, B, P.route + V.cursor, 0u, V.cell_off + V.l * V.pitch, V.len_c, V.c + 1u, V.l, P.H, 0u, V.last,
+                             examined);
+    }
+    Lead L;
+    L.found = h.found;
+    L.lead_abs = 0;
+    L.v_lead = 0.0f;
+    if (h.found) {
+        const uint2 pc = pay[h.cell];
+        L.lead_abs = (int32_t)((h.dist << 10) | pc.x);
+        L.v_lead = __uint_as_float(pc.y);
+    }
+    return L;
 }
 
 // R3 against the own-lane leader, R4 (mandatory tag of Eq. 2, lane-change desire pre-tests).
@@ -288,8 +401,7 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
         if (GEOM_PRIO(V.geom)) {   // PRIORITY: the claim word is the head node of this edge
             O.word = P.n_edges * 8u + P.edge_tab[P.route[V.cursor].z].z;
         } else {                   // GREEN: the lane entry (e+, l+)
-            const uint4 rn = P.route[V.cursor + 1u];
-            O.word = rn.z * 8u + min(l_new, GEOM_LANES(rn.y) - 1u);
+            O.word = V.rn.z * 8u + min(l_new, GEOM_LANES(V.rn.y) - 1u);
         }
         O.kind = KIND_CAND;
         O.nx = (uint32_t)(xn - len_fx);
@@ -427,6 +539,40 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
 }
 
 // ------------------------------------------------------------------------------------------------ U: R2-R9
+// Second pass of one warp: the lane-change evaluations it has parked, densely packed over its lanes.
+template <bool W256>
+__device__ __forceinline__ void drain_lc(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, uint32_t &qn, uint32_t &n_cells,
+                                         uint32_t &n_lc)
+{
+    const int cur = (int)(t & 1u);
+    const u64 *B = P.bits[cur];
+    const uint2 *pay = P.pay[cur];
+    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
+    __syncwarp();
+    while (qn > 0u) {
+        const uint32_t take = min(qn, 32u);
+        const bool have = lane_id < take;
+        Veh V;
+        Outcome O;
+        O.kind = KIND_STAY;
+        if (have) {
+            const uint4 e = sm.q[warp_id][qn - take + lane_id];
+            veh_load(V, P.S0[cur][seg_base + e.x], P.S1[cur][seg_base + e.x]);
+            V.rn = make_uint4(0u, 0u, 0u, 0u);
+            if (!V.last) V.rn = P.route[V.cursor + 1u];
+            Lead ld;
+            ld.found = e.w != 0u;
+            ld.lead_abs = (int32_t)e.y;
+            ld.v_lead = __uint_as_float(e.z);
+            pre_lc(P, t, V, ld);
+            O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);
+        }
+        write_out(P, t, sm, seg_base, have, V, O);
+        qn -= take;
+    }
+    __syncwarp();
+}
+
 // Must be called by ALL threads of the block (contains __syncthreads).
 template <bool W256>
 __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm)
@@ -441,77 +587,40 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
         if (threadIdx.x == 0u) {
             sm.out = 0u;
             sm.xn = 0u;
-            sm.qn = 0u;
         }
         __syncthreads();
-        uint32_t n_cells = 0u, n_lc = 0u;
-        // ---- first pass: everything but the adjacent-lane look-up
+        uint32_t n_cells = 0u, n_lc = 0u, qn = 0u;
         for (uint32_t base = warp_id * 32u; base < n; base += blockDim.x) {
+            // ---- first pass: everything but the adjacent-lane look-up
             const uint32_t i = base + lane_id;
             const bool have = i < n;
-            bool finish = have;
             Veh V;
             Outcome O;
             O.kind = KIND_STAY;
             Lead ld;
-            uint4 s0v = make_uint4(0u, 0u, 0u, 0u), s1v = s0v;
+            ld.found = false;
+            ld.lead_abs = 0;
+            ld.v_lead = 0.0f;
+            bool want_q = false;
             if (have) {
-                s0v = P.S0[cur][seg_base + i];
-                s1v = P.S1[cur][seg_base + i];
-                veh_load(V, s0v, s1v);
+                veh_load(V, P.S0[cur][seg_base + i], P.S1[cur][seg_base + i]);
                 ld = leader_search<W256>(P, B, pay, V, n_cells);
                 pre_lc(P, t, V, ld);
+                want_q = V.need_lc;
+                if (!want_q) O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f, n_lc);
             }
-            const bool want_q = have && V.need_lc;
             const uint32_t bal_q = __ballot_sync(0xFFFFFFFFu, want_q);
+            if (want_q)   // parked: vehicles that must look at the adjacent lane (R5) do not hold the warp
+                sm.q[warp_id][qn + __popc(bal_q & ((1u << lane_id) - 1u))] =
+                    make_uint4(i, (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), ld.found ? 1u : 0u);
+            write_out(P, t, sm, seg_base, have && !want_q, V, O);
             if (bal_q) {
-                uint32_t qb = 0u;
-                if (lane_id == 0u) {
-                    qb = atomicAdd(&sm.qn, (uint32_t)__popc(bal_q));
-                    atomicAdd(&sm.stats[ST_EVAL], (u64)__popc(bal_q));
-                }
-                qb = __shfl_sync(0xFFFFFFFFu, qb, 0);
-                if (want_q) {
-                    const uint32_t qi = qb + __popc(bal_q & ((1u << lane_id) - 1u));
-                    if (qi < MANTA_QCAP) {
-                        LcEntry e;
-                        e.s0 = s0v;
-                        e.s1 = s1v;
-                        e.lead_abs = ld.lead_abs;
-                        e.v_lead_bits = __float_as_uint(ld.v_lead);
-                        e.found = ld.found ? 1u : 0u;
-                        e.pad = 0u;
-                        sm.q[qi] = e;
-                        finish = false;
-                    } else {
-                        O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);   // queue full: in line
-                    }
-                }
+                qn += (uint32_t)__popc(bal_q);
+                if (lane_id == 0u) atomicAdd(&sm.stats[ST_EVAL], (u64)__popc(bal_q));
+                if (qn >= 32u) drain_lc<W256>(P, t, sm, seg_base, qn, n_cells, n_lc);
             }
-            if (have && !V.need_lc) O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f, n_lc);
-            write_out(P, t, sm, seg_base, finish, V, O);
         }
-        __syncthreads();
-        // ---- second pass: the queued lane-change evaluations, densely packed
-        const uint32_t nq = min(sm.qn, (uint32_t)MANTA_QCAP);
-        for (uint32_t base = warp_id * 32u; base < nq; base += blockDim.x) {
-            const uint32_t k = base + lane_id;
-            const bool have = k < nq;
-            Veh V;
-            Outcome O;
-            O.kind = KIND_STAY;
-            if (have) {
-                const LcEntry e = sm.q[k];
-                veh_load(V, e.s0, e.s1);
-                Lead ld;
-                ld.found = e.found != 0u;
-                ld.lead_abs = e.lead_abs;
-                ld.v_lead = __uint_as_float(e.v_lead_bits);
-                pre_lc(P, t, V, ld);
-                O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);
-            }
-            write_out(P, t, sm, seg_base, have, V, O);
-        }
+        drain_lc<W256>(P, t, sm, seg_base, qn, n_cells, n_lc);
         // ---- per-segment bookkeeping
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
@@ -591,7 +700,7 @@ __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 }
 
 template <bool W256>
-__global__ void __launch_bounds__(MANTA_NT, 2) k_update(const DevP P, uint32_t t)
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, uint32_t t)
 {
     __shared__ UpdateSmem sm;
     if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
@@ -639,7 +748,7 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
 
 // One cooperative launch = n_steps timesteps; the host is not involved between steps.
 template <bool W256>
-__global__ void __launch_bounds__(MANTA_NT, 2) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps)
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps)
 {
     __shared__ UpdateSmem sm;
     if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
