@@ -440,13 +440,15 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if ((rc = upload(s, &d_qent, q_ent.data(), q_ent.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
     if ((rc = upload(s, &d_qn, q_next.data(), q_next.size()))) return rollback(rc);
-    for (int k = 0; k < 2; k++) {
-        P.S0[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
-        P.S1[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
-        P.acc[k] = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, cap * sizeof(float)) : nullptr;
-        if (!P.S0[k] || !P.S1[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
-        if (P.acc[k]) CUDA_TRY(s, cudaMemsetAsync(P.acc[k], 0, cap * sizeof(float), s->stream));
-        if ((rc = alloc_fill(s, &P.seg_cnt[k], P.n_seg, 0))) return rollback(rc);
+    {
+        uint4 **arr[4] = {&P.S0, &P.S1, &P.S2, &P.S3};
+        for (int k = 0; k < 4; k++) {
+            *arr[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
+            if (!*arr[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+        }
+        P.acc = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, cap * sizeof(float)) : nullptr;
+        if (P.acc) CUDA_TRY(s, cudaMemsetAsync(P.acc, 0, cap * sizeof(float), s->stream));
+        if ((rc = alloc_fill(s, &P.seg_cnt, P.n_seg, 0))) return rollback(rc);
     }
     if ((rc = alloc_fill(s, &P.seg_xn, P.n_seg, 0))) return rollback(rc);
     P.xlist = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
@@ -460,7 +462,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         if ((rc = upload(s, &d_init, init_a0.data(), n_init))) return rollback(rc);
         std::vector<uint32_t> cnt0(P.n_seg);
         for (uint32_t k = 0; k < P.n_seg; k++) cnt0[k] = n_init / P.n_seg + (k < n_init % P.n_seg ? 1u : 0u);
-        CUDA_TRY(s, cudaMemcpyAsync(P.seg_cnt[0], cnt0.data(), (uint64_t)P.n_seg * 4, cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(P.seg_cnt, cnt0.data(), (uint64_t)P.n_seg * 4, cudaMemcpyHostToDevice, s->stream));
         k_place_initial<<<(n_init + 255) / 256, 256, 0, s->stream>>>(P, d_init, n_init);
         CUDA_TRY(s, cudaGetLastError());
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
@@ -586,7 +588,6 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
     if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint32_t n = s->n_trips;
-    const int cur = (int)(s->t & 1u);
     if (edge_entries)
         CUDA_TRY(s, cudaMemcpyAsync(edge_entries, s->P.edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyDeviceToHost, s->stream));
     if (st || trips || sum) {
@@ -601,7 +602,7 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
         CUDA_TRY(s, cudaMemsetAsync(buf, 0, nn * (3 + 16 + 8), s->stream));
         const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
         k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
-        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, cur, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
+        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
         CUDA_TRY(s, cudaGetLastError());
         std::vector<uint8_t> h_status(n);
         CUDA_TRY(s, cudaMemcpyAsync(h_status.data(), d_status, n, cudaMemcpyDeviceToHost, s->stream));

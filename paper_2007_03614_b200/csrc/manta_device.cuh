@@ -29,18 +29,25 @@ typedef unsigned long long u64;
 // row starts on a word boundary and no word is shared by two rows.
 //
 // Route store: one 16-byte RouteRec per route entry (edge attributes inlined, so following a route costs one
-// gather instead of route -> edge table); consecutive entries of a trip are consecutive in memory, so the next
-// four records of a vehicle are one or two sectors:
+// gather instead of route -> edge table); consecutive entries of a trip are consecutive in memory:
 //   w0 cell_off   w1 geom   w2 edge id   w3 speed limit v0 (fp32 bits)
 // geom bits: 0-15 len_c | 16-19 lanes | 20-22 lo | 23-25 hi | 26 last | 27 head-node PRIORITY | 28-30 lane | 31 tag
-// (lane / tag are only meaningful in a vehicle's private copy).
+// (lane / tag are only meaningful in a vehicle's private copy).  The route store is read only when a vehicle
+// enters an edge or changes lane (admission, cross phase, second pass of the update), never by the per-step
+// look-ahead: what the look-ahead needs of the next four route edges is cached in the vehicle's state (S2, S3).
 //
-// Active vehicles: n_seg SEGMENTS of seg_cap slots, two uint4 per vehicle (32 bytes, one sector), double-buffered.
-// A segment is processed by one thread block per phase, so survivor compaction needs only shared-memory atomics:
-// the update phase reads segment s of buffer t & 1 and writes its survivors, compacted, to segment s of buffer
-// (t+1) & 1.  A vehicle stays in the segment it was admitted to (admission picks the emptier of two segments).
-//   S0 = { x_fx, v bits, vehicle id, route cursor (absolute RouteRec index) }
-//   S1 = { cell_off, geom (+ lane, tag), absolute cell of the time-(t-1) mark or NONE, v0 bits }
+// Active vehicles: n_seg SEGMENTS of seg_cap slots, four uint4 per vehicle (64 bytes), updated IN PLACE.
+// A segment is processed by one thread block per phase.  A vehicle keeps its slot from admission (appended at
+// seg_cnt, admission picks the emptier of two segments) to arrival (slot marked dead: id = NONE); every
+// MANTA_COMPACT_EVERY timesteps the owning block squeezes the dead slots out (order-preserving, no global sync).
+//   S0 = { x_fx, v bits, absolute cell of the time-(t-1) mark or NONE, vehicle id or NONE (dead slot) }
+//   S1 = { row0 = absolute cell at which the row of the vehicle's own lane starts, geom (+ lane, tag),
+//          route cursor (absolute RouteRec index), v0 bits }
+//   S2 = { word index (cell >> 6) of the row the look-ahead continues in on route edges +1, +2, +3, +4
+//          (lane clamped hop by hop, R2) }
+//   S3 = { len_c of edges +1 | +2 << 16, len_c of edges +3 | +4 << 16 (0 = the route ended before),
+//          1 if the route goes on past edge +4, claim word of R8 for this edge's end }
+// A stayer rewrites S0 only (S1 when its tag or lane changed, S2/S3 when its lane changed).
 // Cross list (per segment): 16-byte entries made by the update phase for the few vehicles that need the second
 // phase (edge-end candidates, whose claim must be resolved, and arrivals, whose time-t mark must be cleared).
 // ---------------------------------------------------------------------------------------------------------
@@ -56,6 +63,9 @@ typedef unsigned long long u64;
 #define GEOM_STATIC_MASK 0x0FFFFFFFu
 #define CELL_NONE 0xFFFFFFFFu
 #define XL_DONE 0x80000000u
+#ifndef MANTA_COMPACT_EVERY
+#define MANTA_COMPACT_EVERY 64u   // timesteps between two squeezes of the dead vehicle slots of a segment
+#endif
 
 enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
 
@@ -67,15 +77,6 @@ struct Counters {
 // per-block private statistics and result counters (no global atomics on the hot path; summed at readback)
 struct BlockStats {
     u64 lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel, pad0, pad1;
-};
-
-// entry of the lane-change queue in shared memory (update phase, second pass)
-struct LcEntry {
-    uint4 s0, s1;
-    int32_t lead_abs;       // own-lane leader (R2) found by the first pass
-    uint32_t v_lead_bits;
-    uint32_t found;
-    uint32_t pad;
 };
 
 struct DevP {
@@ -94,13 +95,12 @@ struct DevP {
     uint2 *pay[2];
     // routes
     const uint4 *route;
-    // vehicles: segment s occupies slots [s * seg_cap, s * seg_cap + seg_cnt[k][s]) of buffer k
-    uint4 *S0[2];
-    uint4 *S1[2];
-    uint32_t *seg_cnt[2];
+    // vehicles: segment s occupies slots [s * seg_cap, s * seg_cap + seg_cnt[s]) (live and dead slots)
+    uint4 *S0, *S1, *S2, *S3;
+    uint32_t *seg_cnt;
     uint4 *xlist;                // cross list of segment s at [s * seg_cap, ...): {slot | XL_DONE, claim word | cell, cursor, id}
     uint32_t *seg_xn;            // cross-list entries of each segment (written by the update phase)
-    float *acc[2];               // optional (MANTA_FLAG_RECORD_ACC): acceleration applied in the last step
+    float *acc;                  // optional (MANTA_FLAG_RECORD_ACC): acceleration applied in the last step, per slot
     // per vehicle id
     const uint32_t *route_start;
     uint32_t *admit_step;
@@ -282,6 +282,45 @@ __device__ __forceinline__ bool last_set_w(const u64 *B, uint32_t row, uint32_t 
         if (wl - i == w0) return false;
     }
     return false;
+}
+
+// ------------------------------------------------------------------------------------------- look-ahead cache
+// What R2 needs of the four route edges after the current one, for a vehicle at RouteRec `cursor` in lane l:
+// the word index of the row it would continue in (lane clamped hop by hop: "the lane index carried on is the
+// clamped one") and the edge lengths.  Built when a vehicle enters an edge or changes lane; off the per-step path.
+// The route store is padded with 8 zero records, so the four loads are always in bounds; records past the trip's
+// last one belong to another trip and are ignored (len 0).
+struct Hops {
+    uint4 s2, s3;
+};
+__device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint32_t geom_cur, uint32_t l)
+{
+    const uint4 *rp = P.route + cursor;
+    uint4 r[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) r[k] = rp[k + 1];
+    bool ended = GEOM_LAST(geom_cur) != 0u;
+    uint32_t roww[4], len[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const uint32_t g = r[k].y;
+        const uint32_t lk = min(l, GEOM_LANES(g) - 1u);
+        roww[k] = ended ? 0u : (r[k].x + lk * pitch_of(GEOM_LEN(g))) >> 6;
+        len[k] = ended ? 0u : GEOM_LEN(g);
+        l = ended ? l : lk;
+        ended = ended || GEOM_LAST(g) != 0u;
+    }
+    uint32_t word = 0u;
+    if (!GEOM_LAST(geom_cur)) {
+        if (GEOM_PRIO(geom_cur))       // PRIORITY: the claim word is the head node of this edge (R8)
+            word = P.n_edges * 8u + P.edge_tab[rp[0].z].z;
+        else                           // GREEN: lane entry (e+, l+); the low 3 bits hold lanes(e+) - 1 until l' is known
+            word = r[0].z * 8u + (GEOM_LANES(r[0].y) - 1u);
+    }
+    Hops h;
+    h.s2 = make_uint4(roww[0], roww[1], roww[2], roww[3]);
+    h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), ended ? 0u : 1u, word);
+    return h;
 }
 
 }  // namespace manta

@@ -2,17 +2,20 @@
 //
 //   A admit   (R1)      : one thread per origin-edge FIFO; idle queues cost one coalesced load (q_next); a due head
 //                         trip is released if its entry window is free
-//   U update  (R2-R9)   : one thread block per vehicle segment, one thread per active vehicle.  First pass: leader
-//                         search on the time-t occupancy words (the next four route records are requested up
-//                         front, the words of a row are requested together), IDM, lane-change pre-tests.  Vehicles
-//                         that must look at the adjacent lane (~6 %) are parked in a shared-memory queue and handled
-//                         by a dense second pass, so they do not hold their warps.  Vehicles that stay on their
-//                         edge (the great majority) finish the step here: next state to the compacted next buffer
-//                         of the segment (warp ballot + one shared-memory atomic per warp), time-(t+1) mark and
-//                         payload, time-(t-1) mark toggled off.  Edge-end candidates post a min-id claim and a
-//                         cross-list entry; arrivals post a cross-list entry.
+//   U update  (R2-R9)   : one thread block per vehicle segment, one thread per active vehicle, state updated in
+//                         place.  First pass, branch-free for nearly every vehicle: the (at most eight) occupancy
+//                         words of the whole look-ahead window -- own row and the rows it continues in on the next
+//                         route edges, whose addresses come from the vehicle's own state -- are requested together,
+//                         searched with selects and one find-first-set, then the leader's payload is fetched; IDM,
+//                         lane-change pre-tests, integration, classification.  Vehicles that must look at the
+//                         adjacent lane (~6 %) or whose window does not fit the fast search (< 1 %) are parked in a
+//                         block-wide shared-memory queue and handled by a dense second pass, so they do not hold
+//                         their warps.  Vehicles that stay on their edge finish the step here: next state, time-(t+1)
+//                         mark and payload, time-(t-1) mark toggled off.  Edge-end candidates post a min-id claim
+//                         and a cross-list entry; arrivals post a cross-list entry and free their slot.
 //   X cross   (R8, R9)  : one thread per cross-list entry: resolves the claim (winner moves to its next route
-//                         edge, loser holds at the stop line), writes its mark; clears the marks of arrivals.
+//                         edge and rebuilds its look-ahead cache, loser holds at the stop line), writes its mark;
+//                         clears the marks of arrivals.
 //
 // A grid-wide barrier separates the phases: the software barrier of k_persistent (one cooperative launch runs
 // many timesteps), or kernel boundaries (k_admit / k_update / k_cross: MANTA_FLAG_MULTI_KERNEL, manta_step_timed).
@@ -25,10 +28,11 @@ namespace manta {
 #define MANTA_NT 512      // threads per block of the step kernels
 #endif
 #ifndef MANTA_MINB
-#define MANTA_MINB 1      // blocks per SM the step kernels are compiled for
+#define MANTA_MINB 2      // blocks per SM the step kernels are compiled for
 #endif
 #define MANTA_NW (MANTA_NT / 32)
-#define MANTA_QCAP 64     // lane-change queue entries per warp (drained whenever 32 or more are waiting)
+#define MANTA_QCAP (2 * MANTA_NT)   // second-pass queue entries per block (drained whenever MANTA_NT or more wait)
+#define MANTA_NS 8        // occupancy words the fast look-ahead search requests per vehicle
 #define MANTA_MAX_LANES_DEV 8u
 
 struct Lead {
@@ -41,10 +45,10 @@ struct Lead {
 struct Veh {
     int32_t x;
     float v, v0;
-    uint32_t id, cursor, cell_off, geom, prev;
+    uint32_t id, cursor, row0, geom, prev;
     uint32_t len_c, n, l, c, pitch;
     bool last;
-    uint4 rn;           // next route record (valid unless last)
+    uint32_t claim;     // S3.w
     // after pre_lc
     float acc_cur;
     int32_t bound;
@@ -53,15 +57,16 @@ struct Veh {
 };
 
 struct Outcome {
-    uint32_t kind, nx, l_new, word;
+    uint32_t kind, nx, l_new;
     float vn, acc;
 };
 
 // shared memory of the update phase
 struct UpdateSmem {
     u64 stats[6];                 // lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel (kernel lifetime)
-    uint32_t out, xn, flag, pad;  // per segment: survivors written, cross-list entries; barrier flag
-    uint4 q[MANTA_NW][MANTA_QCAP]; // per-warp queues of lane-change evaluations: {slot, lead_abs, v_lead bits, found}
+    uint32_t xn, qn, flag, pad;   // per segment: cross-list entries, queue fill; barrier flag
+    uint32_t wsum[MANTA_NW];      // compaction: live slots per warp
+    uint4 q[MANTA_QCAP];          // second-pass queue: {slot, lead_abs, v_lead bits, 0 not found | 1 found | 2 search still to do}
 };
 enum { ST_LC = 0, ST_CELLS = 1, ST_EVAL = 2, ST_UPD = 3, ST_DONE = 4, ST_TRAVEL = 5 };
 
@@ -69,11 +74,11 @@ __device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &
 {
     V.x = (int32_t)s0v.x;
     V.v = __uint_as_float(s0v.y);
-    V.id = s0v.z;
-    V.cursor = s0v.w;
-    V.cell_off = s1v.x;
+    V.prev = s0v.z;
+    V.id = s0v.w;
+    V.row0 = s1v.x;
     V.geom = s1v.y;
-    V.prev = s1v.z;
+    V.cursor = s1v.z;
     V.v0 = __uint_as_float(s1v.w);
     V.len_c = GEOM_LEN(V.geom);
     V.n = GEOM_LANES(V.geom);
@@ -99,28 +104,29 @@ __device__ __forceinline__ bool scan_bwd(const u64 *B, uint32_t row, uint32_t st
 // ------------------------------------------------------------------------------------------------ R2
 // Leader search along the own lane and on along the route ("looking up the status of neighboring
 // cells"; G16).  Result: the leader's absolute atlas cell and its distance in cells from the tail of the
-// follower's edge; the caller fetches the payload once, after the search, for the whole warp.
+// follower's edge.
 struct Hit {
     bool found;
     uint32_t cell, dist;
 };
 
-// Generic walk (any H): one row after the other, records fetched as the walk reaches them.  Starts at `hop`
-// records past the vehicle's cursor, in row `row` of length `len` at cell `start`.
-template <bool W256>
-__device__ __forceinline__ Hit walk_rows(const DevP &P, const u64 *B, const uint4 *rp, uint32_t hop, uint32_t row, uint32_t len,
-                                         uint32_t start, uint32_t l, uint32_t rem, uint32_t dist_base, bool last,
-                                         uint32_t &examined)
+// Generic walk (any H, any number of hops): one row after the other, route records fetched as the walk reaches
+// them.  Used by the second pass for the few vehicles whose window does not fit the fast search, and by every
+// vehicle when H > 256.
+__device__ __forceinline__ Hit walk_rows(const DevP &P, const u64 *B, const Veh &V, uint32_t &examined)
 {
     Hit h;
     h.found = false;
     h.cell = 0u;
     h.dist = 0u;
+    const uint4 *rp = P.route + V.cursor;
+    uint32_t hop = 0u, row = V.row0, len = V.len_c, start = V.c + 1u, l = V.l, rem = P.H, dist_base = 0u;
+    bool last = V.last;
     for (;;) {
         const uint32_t end = min(len, start + rem);
         if (start < end) {
             uint32_t j;
-            if (scan_fwd<W256>(B, row, start, end, j)) {
+            if (first_set(B, row, start, end, j)) {
                 examined += j - start + 1u;
                 h.found = true;
                 h.cell = row + j;
@@ -142,110 +148,80 @@ __device__ __forceinline__ Hit walk_rows(const DevP &P, const u64 *B, const uint
     }
 }
 
-// H <= 256.  Three rounds of loads at most for nearly every vehicle: (1) the words of the own row together with
-// the next four route records (consecutive in memory); (2) the first two words of each of the next four rows,
-// all requested together; (3) the leader's payload (by the caller).  Longer walks (a row with more than 128
-// cells to examine after the own one, more than four hops) continue with dependent loads.  Records past the
-// trip's last one belong to another trip: they may be loaded but are never used (the walk stops at `last`).
-__device__ __forceinline__ Hit leader_cells_w(const DevP &P, const u64 *B, Veh &V, uint32_t &examined)
+__device__ __forceinline__ uint32_t ffs64(u64 m)   // index of the lowest set bit; m != 0
 {
-    Hit h;
+    return (uint32_t)__ffsll((long long)m) - 1u;
+}
+
+// Fast search (H <= 256).  The window is a sequence of at most five segments -- the rest of the own row, then
+// the first cells of the rows cached in S2 / S3 -- of n_0 .. n_4 occupancy words; word slot s of the sequence
+// lives at word address s + A_j, j the segment it falls in.  All MANTA_NS word loads are issued before any is
+// examined.  Bits past the end of a segment can only be padding (never set) or lie beyond the H-th examined cell,
+// which the final distance test rejects, so no tail masks are needed.  Returns false if the window does not fit
+// (more than MANTA_NS words, or it runs past the cached hops): the caller then uses walk_rows.
+__device__ __forceinline__ bool leader_cells_fast(const DevP &P, const u64 *B, const Veh &V, const uint4 &s2, const uint4 &s3,
+                                                  Hit &h, uint32_t &examined)
+{
+    const uint32_t start = V.c + 1u;
+    const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
+    uint32_t rem = P.H - own;
+    const uint32_t len1 = s3.x & 0xFFFFu, len2 = s3.x >> 16, len3 = s3.y & 0xFFFFu, len4 = s3.y >> 16;
+    const uint32_t k1 = min(len1, rem);
+    rem -= k1;
+    const uint32_t k2 = min(len2, rem);
+    rem -= k2;
+    const uint32_t k3 = min(len3, rem);
+    rem -= k3;
+    const uint32_t k4 = min(len4, rem);
+    rem -= k4;
+    const uint32_t w0 = start >> 6;
+    const uint32_t n0 = own ? ((start + own - 1u) >> 6) - w0 + 1u : 0u;
+    const uint32_t c0 = n0, c1 = c0 + ((k1 + 63u) >> 6), c2 = c1 + ((k2 + 63u) >> 6), c3 = c2 + ((k3 + 63u) >> 6),
+                   c4 = c3 + ((k4 + 63u) >> 6);
+    if (c4 > (uint32_t)MANTA_NS || (rem > 0u && s3.z != 0u)) return false;
+    // word address of slot s = s + A_j; distance (cells from the tail of the own edge) of bit b of slot s = 64 s + b + D_j
+    const uint32_t A0 = (V.row0 >> 6) + w0, A1 = s2.x - c0, A2 = s2.y - c1, A3 = s2.z - c2, A4 = s2.w - c3;
+    u64 m[MANTA_NS];
+#pragma unroll
+    for (uint32_t s = 0; s < (uint32_t)MANTA_NS; s++) {
+        const uint32_t A = s < c0 ? A0 : (s < c1 ? A1 : (s < c2 ? A2 : (s < c3 ? A3 : A4)));
+        m[s] = s < c4 ? B[A + s] : 0ull;
+    }
+    if (n0) m[0] &= ~0ull << (start & 63u);
+    u64 sel = 0ull;
+    uint32_t si = 0u;
+#pragma unroll
+    for (int s = MANTA_NS - 1; s >= 0; s--)
+        if (m[s]) {
+            sel = m[s];
+            si = (uint32_t)s;
+        }
+    const uint32_t scanned = P.H - rem;
     h.found = false;
     h.cell = 0u;
     h.dist = 0u;
-    const uint4 *rp = P.route + V.cursor;
-    uint2 rr[4];
-    V.rn = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-    for (int k = 0; k < 4; k++) rr[k] = make_uint2(0u, 0u);
-    if (!V.last) {
-        V.rn = rp[1];
-        rr[1] = *reinterpret_cast<const uint2 *>(rp + 2);
-        rr[2] = *reinterpret_cast<const uint2 *>(rp + 3);
-        rr[3] = *reinterpret_cast<const uint2 *>(rp + 4);
-    }
-    uint32_t rem = P.H;
-    const uint32_t row0 = V.cell_off + V.l * V.pitch;
-    {   // own row
-        const uint32_t start = V.c + 1u, end = min(V.len_c, start + rem);
-        if (start < end) {
-            uint32_t j;
-            if (first_set_w(B, row0, start, end, j)) {
-                examined += j - start + 1u;
-                h.found = true;
-                h.cell = row0 + j;
-                h.dist = j;
-                return h;
-            }
-            examined += end - start;
-            rem -= end - start;
+    if (sel) {
+        const uint32_t b = ffs64(sel);
+        const uint32_t d1 = V.len_c, d2 = d1 + len1, d3 = d2 + len2, d4 = d3 + len3;
+        uint32_t A = A4, D = d4 - (c3 << 6);
+        if (si < c3) { A = A3; D = d3 - (c2 << 6); }
+        if (si < c2) { A = A2; D = d2 - (c1 << 6); }
+        if (si < c1) { A = A1; D = d1 - (c0 << 6); }
+        if (si < c0) { A = A0; D = w0 << 6; }
+        const uint32_t dist = (si << 6) + b + D;
+        if (dist - V.c <= P.H) {
+            h.found = true;
+            h.dist = dist;
+            h.cell = ((A + si) << 6) + b;
         }
     }
-    if (rem == 0u || V.last) return h;
-    rr[0] = make_uint2(V.rn.x, V.rn.y);
-    uint32_t rowk[4], nk[4], lenk[4];
-    u64 wa[4], wb[4];
-    bool valid = true;
-    uint32_t lk = V.l;
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        const uint32_t g = rr[k].y;
-        lenk[k] = GEOM_LEN(g);
-        lk = min(lk, GEOM_LANES(g) - 1u);
-        rowk[k] = rr[k].x + lk * pitch_of(lenk[k]);
-        nk[k] = valid ? min(lenk[k], rem) : 0u;
-        wa[k] = nk[k] ? B[rowk[k] >> 6] : 0ull;
-        wb[k] = nk[k] > 64u ? B[(rowk[k] >> 6) + 1u] : 0ull;
-        rem -= nk[k];
-        valid = valid && GEOM_LAST(g) == 0u && rem > 0u;
-    }
-    uint32_t dist_base = V.len_c;
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        if (nk[k] && !h.found) {
-            const u64 ma = wa[k] & bits_below(min(nk[k], 64u));
-            uint32_t j = 0u;
-            bool f = false;
-            if (ma) {
-                j = (uint32_t)__ffsll((long long)ma) - 1u;
-                f = true;
-            } else if (nk[k] > 64u) {
-                const u64 mb = wb[k] & bits_below(min(nk[k] - 64u, 64u));
-                if (mb) {
-                    j = 64u + (uint32_t)__ffsll((long long)mb) - 1u;
-                    f = true;
-                } else if (nk[k] > 128u) {
-                    f = first_set_w(B, rowk[k], 128u, nk[k], j);
-                }
-            }
-            if (f) {
-                examined += j + 1u;
-                h.found = true;
-                h.cell = rowk[k] + j;
-                h.dist = dist_base + j;
-            } else {
-                examined += nk[k];
-            }
-        }
-        dist_base += lenk[k];
-    }
-    if (h.found || !valid) return h;
-    // more than four hops: go on from the end of the fourth row (start = len: nothing left to examine in it)
-    return walk_rows<true>(P, B, rp, 4u, rowk[3], lenk[3], lenk[3], lk, rem, dist_base - lenk[3], false, examined);
+    examined += h.found ? h.dist - V.c : scanned;
+    return true;
 }
 
 template <bool W256>
-__device__ __forceinline__ Lead leader_search(const DevP &P, const u64 *B, const uint2 *pay, Veh &V, uint32_t &examined)
+__device__ __forceinline__ Lead lead_from_hit(const uint2 *pay, const Hit &h)
 {
-    Hit h;
-    if (W256) {
-        h = leader_cells_w(P, B, V, examined);
-    } else {
-        V.rn = make_uint4(0u, 0u, 0u, 0u);
-        if (!V.last) V.rn = P.route[V.cursor + 1u];
-        h = walk_rows<false>(P, B, P.route + V.cursor, 0u, V.cell_off + V.l * V.pitch, V.len_c, V.c + 1u, V.l, P.H, 0u, V.last,
-                             examined);
-    }
     Lead L;
     L.found = h.found;
     L.lead_abs = 0;
@@ -269,7 +245,27 @@ __device__ __forceinline__ void pre_lc(const DevP &P, uint32_t t, Veh &V, const 
         s = sf - P.veh_len;
         V.bound = ld.lead_abs - P.L_fx;
     }
-    V.acc_cur = idm_acc(P, V.v, V.v0, ld.found, s, ld.v_lead);
+    // R3, Eq. (1); the free-road term is kept for the discretionary pre-test of R4
+    float r = V.v / V.v0;
+    float r2 = r * r;
+    float fr = r2 * r2;
+    float inter = 0.0f;
+    if (ld.found) {
+        float dv = V.v - ld.v_lead;
+        float q = V.v * dv;
+        q = q * P.C1;
+        float ss = P.T * V.v;
+        ss = ss + q;
+        ss = fmaxf(0.0f, ss);
+        ss = P.s0 + ss;
+        float se = fmaxf(s, 0.01f);
+        float z = ss / se;
+        inter = z * z;
+    }
+    const float one_m_fr = 1.0f - fr;
+    float acc = one_m_fr - inter;
+    acc = P.a * acc;
+    V.acc_cur = acc;
     // R4: mandatory tag, Eq. (2)
     uint32_t tag = GEOM_TAG(V.geom);
     if (tag == 0u && !V.last && V.n >= 2u) {
@@ -295,11 +291,7 @@ __device__ __forceinline__ void pre_lc(const DevP &P, uint32_t t, Veh &V, const 
         const bool l_in = (V.l >= lo && V.l <= hi), lt_in = (lt >= lo && lt <= hi);
         V.mand = tag == 1u && !l_in && ((V.l < lo && dir > 0) || (V.l > hi && dir < 0));
         if (!(tag == 1u && !lt_in) && ld.found) {  // G9: impeded in the own lane
-            float rr = V.v / V.v0;
-            float rr2 = rr * rr;
-            float fr = rr2 * rr2;
-            float af = 1.0f - fr;
-            af = P.a * af;
+            float af = P.a * one_m_fr;
             float g = af - V.acc_cur;
             V.disc_pre = g > P.dlc_thr;
         }
@@ -311,7 +303,7 @@ __device__ __forceinline__ void pre_lc(const DevP &P, uint32_t t, Veh &V, const 
 // (has_a, x_a, v_a) / (has_b, x_b, v_b): lead / lag found in the target lane (Q22.10 position, speed); ignored
 // unless V.need_lc.
 __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh &V, bool has_a, int32_t x_a, float v_a,
-                                           bool has_b, int32_t x_b, float v_b, uint32_t &n_lc)
+                                           bool has_b, int32_t x_b, float v_b)
 {
     const int32_t x = V.x;
     const float v = V.v;
@@ -366,7 +358,6 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
                 l_new = V.lt;
                 acc = fminf(V.acc_cur, acc_tgt);
                 if (has_a) bound = min(bound, x_a - P.L_fx);
-                n_lc += 1u;
             }
         }
     }
@@ -389,7 +380,6 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
     O.acc = acc;
     O.vn = vn;
     O.l_new = l_new;
-    O.word = 0u;
     const int32_t len_fx = (int32_t)(V.len_c << 10);
     if (xn < len_fx) {
         O.kind = KIND_STAY;
@@ -398,27 +388,66 @@ __device__ __forceinline__ Outcome post_lc(const DevP &P, uint32_t t, const Veh 
         O.kind = KIND_DONE;  // G18
         O.nx = 0u;
     } else {
-        if (GEOM_PRIO(V.geom)) {   // PRIORITY: the claim word is the head node of this edge
-            O.word = P.n_edges * 8u + P.edge_tab[P.route[V.cursor].z].z;
-        } else {                   // GREEN: the lane entry (e+, l+)
-            O.word = V.rn.z * 8u + min(l_new, GEOM_LANES(V.rn.y) - 1u);
-        }
         O.kind = KIND_CAND;
         O.nx = (uint32_t)(xn - len_fx);
-        // smallest id wins; the key carries ~t in the high word so claim words never need a reset
-        const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)V.id;
-        atomicMin(&P.claim[O.word], key);
     }
     return O;
+}
+
+// R9 for one vehicle, in place: next state, time-(t+1) mark and payload for stayers, time-(t-1) mark toggled
+// off, claim + cross-list entry for edge-end candidates, cross-list entry + freed slot for arrivals.
+__device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, uint32_t slot, const Veh &V,
+                                          const Outcome &O)
+{
+    const int nxt = (int)((t & 1u) ^ 1u);
+    u64 *Bn = P.bits[nxt];
+    const uint32_t cur_abs = V.row0 + V.c;
+    const uint32_t at = seg_base + slot;
+    const bool changed = O.l_new != V.l;
+    const uint32_t row_n = changed ? (O.l_new > V.l ? V.row0 + V.pitch : V.row0 - V.pitch) : V.row0;
+    const uint32_t geom_n = (V.geom & GEOM_STATIC_MASK) | (O.l_new << 28) | (V.tag << 31);
+    if (O.kind == KIND_STAY) {
+        const uint32_t cell = row_n + (O.nx >> 10);
+        if (V.prev != CELL_NONE)
+            mark_move(Bn, V.prev, cell);
+        else
+            mark_toggle(Bn, cell);
+        P.pay[nxt][cell] = make_uint2(O.nx & 1023u, __float_as_uint(O.vn));
+        P.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);
+    } else {
+        if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
+        const uint32_t xpos = seg_base + atomicAdd(&sm.xn, 1u);
+        if (O.kind == KIND_DONE) {
+            P.xlist[xpos] = make_uint4(XL_DONE, cur_abs, 0u, 0u);
+            P.arrive_step[V.id] = t + 1u;
+            atomicAdd(&sm.stats[ST_DONE], 1ull);
+            atomicAdd(&sm.stats[ST_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
+            P.S0[at] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);   // dead slot
+        } else {
+            // smallest id wins; the key carries ~t in the high word so claim words never need a reset
+            const uint32_t word = GEOM_PRIO(V.geom) ? V.claim : (V.claim & ~7u) + min(O.l_new, V.claim & 7u);
+            const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)V.id;
+            atomicMin(&P.claim[word], key);
+            P.xlist[xpos] = make_uint4(slot, word, V.cursor, V.id);
+            P.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state; the cross phase decides
+        }
+    }
+    if (geom_n != V.geom) P.S1[at] = make_uint4(row_n, geom_n, V.cursor, __float_as_uint(V.v0));
+    if (changed) {   // executed lane change: the look-ahead continues in other rows now
+        atomicAdd(&sm.stats[ST_LC], 1ull);
+        const Hops hp = build_hops(P, V.cursor, V.geom, O.l_new);
+        P.S2[at] = hp.s2;
+        P.S3[at] = hp.s3;
+    }
+    if (P.acc) P.acc[at] = O.acc;
 }
 
 // R5: lead (first occupied cell >= c, within the edge) and lag (last occupied cell < c) in the target lane, then
 // the rest of the update.
 template <bool W256>
-__device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_t t, const u64 *B, const uint2 *pay, const Veh &V,
-                                                          uint32_t &n_lc)
+__device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_t t, const u64 *B, const uint2 *pay, const Veh &V)
 {
-    const uint32_t rowt = V.cell_off + V.lt * V.pitch;
+    const uint32_t rowt = V.lt > V.l ? V.row0 + V.pitch : V.row0 - V.pitch;
     uint32_t ja = 0u, jb = 0u;
     const uint32_t b0 = V.c > P.lookback ? V.c - P.lookback : 0u;
     const bool has_a = scan_fwd<W256>(B, rowt, V.c, min(V.len_c, V.c + P.H), ja);
@@ -436,56 +465,7 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
         x_b = (int32_t)((jb << 10) | pb.x);
         v_b = __uint_as_float(pb.y);
     }
-    return post_lc(P, t, V, has_a, x_a, v_a, has_b, x_b, v_b, n_lc);
-}
-
-// R9 for one warp's vehicles: survivors compacted into the segment's next buffer (warp ballot + one shared-memory
-// atomic), time-(t+1) mark and payload for stayers, time-(t-1) mark toggled off, cross-list entries.  Must be
-// called by all 32 lanes; `have` says whether this lane carries a vehicle.
-__device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, bool have, const Veh &V,
-                                          const Outcome &O)
-{
-    const int nxt = (int)((t & 1u) ^ 1u);
-    u64 *Bn = P.bits[nxt];
-    const uint32_t lane_id = threadIdx.x & 31u;
-    const bool alive = have && O.kind != KIND_DONE, listed = have && O.kind != KIND_STAY;
-    const uint32_t bal_a = __ballot_sync(0xFFFFFFFFu, alive), bal_x = __ballot_sync(0xFFFFFFFFu, listed);
-    uint32_t base_a = 0u, base_x = 0u;
-    if (lane_id == 0u) {
-        if (bal_a) base_a = atomicAdd(&sm.out, (uint32_t)__popc(bal_a));
-        if (bal_x) base_x = atomicAdd(&sm.xn, (uint32_t)__popc(bal_x));
-    }
-    base_a = __shfl_sync(0xFFFFFFFFu, base_a, 0);
-    base_x = __shfl_sync(0xFFFFFFFFu, base_x, 0);
-    if (!have) return;
-    const uint32_t lt_mask = (1u << lane_id) - 1u;
-    const uint32_t pos = base_a + __popc(bal_a & lt_mask);
-    const uint32_t xpos = seg_base + base_x + __popc(bal_x & lt_mask);
-    const uint32_t cur_abs = V.cell_off + V.l * V.pitch + V.c;
-    const uint32_t geom_n = (V.geom & GEOM_STATIC_MASK) | (O.l_new << 28) | (V.tag << 31);
-    if (O.kind == KIND_STAY) {
-        const uint32_t cell = V.cell_off + O.l_new * V.pitch + (O.nx >> 10);
-        if (V.prev != CELL_NONE)
-            mark_move(Bn, V.prev, cell);
-        else
-            mark_toggle(Bn, cell);
-        P.pay[nxt][cell] = make_uint2(O.nx & 1023u, __float_as_uint(O.vn));
-    } else {
-        if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
-        if (O.kind == KIND_DONE) {
-            P.xlist[xpos] = make_uint4(XL_DONE, cur_abs, 0u, 0u);
-            P.arrive_step[V.id] = t + 1u;
-            atomicAdd(&sm.stats[ST_DONE], 1ull);
-            atomicAdd(&sm.stats[ST_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
-        } else {
-            P.xlist[xpos] = make_uint4(pos, O.word, V.cursor, V.id);
-        }
-    }
-    if (alive) {  // candidates: tentative winner state; the cross phase decides
-        P.S0[nxt][seg_base + pos] = make_uint4(O.nx, __float_as_uint(O.vn), V.id, V.cursor);
-        P.S1[nxt][seg_base + pos] = make_uint4(V.cell_off, geom_n, cur_abs, __float_as_uint(V.v0));
-        if (P.acc[nxt]) P.acc[nxt][seg_base + pos] = O.acc;
-    }
+    return post_lc(P, t, V, has_a, x_a, v_a, has_b, x_b, v_b);
 }
 
 // ------------------------------------------------------------------------------------------------ A: R1
@@ -513,22 +493,26 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
         if (l_sel == 0xFFFFFFFFu) continue;
         const uint32_t id = ent.x, cursor = ent.z;
         const uint4 rr = P.route[cursor];
+        const uint32_t geom = (rr.y & GEOM_STATIC_MASK) | (l_sel << 28);
+        const Hops hp = build_hops(P, cursor, geom, l_sel);
         // the emptier of two pseudo-random segments (keeps the segments balanced as trips come and go)
         uint32_t hsh = mix32(k * 0x9E3779B9u + t);
         uint32_t sa = hsh % P.n_seg, sb = (sa + 1u + (hsh >> 16) % max(P.n_seg - 1u, 1u)) % P.n_seg;
-        uint32_t seg = P.seg_cnt[cur][sb] < P.seg_cnt[cur][sa] ? sb : sa;
+        uint32_t seg = P.seg_cnt[sb] < P.seg_cnt[sa] ? sb : sa;
         uint32_t slot;
         for (;;) {
-            slot = atomicAdd(&P.seg_cnt[cur][seg], 1u);
+            slot = atomicAdd(&P.seg_cnt[seg], 1u);
             if (slot < P.seg_cap) break;
-            atomicSub(&P.seg_cnt[cur][seg], 1u);       // full: the total capacity covers every trip, so another has room
+            atomicSub(&P.seg_cnt[seg], 1u);            // full: the total capacity covers every trip, so another has room
             seg = seg + 1u == P.n_seg ? 0u : seg + 1u;
         }
         const uint32_t row = er.x + l_sel * pitch;
         const size_t at = (size_t)seg * P.seg_cap + slot;
-        P.S0[cur][at] = make_uint4(0u, 0u, id, cursor);
-        P.S1[cur][at] = make_uint4(rr.x, (rr.y & GEOM_STATIC_MASK) | (l_sel << 28), CELL_NONE, rr.w);
-        if (P.acc[cur]) P.acc[cur][at] = 0.0f;
+        P.S0[at] = make_uint4(0u, 0u, CELL_NONE, id);
+        P.S1[at] = make_uint4(row, geom, cursor, rr.w);
+        P.S2[at] = hp.s2;
+        P.S3[at] = hp.s3;
+        if (P.acc) P.acc[at] = 0.0f;
         mark_toggle(B, row);                           // cell 0, frac10 = 0, v = 0: visible to this step's update
         pay[(size_t)row] = make_uint2(0u, 0u);
         P.admit_step[id] = t;
@@ -538,105 +522,163 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
     }
 }
 
+// ------------------------------------------------------------------------------------------------ A8
+// Squeezes the dead slots out of one segment, keeping the order of the live ones.  Called by all threads of the
+// block that owns the segment; returns the new slot count.  Chunk by chunk: read, barrier, write -- a slot is
+// never written before the chunk that holds it has been read (write index <= read index).
+__device__ __forceinline__ uint32_t compact_segment(const DevP &P, UpdateSmem &sm, uint32_t seg, uint32_t n)
+{
+    const size_t seg_base = (size_t)seg * P.seg_cap;
+    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
+    uint32_t out = 0u;
+    for (uint32_t base = 0u; base < n; base += blockDim.x) {
+        const uint32_t i = base + threadIdx.x;
+        uint4 a0 = make_uint4(0u, 0u, 0u, CELL_NONE), a1 = a0, a2 = a0, a3 = a0;
+        float ac = 0.0f;
+        if (i < n) {
+            a0 = P.S0[seg_base + i];
+            if (a0.w != CELL_NONE) {
+                a1 = P.S1[seg_base + i];
+                a2 = P.S2[seg_base + i];
+                a3 = P.S3[seg_base + i];
+                if (P.acc) ac = P.acc[seg_base + i];
+            }
+        }
+        const bool live = a0.w != CELL_NONE;
+        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, live);
+        if (lane_id == 0u) sm.wsum[warp_id] = (uint32_t)__popc(bal);
+        __syncthreads();   // all reads of this chunk done; warp totals visible
+        uint32_t pre = 0u, tot = 0u;
+        for (uint32_t w = 0; w < (blockDim.x >> 5); w++) {
+            const uint32_t c = sm.wsum[w];
+            pre += w < warp_id ? c : 0u;
+            tot += c;
+        }
+        if (live) {
+            const uint32_t pos = out + pre + (uint32_t)__popc(bal & ((1u << lane_id) - 1u));
+            if (pos != i) {
+                P.S0[seg_base + pos] = a0;
+                P.S1[seg_base + pos] = a1;
+                P.S2[seg_base + pos] = a2;
+                P.S3[seg_base + pos] = a3;
+                if (P.acc) P.acc[seg_base + pos] = ac;
+            }
+        }
+        out += tot;
+        __syncthreads();   // wsum may be rewritten; writes of this chunk precede the next chunk's reads
+    }
+    return out;
+}
+
 // ------------------------------------------------------------------------------------------------ U: R2-R9
-// Second pass of one warp: the lane-change evaluations it has parked, densely packed over its lanes.
+// Second pass: `take` queue entries starting at q0, one per thread, densely packed over the block.
 template <bool W256>
-__device__ __forceinline__ void drain_lc(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, uint32_t &qn, uint32_t &n_cells,
-                                         uint32_t &n_lc)
+__device__ __forceinline__ void drain_queue(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, uint32_t q0, uint32_t take,
+                                            uint32_t &n_cells)
 {
     const int cur = (int)(t & 1u);
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
-    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
-    __syncwarp();
-    while (qn > 0u) {
-        const uint32_t take = min(qn, 32u);
-        const bool have = lane_id < take;
-        Veh V;
-        Outcome O;
-        O.kind = KIND_STAY;
-        if (have) {
-            const uint4 e = sm.q[warp_id][qn - take + lane_id];
-            veh_load(V, P.S0[cur][seg_base + e.x], P.S1[cur][seg_base + e.x]);
-            V.rn = make_uint4(0u, 0u, 0u, 0u);
-            if (!V.last) V.rn = P.route[V.cursor + 1u];
-            Lead ld;
-            ld.found = e.w != 0u;
-            ld.lead_abs = (int32_t)e.y;
-            ld.v_lead = __uint_as_float(e.z);
-            pre_lc(P, t, V, ld);
-            O = lane_change_and_finish<W256>(P, t, B, pay, V, n_lc);
-        }
-        write_out(P, t, sm, seg_base, have, V, O);
-        qn -= take;
+    if (threadIdx.x >= take) return;
+    const uint4 e = sm.q[q0 + threadIdx.x];
+    Veh V;
+    veh_load(V, P.S0[seg_base + e.x], P.S1[seg_base + e.x]);
+    V.claim = P.S3[seg_base + e.x].w;
+    Lead ld;
+    if (e.w == 2u) {   // the window did not fit the fast search
+        Hit h = walk_rows(P, B, V, n_cells);
+        ld = lead_from_hit<W256>(pay, h);
+    } else {
+        ld.found = e.w != 0u;
+        ld.lead_abs = (int32_t)e.y;
+        ld.v_lead = __uint_as_float(e.z);
     }
-    __syncwarp();
+    pre_lc(P, t, V, ld);
+    Outcome O;
+    if (V.need_lc) {
+        atomicAdd(&sm.stats[ST_EVAL], 1ull);
+        O = lane_change_and_finish<W256>(P, t, B, pay, V);
+    } else {
+        O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+    }
+    write_out(P, t, sm, seg_base, e.x, V, O);
 }
 
 // Must be called by ALL threads of the block (contains __syncthreads).
 template <bool W256>
-__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm)
+__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd)
 {
-    const int cur = (int)(t & 1u), nxt = cur ^ 1;
+    const int cur = (int)(t & 1u);
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
-    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
-        const uint32_t n = P.seg_cnt[cur][seg];
+        uint32_t n = P.seg_cnt[seg];
         const uint32_t seg_base = seg * P.seg_cap;
         if (threadIdx.x == 0u) {
-            sm.out = 0u;
             sm.xn = 0u;
+            sm.qn = 0u;
         }
         __syncthreads();
-        uint32_t n_cells = 0u, n_lc = 0u, qn = 0u;
-        for (uint32_t base = warp_id * 32u; base < n; base += blockDim.x) {
+        if (t % MANTA_COMPACT_EVERY == 0u && n > 0u) {
+            n = compact_segment(P, sm, seg, n);
+            if (threadIdx.x == 0u) P.seg_cnt[seg] = n;
+        }
+        for (uint32_t base = 0u; base < n; base += blockDim.x) {
             // ---- first pass: everything but the adjacent-lane look-up
-            const uint32_t i = base + lane_id;
-            const bool have = i < n;
-            Veh V;
-            Outcome O;
-            O.kind = KIND_STAY;
-            Lead ld;
-            ld.found = false;
-            ld.lead_abs = 0;
-            ld.v_lead = 0.0f;
-            bool want_q = false;
-            if (have) {
-                veh_load(V, P.S0[cur][seg_base + i], P.S1[cur][seg_base + i]);
-                ld = leader_search<W256>(P, B, pay, V, n_cells);
-                pre_lc(P, t, V, ld);
-                want_q = V.need_lc;
-                if (!want_q) O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f, n_lc);
+            const uint32_t i = base + threadIdx.x;
+            uint4 s0v = make_uint4(0u, 0u, 0u, CELL_NONE);
+            if (i < n) s0v = P.S0[seg_base + i];
+            if (s0v.w != CELL_NONE) {   // live slot
+                const uint4 s1v = P.S1[seg_base + i];
+                const uint4 s2v = P.S2[seg_base + i];
+                const uint4 s3v = P.S3[seg_base + i];
+                Veh V;
+                veh_load(V, s0v, s1v);
+                V.claim = s3v.w;
+                n_upd += 1u;
+                Hit h;
+                bool fits;
+                if (W256) {
+                    fits = leader_cells_fast(P, B, V, s2v, s3v, h, n_cells);
+                } else {
+                    h = walk_rows(P, B, V, n_cells);
+                    fits = true;
+                }
+                uint32_t qkind = 0xFFFFFFFFu;
+                Lead ld;
+                ld.found = false;
+                ld.lead_abs = 0;
+                ld.v_lead = 0.0f;
+                if (fits) {
+                    ld = lead_from_hit<W256>(pay, h);
+                    pre_lc(P, t, V, ld);
+                    if (V.need_lc) qkind = ld.found ? 1u : 0u;
+                } else {
+                    qkind = 2u;
+                }
+                if (qkind != 0xFFFFFFFFu) {   // parked: the second pass finishes this vehicle
+                    const uint32_t qp = atomicAdd(&sm.qn, 1u);
+                    sm.q[qp] = make_uint4(i, (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), qkind);
+                } else {
+                    const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+                    write_out(P, t, sm, seg_base, i, V, O);
+                }
             }
-            const uint32_t bal_q = __ballot_sync(0xFFFFFFFFu, want_q);
-            if (want_q)   // parked: vehicles that must look at the adjacent lane (R5) do not hold the warp
-                sm.q[warp_id][qn + __popc(bal_q & ((1u << lane_id) - 1u))] =
-                    make_uint4(i, (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), ld.found ? 1u : 0u);
-            write_out(P, t, sm, seg_base, have && !want_q, V, O);
-            if (bal_q) {
-                qn += (uint32_t)__popc(bal_q);
-                if (lane_id == 0u) atomicAdd(&sm.stats[ST_EVAL], (u64)__popc(bal_q));
-                if (qn >= 32u) drain_lc<W256>(P, t, sm, seg_base, qn, n_cells, n_lc);
+            __syncthreads();
+            const uint32_t qn = sm.qn;
+            if (qn >= blockDim.x) {   // block-uniform
+                drain_queue<W256>(P, t, sm, seg_base, qn - blockDim.x, blockDim.x, n_cells);
+                __syncthreads();
+                if (threadIdx.x == 0u) sm.qn = qn - blockDim.x;
+                __syncthreads();
             }
         }
-        drain_lc<W256>(P, t, sm, seg_base, qn, n_cells, n_lc);
-        // ---- per-segment bookkeeping
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
-            n_lc += __shfl_down_sync(0xFFFFFFFFu, n_lc, d);
-        }
-        if (lane_id == 0u) {
-            if (n_cells) atomicAdd(&sm.stats[ST_CELLS], (u64)n_cells);
-            if (n_lc) atomicAdd(&sm.stats[ST_LC], (u64)n_lc);
+        {
+            const uint32_t qn = sm.qn;   // < blockDim.x; visible to all since the last barrier
+            drain_queue<W256>(P, t, sm, seg_base, 0u, qn, n_cells);
         }
         __syncthreads();
-        if (threadIdx.x == 0u) {
-            P.seg_cnt[nxt][seg] = sm.out;
-            P.seg_xn[seg] = sm.xn;
-            sm.stats[ST_UPD] += (u64)n;
-        }
+        if (threadIdx.x == 0u) P.seg_xn[seg] = sm.xn;
     }
 }
 
@@ -656,31 +698,48 @@ __device__ __forceinline__ void cross_phase(const DevP &P, uint32_t t)
                 mark_toggle(Bc, xl.y);    // an arrival leaves no time-(t+1) state to clear its time-t mark later
                 continue;
             }
-            uint4 s0 = P.S0[nxt][seg_base + xl.x];
-            uint4 s1 = P.S1[nxt][seg_base + xl.x];
+            const size_t at = seg_base + xl.x;
+            uint4 s0 = P.S0[at];
+            const uint4 s1 = P.S1[at];
             const u64 won = P.claim[xl.y];
             const uint4 rn = P.route[xl.z + 1u];
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)xl.w;
+            uint32_t cell;
             if (won == key) {             // winner crosses (R8)
                 const uint32_t lplus = min(GEOM_LANE(s1.y), GEOM_LANES(rn.y) - 1u);
-                s0.w += 1u;
-                s1 = make_uint4(rn.x, (rn.y & GEOM_STATIC_MASK) | (lplus << 28), s1.z, rn.w);
+                const uint32_t geom = (rn.y & GEOM_STATIC_MASK) | (lplus << 28);
+                const uint32_t row = rn.x + lplus * pitch_of(GEOM_LEN(rn.y));
+                const Hops hp = build_hops(P, xl.z + 1u, geom, lplus);
+                P.S1[at] = make_uint4(row, geom, xl.z + 1u, rn.w);
+                P.S2[at] = hp.s2;
+                P.S3[at] = hp.s3;
                 atomicAdd(&P.edge_entries[rn.z], 1u);
+                cell = row + (s0.x >> 10);
             } else {                      // loser holds at the stop line (G15)
                 s0.x = (GEOM_LEN(s1.y) << 10) - 1u;
                 s0.y = 0u;
+                P.S0[at] = s0;
+                cell = s1.x + (s0.x >> 10);
             }
-            P.S0[nxt][seg_base + xl.x] = s0;
-            P.S1[nxt][seg_base + xl.x] = s1;
-            const uint32_t cell = s1.x + GEOM_LANE(s1.y) * pitch_of(GEOM_LEN(s1.y)) + (s0.x >> 10);
             mark_toggle(Bn, cell);
             payn[cell] = make_uint2(s0.x & 1023u, s0.y);
         }
     }
 }
 
-__device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm)
+// per-thread counters -> shared -> this block's record (once per kernel)
+__device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint32_t n_cells32, uint32_t n_upd32)
 {
+    u64 n_cells = n_cells32, n_upd = n_upd32;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
+        n_upd += __shfl_down_sync(0xFFFFFFFFu, n_upd, d);
+    }
+    if ((threadIdx.x & 31u) == 0u) {
+        if (n_cells) atomicAdd(&sm.stats[ST_CELLS], n_cells);
+        if (n_upd) atomicAdd(&sm.stats[ST_UPD], n_upd);
+    }
     __syncthreads();
     if (threadIdx.x == 0u) {
         BlockStats *b = &P.blk[blockIdx.x];
@@ -705,8 +764,9 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, u
     __shared__ UpdateSmem sm;
     if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
     __syncthreads();
-    update_phase<W256>(P, t, sm);
-    flush_stats(P, sm);
+    uint32_t n_cells = 0u, n_upd = 0u;
+    update_phase<W256>(P, t, sm, n_cells, n_upd);
+    flush_stats(P, sm, n_cells, n_upd);
 }
 
 __global__ void __launch_bounds__(256) k_cross(const DevP P, uint32_t t) { cross_phase(P, t); }
@@ -753,16 +813,17 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
     __shared__ UpdateSmem sm;
     if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
     unsigned gen = 0u;
+    uint32_t n_cells = 0u, n_upd = 0u;
     const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
     for (uint32_t t = t0; t < t0 + n_steps; t++) {
         admit_phase(P, t, gtid, gsize);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-        update_phase<W256>(P, t, sm);
+        update_phase<W256>(P, t, sm, n_cells, n_upd);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         cross_phase(P, t);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     }
-    flush_stats(P, sm);
+    flush_stats(P, sm, n_cells, n_upd);
 }
 
 // ------------------------------------------------------------------------------------------------ set-up kernels
@@ -799,41 +860,46 @@ __global__ void k_mark_last(const uint64_t *route_ptr, uint32_t n_trips, uint4 *
         route[k] = r;
     }
 }
-// Pre-placed vehicles (R1, last sentence): vehicle i of the list goes to segment i % n_seg; fill S1 from the route
-// store, mark atlas_0, count the entry.
+// Pre-placed vehicles (R1, last sentence): vehicle i of the list goes to segment i % n_seg; fill the state from the
+// route store, mark atlas_0, count the entry.  init = {x_fx, v bits, vehicle id, route cursor}.
 __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init)
 {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_init; i += gridDim.x * blockDim.x) {
-        const uint4 s0v = init[i];
-        const uint4 rr = P.route[s0v.w];
+        const uint4 iv = init[i];
+        const uint4 rr = P.route[iv.w];
         const size_t at = (size_t)(i % P.n_seg) * P.seg_cap + i / P.n_seg;
-        P.S0[0][at] = s0v;
-        P.S1[0][at] = make_uint4(rr.x, rr.y & GEOM_STATIC_MASK, CELL_NONE, rr.w);  // lane 0, tag 0, no earlier mark
-        const uint32_t cell = rr.x + (s0v.x >> 10);
+        const uint32_t geom = rr.y & GEOM_STATIC_MASK;      // lane 0, tag 0
+        const Hops hp = build_hops(P, iv.w, geom, 0u);
+        P.S0[at] = make_uint4(iv.x, iv.y, CELL_NONE, iv.z);   // no earlier mark
+        P.S1[at] = make_uint4(rr.x, geom, iv.w, rr.w);
+        P.S2[at] = hp.s2;
+        P.S3[at] = hp.s3;
+        const uint32_t cell = rr.x + (iv.x >> 10);
         mark_toggle(P.bits[0], cell);
-        P.pay[0][cell] = make_uint2(s0v.x & 1023u, s0v.y);
-        P.admit_step[s0v.z] = 0u;
+        P.pay[0][cell] = make_uint2(iv.x & 1023u, iv.y);
+        P.admit_step[iv.z] = 0u;
         atomicAdd(&P.edge_entries[rr.z], 1u);
     }
 }
-// Readback: scatter the active segments into per-trip arrays (caller order).
-__global__ void k_gather_state(const DevP P, int cur, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
+// Readback: scatter the live slots of the segments into per-trip arrays (caller order).
+__global__ void k_gather_state(const DevP P, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
                                uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc)
 {
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
-        const uint32_t n = P.seg_cnt[cur][seg];
+        const uint32_t n = P.seg_cnt[seg];
         const size_t seg_base = (size_t)seg * P.seg_cap;
         for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
-            const uint4 s0v = P.S0[cur][seg_base + i];
-            const uint4 s1v = P.S1[cur][seg_base + i];
-            const uint32_t tr = trip_of_id[s0v.z];
+            const uint4 s0v = P.S0[seg_base + i];
+            if (s0v.w == CELL_NONE) continue;
+            const uint4 s1v = P.S1[seg_base + i];
+            const uint32_t tr = trip_of_id[s0v.w];
             status[tr] = 1u;
-            route_pos[tr] = s0v.w - P.route_start[s0v.z];
+            route_pos[tr] = s1v.z - P.route_start[s0v.w];
             lane[tr] = (uint8_t)GEOM_LANE(s1v.y);
             tag[tr] = (uint8_t)GEOM_TAG(s1v.y);
             x_fx[tr] = s0v.x;
             v[tr] = __uint_as_float(s0v.y);
-            acc[tr] = P.acc[cur] ? P.acc[cur][seg_base + i] : 0.0f;
+            acc[tr] = P.acc ? P.acc[seg_base + i] : 0.0f;
         }
     }
 }
