@@ -117,13 +117,15 @@ class ClockSampler:
 
 
 def algorithmic_bytes(hbar, flc, lookback):
-    """Algorithmic bytes per vehicle-update of the 1-bit-occupancy layout.
-    update phase: state read 32 + compacted state write 32, next route record 16, own-lane occupancy bits
-    hbar / 8, leader payload 8, new mark (8-byte word) 8 + payload 8, clearing of the old mark 8; a lane-change
-    evaluation adds the target row's bits ahead and behind plus two payloads.  The whole step adds the cross
-    list entry and the second state pass of the ~2 % of vehicles at an edge end (folded in as 2 B)."""
-    upd = 32.0 + 32.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0 + flc * ((hbar + lookback) / 8.0 + 16.0)
-    return upd, upd + 2.0
+    """Algorithmic bytes per vehicle-update, 1-bit occupancy plane + 8-byte payload plane +
+    64-byte in-place vehicle state.  Update phase: state read 64 (position / speed, edge geometry, cached rows and
+    lengths of the next four route edges) + rewritten position word 16, own-lane occupancy bits hbar / 8, leader
+    payload 8, new mark (8-byte word) 8 + own payload 8, toggling the old mark off 8; a deferred adjacent-lane
+    evaluation adds its list entry (16 written + 16 read), the target row's bits ahead and behind and two payloads.
+    The whole step adds the cross-list entry and claim of the ~2 % of vehicles at an edge end and the amortised
+    re-sort (128 B per vehicle every MANTA_SORT_EVERY = 32 steps), folded in as 6 B."""
+    upd = 64.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0 + flc * (32.0 + (hbar + lookback) / 8.0 + 16.0)
+    return upd, upd + 6.0
 
 
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
@@ -276,7 +278,7 @@ def main():
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_update": bytes_update, "updates_per_launch": upd_per_launch,
                 "avg_launch_us": t_update * 1e6, "hbar_cells": hbar, "f_lc": flc,
-                "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "commit": ph[2] / Kp},
+                "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp},
                 "step_bytes_per_update": bytes_step,
                 "step_frac": bytes_step * value / world / 1e9 / peak}
 

@@ -50,6 +50,8 @@ extern "C" {
 /* manta_params.flags */
 #define MANTA_FLAG_MULTI_KERNEL 2u     /* three launches per timestep instead of the persistent cooperative kernel */
 #define MANTA_FLAG_RECORD_ACC 4u       /* keep each vehicle's last acceleration for manta_state.acc (tests)  */
+#define MANTA_FLAG_NO_L2_PIN 8u        /* do not pin the occupancy planes in L2 (A/B switch; the default sets the
+                                          device's cudaLimitPersistingL2CacheSize to the size of the two planes)   */
 
 typedef struct manta_sim manta_sim; /* opaque; owned by the library; one simulation on one device */
 
@@ -138,7 +140,7 @@ int manta_step_async(manta_sim *sim, uint32_t n_steps);
 int manta_sync(manta_sim *sim);
 
 /* Same as manta_step, with CUDA events recorded on the simulation's stream around every phase; adds the device
- * time of the admission, update and commit phases (milliseconds, summed over the n_steps) to phase_ms[0..2].
+ * time of the admission, update and second (claim resolution) phases (ms, summed over the n_steps) to phase_ms[0..2].
  * For measurement only (the events cost a little); results are identical to manta_step. */
 int manta_step_timed(manta_sim *sim, uint32_t n_steps, double phase_ms[3]);
 

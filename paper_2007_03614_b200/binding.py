@@ -178,7 +178,7 @@ class Sim:
         self._check(load_library().manta_step_async(self.h, int(n)))
 
     def step_timed(self, n=1):
-        """manta_step with per-phase CUDA-event timing; returns [admit_ms, update_ms, commit_ms] summed over n."""
+        """manta_step with per-phase CUDA-event timing; returns [admit_ms, update_ms, second_phase_ms] summed over n."""
         ms = (C.c_double * 3)(0.0, 0.0, 0.0)
         self._check(load_library().manta_step_timed(self.h, int(n), C.byref(ms)))
         return [float(x) for x in ms]

@@ -53,6 +53,9 @@ struct manta_sim {
     int sm_count = 148;
     int grid_step = 1, grid_admit = 1, grid_persist = 0;   // blocks of the segment kernels / admission / persistent kernel
     bool w256 = true;             // look-ahead <= 256 cells and look-back <= 128: whole-window scans
+    void *l2_window_base = nullptr;   // occupancy planes: L2 access-policy window of the step kernels
+    uint64_t l2_window_bytes = 0;
+    size_t l2_persist = 0;            // persisting L2 carve-out granted (0 = no pinning)
     uint32_t n_blk_stats = 0;
 };
 
@@ -284,8 +287,30 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     if ((rc = alloc_fill(s, &d_ctr, 1, 0))) return bail(rc);
     s->n_blk_stats = (uint32_t)s->sm_count * 16u;
     if ((rc = alloc_fill(s, &d_blk, s->n_blk_stats, 0))) return bail(rc);
-    for (int k = 0; k < 2; k++)
-        if ((rc = alloc_fill(s, &P.bits[k], cells / 64 + 8, 0))) return bail(rc);
+    {   // both occupancy planes in one allocation, so that one L2 access-policy window covers them
+        const uint64_t plane_words = ((cells / 64 + 8) + 15) & ~15ull;
+        u64 *planes;
+        if ((rc = alloc_fill(s, &planes, 2 * plane_words, 0))) return bail(rc);
+        P.bits[0] = planes;
+        P.bits[1] = planes + plane_words;
+        // The occupancy planes are the most re-read data of a step (every look-ahead reads them, every vehicle
+        // toggles two marks); pin them in L2 so that the streamed state and payload sectors do not evict them.
+        s->l2_window_base = planes;
+        s->l2_window_bytes = 2 * plane_words * sizeof(u64);
+        int max_persist = 0, max_window = 0;
+        cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cuda_device);
+        cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, cuda_device);
+        s->l2_persist = 0;
+        if (!(p.flags & MANTA_FLAG_NO_L2_PIN) && max_persist > 0 && max_window > 0) {
+            const size_t want = (size_t)std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_persist);
+            if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
+                s->l2_persist = want;
+                s->l2_window_bytes = std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_window);
+            } else {
+                cudaGetLastError();
+            }
+        }
+    }
     for (int k = 0; k < 2; k++)
         if ((rc = alloc_fill(s, &P.pay[k], cells + 64, 0))) return bail(rc);
     P.edge_tab = d_et; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
@@ -411,7 +436,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     }
     DevP &P = s->P;
     P.n_seg = (uint32_t)s->grid_step;
-    P.seg_cap = (n_trips + P.n_seg - 1u) / P.n_seg + 64u;
+    P.seg_cap = (n_trips + P.n_seg - 1u) / P.n_seg + 256u;
     const uint64_t cap = (uint64_t)P.n_seg * P.seg_cap;
     if (cap >= 0xFFFFFFFFull) return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
     // ---- upload; expand the route store on the device
@@ -440,19 +465,32 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if ((rc = upload(s, &d_qent, q_ent.data(), q_ent.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
     if ((rc = upload(s, &d_qn, q_next.data(), q_next.size()))) return rollback(rc);
-    {
-        uint4 **arr[4] = {&P.S0, &P.S1, &P.S2, &P.S3};
-        for (int k = 0; k < 4; k++) {
-            *arr[k] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
-            if (!*arr[k]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+    for (int k = 0; k < 2; k++) {
+        uint4 **arr[4] = {&P.st[k].S0, &P.st[k].S1, &P.st[k].S2, &P.st[k].S3};
+        for (int a = 0; a < 4; a++) {
+            *arr[a] = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
+            if (!*arr[a]) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
         }
-        P.acc = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, cap * sizeof(float)) : nullptr;
-        if (P.acc) CUDA_TRY(s, cudaMemsetAsync(P.acc, 0, cap * sizeof(float), s->stream));
-        if ((rc = alloc_fill(s, &P.seg_cnt, P.n_seg, 0))) return rollback(rc);
+        P.st[k].acc = (s->prm.flags & MANTA_FLAG_RECORD_ACC) ? (float *)dev_alloc(s, cap * sizeof(float)) : nullptr;
+        if (P.st[k].acc) CUDA_TRY(s, cudaMemsetAsync(P.st[k].acc, 0, cap * sizeof(float), s->stream));
+    }
+    if ((rc = alloc_fill(s, &P.seg_cnt, P.n_seg, 0))) return rollback(rc);
+    {   // re-sort scratch; until the first sort admission spreads the origins evenly over the segments
+        P.n_buckets = (uint32_t)((s->n_cells + (1ull << MANTA_BUCKET_SHIFT) - 1) >> MANTA_BUCKET_SHIFT) + 1u;
+        if ((rc = alloc_fill(s, &P.sort_hist, (uint64_t)P.n_buckets + 1, 0))) return rollback(rc);
+        if ((rc = alloc_fill(s, &P.sort_part, (uint64_t)P.n_seg + 2, 0))) return rollback(rc);
+        if ((rc = alloc_fill(s, &P.sort_rank, cap, 0xFF))) return rollback(rc);
+        std::vector<uint32_t> bs(P.n_buckets);
+        for (uint32_t b = 0; b < P.n_buckets; b++) bs[b] = (uint32_t)(((uint64_t)b * P.n_seg) / P.n_buckets);
+        if ((rc = upload(s, &P.bucket_seg, bs.data(), bs.size()))) return rollback(rc);
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // bs goes out of scope
     }
     if ((rc = alloc_fill(s, &P.seg_xn, P.n_seg, 0))) return rollback(rc);
+    if ((rc = alloc_fill(s, &P.dbg_buf, (uint64_t)P.n_seg * 8, 0))) return rollback(rc);
+    if ((rc = alloc_fill(s, &P.seg_qn, P.n_seg, 0))) return rollback(rc);
     P.xlist = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
-    if (!P.xlist) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
+    P.dlist = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
+    if (!P.xlist || !P.dlist) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
     P.route = d_route; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
     P.q_row = d_qrow; P.q_ent = d_qent; P.q_head = d_qh; P.q_next = d_qn; P.q_ptr = nullptr;
     P.n_queues = (uint32_t)q_edge.size();
@@ -490,18 +528,58 @@ int check_ready(manta_sim *s, uint32_t n_steps)
     return MANTA_OK;
 }
 
+// Launch attributes of the step kernels: L2 access-policy window over the occupancy planes (+ cooperative).
+int step_attrs(const manta_sim *s, cudaLaunchAttribute *at, bool coop)
+{
+    int n = 0;
+    if (s->l2_persist) {
+        at[n].id = cudaLaunchAttributeAccessPolicyWindow;
+        at[n].val.accessPolicyWindow.base_ptr = s->l2_window_base;
+        at[n].val.accessPolicyWindow.num_bytes = (size_t)s->l2_window_bytes;
+        at[n].val.accessPolicyWindow.hitRatio = (float)std::min(1.0, (double)s->l2_persist / (double)s->l2_window_bytes);
+        at[n].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        at[n].val.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+        n++;
+    }
+    if (coop) {
+        at[n].id = cudaLaunchAttributeCooperative;
+        at[n].val.cooperative = 1;
+        n++;
+    }
+    return n;
+}
+extern "C++" template <class... KArgs, class... Args>
+cudaError_t launch_k(const manta_sim *s, void (*kern)(KArgs...), int grid, int block, bool coop, Args... args)
+{
+    cudaLaunchAttribute at[2];
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s->stream;
+    cfg.attrs = at;
+    cfg.numAttrs = (unsigned)step_attrs(s, at, coop);
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 // three launches per timestep (MANTA_FLAG_MULTI_KERNEL, manta_step_timed, devices without cooperative launch)
 void launch_step_multi(manta_sim *s, uint32_t t, cudaEvent_t *ev)
 {
+    if (t != 0u && t % MANTA_SORT_EVERY == 0u) {   // spatial re-sort of the vehicle slots (five stages)
+        const int from = (int)(((t - 1u) / MANTA_SORT_EVERY) & 1u);
+        launch_k(s, k_sort_zero, s->grid_step, MANTA_NT, false, s->P);
+        launch_k(s, k_sort_count, s->grid_step, MANTA_NT, false, s->P, from);
+        launch_k(s, k_sort_partial, s->grid_step, MANTA_NT, false, s->P);
+        launch_k(s, k_sort_scan, s->grid_step, MANTA_NT, false, s->P);
+        launch_k(s, k_sort_scatter, s->grid_step, MANTA_NT, false, s->P, from);
+        s->launches += 5;
+    }
     if (ev) cudaEventRecord(ev[0], s->stream);
-    k_admit<<<s->grid_admit, 256, 0, s->stream>>>(s->P, t);
+    launch_k(s, k_admit, s->grid_admit, 256, false, s->P, t);
     if (ev) cudaEventRecord(ev[1], s->stream);
-    if (s->w256)
-        k_update<true><<<s->grid_step, MANTA_NT, 0, s->stream>>>(s->P, t);
-    else
-        k_update<false><<<s->grid_step, MANTA_NT, 0, s->stream>>>(s->P, t);
+    launch_k(s, s->w256 ? k_update<true> : k_update<false>, s->grid_step, MANTA_NT, false, s->P, t);
     if (ev) cudaEventRecord(ev[2], s->stream);
-    k_cross<<<s->grid_step, 256, 0, s->stream>>>(s->P, t);
+    launch_k(s, k_second, s->grid_step, 256, false, s->P, t);
     if (ev) cudaEventRecord(ev[3], s->stream);
     s->launches += 3;
 }
@@ -519,10 +597,8 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
         // one cooperative launch per chunk of timesteps; the grid barrier words restart from zero every launch
         for (uint32_t done = 0; done < n_steps;) {
             uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s->t;
-            CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 2 * sizeof(unsigned int), s->stream));
-            void *args[] = {(void *)&s->P, (void *)&t0, (void *)&m};
-            const void *fn = s->w256 ? (const void *)k_persistent<true> : (const void *)k_persistent<false>;
-            CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3((unsigned)s->grid_persist), dim3(MANTA_NT), args, 0, s->stream));
+            CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 33 * sizeof(unsigned int), s->stream));   // bar_count .. bar_gen
+            CUDA_TRY(s, launch_k(s, s->w256 ? k_persistent<true> : k_persistent<false>, s->grid_persist, MANTA_NT, true, s->P, t0, m));
             s->launches += 1;
             s->t += m;
             done += m;
@@ -556,6 +632,16 @@ int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
     for (auto &e : ev) cudaEventDestroy(e);
     return MANTA_OK;
 }
+
+#ifdef MANTA_DBG
+int manta_debug_read(manta_sim *s, uint64_t *out, uint32_t n_words)
+{
+    cudaStreamSynchronize(s->stream);
+    const uint32_t n = std::min<uint32_t>(n_words, s->P.n_seg * 8u);
+    cudaMemcpy(out, s->P.dbg_buf, (size_t)n * 8, cudaMemcpyDeviceToHost);
+    return (int)s->P.n_seg;
+}
+#endif
 
 int manta_sync(manta_sim *s)
 {
@@ -602,7 +688,7 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
         CUDA_TRY(s, cudaMemsetAsync(buf, 0, nn * (3 + 16 + 8), s->stream));
         const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
         k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
-        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
+        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->t == 0 ? 0 : (int)(((s->t - 1u) / MANTA_SORT_EVERY) & 1u), s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
         CUDA_TRY(s, cudaGetLastError());
         std::vector<uint8_t> h_status(n);
         CUDA_TRY(s, cudaMemcpyAsync(h_status.data(), d_status, n, cudaMemcpyDeviceToHost, s->stream));

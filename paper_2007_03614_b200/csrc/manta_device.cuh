@@ -37,19 +37,28 @@ typedef unsigned long long u64;
 // look-ahead: what the look-ahead needs of the next four route edges is cached in the vehicle's state (S2, S3).
 //
 // Active vehicles: n_seg SEGMENTS of seg_cap slots, four uint4 per vehicle (64 bytes), updated IN PLACE.
-// A segment is processed by one thread block per phase.  A vehicle keeps its slot from admission (appended at
-// seg_cnt, admission picks the emptier of two segments) to arrival (slot marked dead: id = NONE); every
-// MANTA_COMPACT_EVERY timesteps the owning block squeezes the dead slots out (order-preserving, no global sync).
+// A segment is processed by one thread block per phase.  Every MANTA_SORT_EVERY timesteps all live slots are
+// re-sorted by atlas position (counting sort on absolute cell >> MANTA_BUCKET_SHIFT, into the second state buffer)
+// and dealt out in equal shares: segment s then holds the vehicles of one contiguous stretch of the atlas, so a
+// block's look-ahead, payload and mark traffic stays inside a few hundred KB that its SM's L1 and one L2 partition
+// can hold, and DRAM sees runs of neighbouring sectors instead of single random ones.  Dead slots (arrived
+// vehicles, id = NONE) are dropped by the same pass.  Between two sorts a vehicle keeps its slot; admission
+// appends to the segment that currently covers the origin edge's stretch.
 //   S0 = { x_fx, v bits, absolute cell of the time-(t-1) mark or NONE, vehicle id or NONE (dead slot) }
 //   S1 = { row0 = absolute cell at which the row of the vehicle's own lane starts, geom (+ lane, tag),
 //          route cursor (absolute RouteRec index), v0 bits }
 //   S2 = { word index (cell >> 6) of the row the look-ahead continues in on route edges +1, +2, +3, +4
 //          (lane clamped hop by hop, R2) }
 //   S3 = { len_c of edges +1 | +2 << 16, len_c of edges +3 | +4 << 16 (0 = the route ended before),
-//          1 if the route goes on past edge +4, claim word of R8 for this edge's end }
-// A stayer rewrites S0 only (S1 when its tag or lane changed, S2/S3 when its lane changed).
-// Cross list (per segment): 16-byte entries made by the update phase for the few vehicles that need the second
-// phase (edge-end candidates, whose claim must be resolved, and arrivals, whose time-t mark must be cleared).
+//          bit 0: the route goes on past edge +4, bits 1-3: the (clamped) lane the look-ahead is in on edge +4,
+//          claim word of R8 for this edge's end }
+// A stayer rewrites S0 only (S1 when its tag or lane changed, S2/S3 when its lane changed).  A vehicle that
+// arrives leaves a GHOST in its slot for one step, which toggles the vehicle's last mark off (that mark is in the
+// plane everybody reads during the arrival step, so it cannot be cleared earlier) and then frees the slot.
+// Two per-segment lists of 16-byte entries carry the few vehicles that need the second phase: the CROSS list
+// (edge-end candidates, whose claim must be resolved) and the DEFERRED list (vehicles that must look at the
+// adjacent lane, R5, or whose look-ahead window does not fit the fast search; neither can reach its edge end in
+// this step, so nothing they do can matter to a claim).
 // ---------------------------------------------------------------------------------------------------------
 
 #define GEOM_LEN(g) ((g) & 0xFFFFu)
@@ -62,21 +71,31 @@ typedef unsigned long long u64;
 #define GEOM_TAG(g) ((g) >> 31)
 #define GEOM_STATIC_MASK 0x0FFFFFFFu
 #define CELL_NONE 0xFFFFFFFFu
-#define XL_DONE 0x80000000u
-#ifndef MANTA_COMPACT_EVERY
-#define MANTA_COMPACT_EVERY 64u   // timesteps between two squeezes of the dead vehicle slots of a segment
+#define ID_GHOST 0xFFFFFFFEu   // slot of a vehicle that arrived in the previous step: clears its last mark, then dies
+#ifndef MANTA_SORT_EVERY
+#define MANTA_SORT_EVERY 32u      // timesteps between two spatial re-sorts of the vehicle slots
+#endif
+#ifndef MANTA_BUCKET_SHIFT
+#define MANTA_BUCKET_SHIFT 8      // sort key = absolute atlas cell >> this
 #endif
 
 enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
 
-struct Counters {
-    unsigned int bar_count, bar_gen;     // grid barrier of the persistent kernel
-    unsigned int abort, pad;
+struct Counters {                        // grid barrier of the persistent kernel; one 128-byte line per word, so
+    unsigned int bar_count, pad0[31];    // the arrival atomics, the generation polls and the abort flag do not
+    unsigned int bar_gen, pad1[31];      // queue up on one L2 sector
+    unsigned int abort, pad2[31];
 };
 
 // per-block private statistics and result counters (no global atomics on the hot path; summed at readback)
 struct BlockStats {
     u64 lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel, pad0, pad1;
+};
+
+// one buffer of vehicle state (see the layout comment); acc is optional (MANTA_FLAG_RECORD_ACC)
+struct StBuf {
+    uint4 *S0, *S1, *S2, *S3;
+    float *acc;
 };
 
 struct DevP {
@@ -96,11 +115,18 @@ struct DevP {
     // routes
     const uint4 *route;
     // vehicles: segment s occupies slots [s * seg_cap, s * seg_cap + seg_cnt[s]) (live and dead slots)
-    uint4 *S0, *S1, *S2, *S3;
+    StBuf st[2];                 // step t uses buffer sbuf_of(t); the periodic spatial re-sort copies into the other one
     uint32_t *seg_cnt;
-    uint4 *xlist;                // cross list of segment s at [s * seg_cap, ...): {slot | XL_DONE, claim word | cell, cursor, id}
+    uint4 *xlist;                // cross list of segment s at [s * seg_cap, ...): {slot, claim word, cursor, id}
+    uint4 *dlist;                // deferred list of segment s, same place: {slot, lead_abs, v_lead bits, 0 | 1 found | 2 search to do}
     uint32_t *seg_xn;            // cross-list entries of each segment (written by the update phase)
-    float *acc;                  // optional (MANTA_FLAG_RECORD_ACC): acceleration applied in the last step, per slot
+    uint32_t *seg_qn;            // (unused)
+    // spatial re-sort (every MANTA_SORT_EVERY steps): counting sort of the live slots by atlas bucket
+    uint32_t n_buckets;          // buckets of 2^MANTA_BUCKET_SHIFT atlas cells
+    uint32_t *sort_hist;         // [n_buckets + 1] counts, then exclusive offsets
+    uint32_t *sort_part;         // [n_seg] per-block partial sums of the scan; [n_seg] = live total
+    uint32_t *sort_rank;         // [n_seg * seg_cap] rank of each slot inside its bucket (NONE = dead)
+    uint32_t *bucket_seg;        // [n_buckets] segment that holds the bucket's vehicles: where admission appends
     // per vehicle id
     const uint32_t *route_start;
     uint32_t *admit_step;
@@ -116,9 +142,11 @@ struct DevP {
     uint32_t *edge_entries;
     const uint32_t *P_mlc;       // [5 * Lam + 1]
     Counters *ctr;
+    u64 *dbg_buf;               // [n_seg * 8] timestamps (MANTA_DBG builds only)
     BlockStats *blk;
 };
 
+__device__ __forceinline__ int sbuf_of(uint32_t t) { return (int)((t / MANTA_SORT_EVERY) & 1u); }
 __device__ __forceinline__ uint32_t pitch_of(uint32_t len_c) { return (len_c + 63u) & ~63u; }
 
 // ------------------------------------------------------------------------------------------- G22: rng(id, t, k)
@@ -241,6 +269,30 @@ __device__ __forceinline__ void mark_move(u64 *B, uint32_t cell_old, uint32_t ce
     }
 }
 
+// Payload of the vehicle in `cell`: written as the whole aligned 32-byte sector (four cells).  Vehicles in one row
+// are at least L >= 4 m apart, so no second vehicle can be in the same aligned group of four cells at the same
+// time: the other three entries are nobody's, and a full-sector store needs no read-modify-write in L2 / DRAM.
+__device__ __forceinline__ void pay_store(const DevP &P, uint2 *pay, uint32_t cell, uint32_t frac, uint32_t vbits)
+{
+    if (P.L_fx < 4096) {   // vehicles shorter than 4 m: plain 8-byte entry
+        pay[cell] = make_uint2(frac, vbits);
+        return;
+    }
+    const uint32_t k = cell & 3u;
+    uint4 lo, hi;
+    lo.x = k == 0u ? frac : 0u;
+    lo.y = k == 0u ? vbits : 0u;
+    lo.z = k == 1u ? frac : 0u;
+    lo.w = k == 1u ? vbits : 0u;
+    hi.x = k == 2u ? frac : 0u;
+    hi.y = k == 2u ? vbits : 0u;
+    hi.z = k == 3u ? frac : 0u;
+    hi.w = k == 3u ? vbits : 0u;
+    uint4 *p = reinterpret_cast<uint4 *>(pay + (cell & ~3u));
+    p[0] = lo;
+    p[1] = hi;
+}
+
 // first occupied cell j in [start, end) of a row, for windows of at most 256 cells (H <= 256): the up-to-five words
 // are requested together, then examined.  Requires start < end <= start + 256.
 __device__ __forceinline__ bool first_set_w(const u64 *B, uint32_t row, uint32_t start, uint32_t end, uint32_t &j)
@@ -319,7 +371,7 @@ __device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint3
     }
     Hops h;
     h.s2 = make_uint4(roww[0], roww[1], roww[2], roww[3]);
-    h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), ended ? 0u : 1u, word);
+    h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), (ended ? 0u : 1u) | (l << 1), word);
     return h;
 }
 

@@ -3,22 +3,23 @@
 //   A admit   (R1)      : one thread per origin-edge FIFO; idle queues cost one coalesced load (q_next); a due head
 //                         trip is released if its entry window is free
 //   U update  (R2-R9)   : one thread block per vehicle segment, one thread per active vehicle, state updated in
-//                         place.  First pass, branch-free for nearly every vehicle: the (at most eight) occupancy
-//                         words of the whole look-ahead window -- own row and the rows it continues in on the next
-//                         route edges, whose addresses come from the vehicle's own state -- are requested together,
-//                         searched with selects and one find-first-set, then the leader's payload is fetched; IDM,
-//                         lane-change pre-tests, integration, classification.  Vehicles that must look at the
-//                         adjacent lane (~6 %) or whose window does not fit the fast search (< 1 %) are parked in a
-//                         block-wide shared-memory queue and handled by a dense second pass, so they do not hold
-//                         their warps.  Vehicles that stay on their edge finish the step here: next state, time-(t+1)
-//                         mark and payload, time-(t-1) mark toggled off.  Edge-end candidates post a min-id claim
-//                         and a cross-list entry; arrivals post a cross-list entry and free their slot.
-//   X cross   (R8, R9)  : one thread per cross-list entry: resolves the claim (winner moves to its next route
-//                         edge and rebuilds its look-ahead cache, loser holds at the stop line), writes its mark;
-//                         clears the marks of arrivals.
+//                         place, no block barrier inside.  Branch-free for nearly every vehicle: the (at most
+//                         eight) occupancy words of the whole look-ahead window -- own row and the rows it continues
+//                         in on the next route edges, whose addresses come from the vehicle's own state -- are
+//                         requested together, searched with selects and one find-first-set, then the leader's
+//                         payload is fetched; IDM, lane-change pre-tests, integration, classification.  Vehicles
+//                         that stay on their edge finish the step here: next state, time-(t+1) mark and payload,
+//                         time-(t-1) mark toggled off.  Edge-end candidates post a min-id claim and a cross-list
+//                         entry.  Vehicles that must look at the adjacent lane (~6 %) or whose window does not fit
+//                         the fast search are put on the deferred list: they cannot reach their edge end in this
+//                         step, so they do not hold their warps here.
+//   X second  (R5-R9)   : one thread per list entry, densely packed: cross-list entries resolve their claim (winner
+//                         moves to its next route edge and rebuilds its look-ahead cache, loser holds at the stop
+//                         line) and write their mark; deferred entries run the adjacent-lane search, gap acceptance
+//                         and the rest of the update.
 //
 // A grid-wide barrier separates the phases: the software barrier of k_persistent (one cooperative launch runs
-// many timesteps), or kernel boundaries (k_admit / k_update / k_cross: MANTA_FLAG_MULTI_KERNEL, manta_step_timed).
+// many timesteps), or kernel boundaries (k_admit / k_update / k_second: MANTA_FLAG_MULTI_KERNEL, manta_step_timed).
 #pragma once
 #include "manta_device.cuh"
 
@@ -31,10 +32,17 @@ namespace manta {
 #define MANTA_MINB 2      // blocks per SM the step kernels are compiled for
 #endif
 #define MANTA_NW (MANTA_NT / 32)
-#define MANTA_QCAP (2 * MANTA_NT)   // second-pass queue entries per block (drained whenever MANTA_NT or more wait)
 #define MANTA_NS 8        // occupancy words the fast look-ahead search requests per vehicle
 #define MANTA_MAX_LANES_DEV 8u
 
+// MANTA_DBG builds stamp %globaltimer per block at the phase boundaries of one step in 32 (manta_debug_read): the
+// per-block timeline that the phase structure was tuned with.  Compiled out of the product build.
+#ifdef MANTA_DBG
+__device__ __forceinline__ u64 gtimer() { u64 v; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(v)); return v; }
+#define DBG_STAMP(k) do { if (threadIdx.x == 0u && (t & 31u) == 7u) P.dbg_buf[blockIdx.x * 8u + (k)] = gtimer(); } while (0)
+#else
+#define DBG_STAMP(k) do { } while (0)
+#endif
 struct Lead {
     bool found;
     int32_t lead_abs;   // leader position in the follower's frame, Q22.10 (R2)
@@ -61,14 +69,13 @@ struct Outcome {
     float vn, acc;
 };
 
-// shared memory of the update phase
+// shared memory of the step kernels
 struct UpdateSmem {
-    u64 stats[6];                 // lane_changes, cells_examined, lc_evals, n_updates, n_done, sum_travel (kernel lifetime)
-    uint32_t xn, qn, flag, pad;   // per segment: cross-list entries, queue fill; barrier flag
-    uint32_t wsum[MANTA_NW];      // compaction: live slots per warp
-    uint4 q[MANTA_QCAP];          // second-pass queue: {slot, lead_abs, v_lead bits, 0 not found | 1 found | 2 search still to do}
+    uint32_t ev[4];               // event counters of this kernel: lane changes, lane-change evaluations, arrivals, travel steps
+    uint32_t xn, qn, flag, next;  // per segment: cross-list / deferred-list entries, next unclaimed chunk; barrier flag
+    uint32_t wsum[MANTA_NW];      // re-sort: per-warp partial sums
 };
-enum { ST_LC = 0, ST_CELLS = 1, ST_EVAL = 2, ST_UPD = 3, ST_DONE = 4, ST_TRAVEL = 5 };
+enum { EV_LC = 0, EV_EVAL = 1, EV_DONE = 2, EV_TRAVEL = 3 };
 
 __device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &s1v)
 {
@@ -157,14 +164,19 @@ __device__ __forceinline__ uint32_t ffs64(u64 m)   // index of the lowest set bi
 // the first cells of the rows cached in S2 / S3 -- of n_0 .. n_4 occupancy words; word slot s of the sequence
 // lives at word address s + A_j, j the segment it falls in.  All MANTA_NS word loads are issued before any is
 // examined.  Bits past the end of a segment can only be padding (never set) or lie beyond the H-th examined cell,
-// which the final distance test rejects, so no tail masks are needed.  Returns false if the window does not fit
-// (more than MANTA_NS words, or it runs past the cached hops): the caller then uses walk_rows.
-__device__ __forceinline__ bool leader_cells_fast(const DevP &P, const u64 *B, const Veh &V, const uint4 &s2, const uint4 &s3,
-                                                  Hit &h, uint32_t &examined)
+// which the final distance test rejects, so no tail masks are needed.
+//   own-row part : `own` cells starting at cell `start` of the row whose cell 0 is absolute cell row0 (own = 0: none)
+//   hops         : rows s2, lengths s3.x / s3.y; the first hop row starts dist_hops cells from the tail of the
+//                  vehicle's edge; at most `budget` cells are examined in total
+// Returns WIN_DONE (h valid: leader found, or the window is exhausted / the route ends), WIN_MORE (nothing found
+// and the look-ahead goes on past the four cached hops: budget_left cells remain, starting dist_next cells from
+// the tail) or WIN_NOFIT (more than MANTA_NS words: use walk_rows).
+enum { WIN_DONE = 0, WIN_MORE = 1, WIN_NOFIT = 2 };
+__device__ __forceinline__ int leader_window(const DevP &P, const u64 *B, uint32_t c, uint32_t row0, uint32_t start, uint32_t own,
+                                             uint32_t dist_hops, uint32_t budget, const uint4 &s2, const uint4 &s3, Hit &h,
+                                             uint32_t &budget_left, uint32_t &dist_next)
 {
-    const uint32_t start = V.c + 1u;
-    const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
-    uint32_t rem = P.H - own;
+    uint32_t rem = budget - own;
     const uint32_t len1 = s3.x & 0xFFFFu, len2 = s3.x >> 16, len3 = s3.y & 0xFFFFu, len4 = s3.y >> 16;
     const uint32_t k1 = min(len1, rem);
     rem -= k1;
@@ -178,9 +190,15 @@ __device__ __forceinline__ bool leader_cells_fast(const DevP &P, const u64 *B, c
     const uint32_t n0 = own ? ((start + own - 1u) >> 6) - w0 + 1u : 0u;
     const uint32_t c0 = n0, c1 = c0 + ((k1 + 63u) >> 6), c2 = c1 + ((k2 + 63u) >> 6), c3 = c2 + ((k3 + 63u) >> 6),
                    c4 = c3 + ((k4 + 63u) >> 6);
-    if (c4 > (uint32_t)MANTA_NS || (rem > 0u && s3.z != 0u)) return false;
+    h.found = false;
+    h.cell = 0u;
+    h.dist = 0u;
+    budget_left = rem;
+    const uint32_t d1 = dist_hops, d2 = d1 + len1, d3 = d2 + len2, d4 = d3 + len3;
+    dist_next = d4 + len4;
+    if (c4 > (uint32_t)MANTA_NS) return WIN_NOFIT;
     // word address of slot s = s + A_j; distance (cells from the tail of the own edge) of bit b of slot s = 64 s + b + D_j
-    const uint32_t A0 = (V.row0 >> 6) + w0, A1 = s2.x - c0, A2 = s2.y - c1, A3 = s2.z - c2, A4 = s2.w - c3;
+    const uint32_t A0 = (row0 >> 6) + w0, A1 = s2.x - c0, A2 = s2.y - c1, A3 = s2.z - c2, A4 = s2.w - c3;
     u64 m[MANTA_NS];
 #pragma unroll
     for (uint32_t s = 0; s < (uint32_t)MANTA_NS; s++) {
@@ -196,27 +214,22 @@ __device__ __forceinline__ bool leader_cells_fast(const DevP &P, const u64 *B, c
             sel = m[s];
             si = (uint32_t)s;
         }
-    const uint32_t scanned = P.H - rem;
-    h.found = false;
-    h.cell = 0u;
-    h.dist = 0u;
     if (sel) {
         const uint32_t b = ffs64(sel);
-        const uint32_t d1 = V.len_c, d2 = d1 + len1, d3 = d2 + len2, d4 = d3 + len3;
         uint32_t A = A4, D = d4 - (c3 << 6);
         if (si < c3) { A = A3; D = d3 - (c2 << 6); }
         if (si < c2) { A = A2; D = d2 - (c1 << 6); }
         if (si < c1) { A = A1; D = d1 - (c0 << 6); }
         if (si < c0) { A = A0; D = w0 << 6; }
         const uint32_t dist = (si << 6) + b + D;
-        if (dist - V.c <= P.H) {
+        if (dist - c <= P.H) {
             h.found = true;
             h.dist = dist;
             h.cell = ((A + si) << 6) + b;
+            return WIN_DONE;
         }
     }
-    examined += h.found ? h.dist - V.c : scanned;
-    return true;
+    return (rem > 0u && (s3.z & 1u)) ? WIN_MORE : WIN_DONE;
 }
 
 template <bool W256>
@@ -400,6 +413,7 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
                                           const Outcome &O)
 {
     const int nxt = (int)((t & 1u) ^ 1u);
+    const StBuf &S = P.st[sbuf_of(t)];
     u64 *Bn = P.bits[nxt];
     const uint32_t cur_abs = V.row0 + V.c;
     const uint32_t at = seg_base + slot;
@@ -412,34 +426,32 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
             mark_move(Bn, V.prev, cell);
         else
             mark_toggle(Bn, cell);
-        P.pay[nxt][cell] = make_uint2(O.nx & 1023u, __float_as_uint(O.vn));
-        P.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);
+        pay_store(P, P.pay[nxt], cell, O.nx & 1023u, __float_as_uint(O.vn));
+        S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);
     } else {
         if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
-        const uint32_t xpos = seg_base + atomicAdd(&sm.xn, 1u);
         if (O.kind == KIND_DONE) {
-            P.xlist[xpos] = make_uint4(XL_DONE, cur_abs, 0u, 0u);
             P.arrive_step[V.id] = t + 1u;
-            atomicAdd(&sm.stats[ST_DONE], 1ull);
-            atomicAdd(&sm.stats[ST_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
-            P.S0[at] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);   // dead slot
+            atomicAdd(&sm.ev[EV_DONE], 1u);
+            atomicAdd(&sm.ev[EV_TRAVEL], t + 1u - P.admit_step[V.id]);
+            S.S0[at] = make_uint4(0u, 0u, cur_abs, ID_GHOST);   // the ghost clears the time-t mark in the next step
         } else {
             // smallest id wins; the key carries ~t in the high word so claim words never need a reset
             const uint32_t word = GEOM_PRIO(V.geom) ? V.claim : (V.claim & ~7u) + min(O.l_new, V.claim & 7u);
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)V.id;
             atomicMin(&P.claim[word], key);
-            P.xlist[xpos] = make_uint4(slot, word, V.cursor, V.id);
-            P.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state; the cross phase decides
+            P.xlist[seg_base + atomicAdd(&sm.xn, 1u)] = make_uint4(slot, word, V.cursor, V.id);
+            S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state; the second phase decides
         }
     }
-    if (geom_n != V.geom) P.S1[at] = make_uint4(row_n, geom_n, V.cursor, __float_as_uint(V.v0));
+    if (geom_n != V.geom) S.S1[at] = make_uint4(row_n, geom_n, V.cursor, __float_as_uint(V.v0));
     if (changed) {   // executed lane change: the look-ahead continues in other rows now
-        atomicAdd(&sm.stats[ST_LC], 1ull);
+        atomicAdd(&sm.ev[EV_LC], 1u);
         const Hops hp = build_hops(P, V.cursor, V.geom, O.l_new);
-        P.S2[at] = hp.s2;
-        P.S3[at] = hp.s3;
+        S.S2[at] = hp.s2;
+        S.S3[at] = hp.s3;
     }
-    if (P.acc) P.acc[at] = O.acc;
+    if (S.acc) S.acc[at] = O.acc;
 }
 
 // R5: lead (first occupied cell >= c, within the edge) and lag (last occupied cell < c) in the target lane, then
@@ -474,6 +486,7 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
 __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize)
 {
     const int cur = (int)(t & 1u);
+    const StBuf &S = P.st[sbuf_of(t)];
     u64 *B = P.bits[cur];
     uint2 *pay = P.pay[cur];
     const u64 window = bits_below(P.L_c + 1u);
@@ -495,10 +508,8 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
         const uint4 rr = P.route[cursor];
         const uint32_t geom = (rr.y & GEOM_STATIC_MASK) | (l_sel << 28);
         const Hops hp = build_hops(P, cursor, geom, l_sel);
-        // the emptier of two pseudo-random segments (keeps the segments balanced as trips come and go)
-        uint32_t hsh = mix32(k * 0x9E3779B9u + t);
-        uint32_t sa = hsh % P.n_seg, sb = (sa + 1u + (hsh >> 16) % max(P.n_seg - 1u, 1u)) % P.n_seg;
-        uint32_t seg = P.seg_cnt[sb] < P.seg_cnt[sa] ? sb : sa;
+        // the segment that currently holds the vehicles of this stretch of the atlas (see the re-sort)
+        uint32_t seg = P.bucket_seg[er.x >> MANTA_BUCKET_SHIFT];
         uint32_t slot;
         for (;;) {
             slot = atomicAdd(&P.seg_cnt[seg], 1u);
@@ -508,13 +519,13 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
         }
         const uint32_t row = er.x + l_sel * pitch;
         const size_t at = (size_t)seg * P.seg_cap + slot;
-        P.S0[at] = make_uint4(0u, 0u, CELL_NONE, id);
-        P.S1[at] = make_uint4(row, geom, cursor, rr.w);
-        P.S2[at] = hp.s2;
-        P.S3[at] = hp.s3;
-        if (P.acc) P.acc[at] = 0.0f;
+        S.S0[at] = make_uint4(0u, 0u, CELL_NONE, id);
+        S.S1[at] = make_uint4(row, geom, cursor, rr.w);
+        S.S2[at] = hp.s2;
+        S.S3[at] = hp.s3;
+        if (S.acc) S.acc[at] = 0.0f;
         mark_toggle(B, row);                           // cell 0, frac10 = 0, v = 0: visible to this step's update
-        pay[(size_t)row] = make_uint2(0u, 0u);
+        pay_store(P, pay, row, 0u, 0u);
         P.admit_step[id] = t;
         atomicAdd(&P.edge_entries[rr.z], 1u);
         P.q_head[k] = h + 1u;
@@ -522,212 +533,332 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
     }
 }
 
-// ------------------------------------------------------------------------------------------------ A8
-// Squeezes the dead slots out of one segment, keeping the order of the live ones.  Called by all threads of the
-// block that owns the segment; returns the new slot count.  Chunk by chunk: read, barrier, write -- a slot is
-// never written before the chunk that holds it has been read (write index <= read index).
-__device__ __forceinline__ uint32_t compact_segment(const DevP &P, UpdateSmem &sm, uint32_t seg, uint32_t n)
+// ------------------------------------------------------------------------------------------------ A8: re-sort
+// Spatial re-sort of the vehicle slots (before step t, t a multiple of MANTA_SORT_EVERY): counting sort of all
+// live slots of buffer `from` by atlas bucket into buffer `from ^ 1`, dealt out in equal shares of per_seg slots.
+// Five grid-wide stages: zero the histogram | count (each slot gets its rank inside its bucket) | per-block sums
+// of the histogram | exclusive scan (offsets, and the bucket -> segment map admission uses) | scatter.
+// Results do not depend on slot order (every rule reads time-t state only), so any order inside a bucket will do.
+__device__ __forceinline__ uint32_t sort_key(const uint4 &s0v, uint32_t row0)
 {
-    const size_t seg_base = (size_t)seg * P.seg_cap;
-    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
-    uint32_t out = 0u;
-    for (uint32_t base = 0u; base < n; base += blockDim.x) {
-        const uint32_t i = base + threadIdx.x;
-        uint4 a0 = make_uint4(0u, 0u, 0u, CELL_NONE), a1 = a0, a2 = a0, a3 = a0;
-        float ac = 0.0f;
-        if (i < n) {
-            a0 = P.S0[seg_base + i];
-            if (a0.w != CELL_NONE) {
-                a1 = P.S1[seg_base + i];
-                a2 = P.S2[seg_base + i];
-                a3 = P.S3[seg_base + i];
-                if (P.acc) ac = P.acc[seg_base + i];
-            }
-        }
-        const bool live = a0.w != CELL_NONE;
-        const uint32_t bal = __ballot_sync(0xFFFFFFFFu, live);
-        if (lane_id == 0u) sm.wsum[warp_id] = (uint32_t)__popc(bal);
-        __syncthreads();   // all reads of this chunk done; warp totals visible
-        uint32_t pre = 0u, tot = 0u;
-        for (uint32_t w = 0; w < (blockDim.x >> 5); w++) {
-            const uint32_t c = sm.wsum[w];
-            pre += w < warp_id ? c : 0u;
-            tot += c;
-        }
-        if (live) {
-            const uint32_t pos = out + pre + (uint32_t)__popc(bal & ((1u << lane_id) - 1u));
-            if (pos != i) {
-                P.S0[seg_base + pos] = a0;
-                P.S1[seg_base + pos] = a1;
-                P.S2[seg_base + pos] = a2;
-                P.S3[seg_base + pos] = a3;
-                if (P.acc) P.acc[seg_base + pos] = ac;
-            }
-        }
-        out += tot;
-        __syncthreads();   // wsum may be rewritten; writes of this chunk precede the next chunk's reads
-    }
-    return out;
+    const uint32_t cell = s0v.w == ID_GHOST ? s0v.z : row0 + (s0v.x >> 10);   // a ghost sorts by the mark it has to clear
+    return cell >> MANTA_BUCKET_SHIFT;
 }
+__device__ __forceinline__ void sort_zero(const DevP &P)
+{
+    for (uint32_t b = blockIdx.x * blockDim.x + threadIdx.x; b <= P.n_buckets; b += gridDim.x * blockDim.x) P.sort_hist[b] = 0u;
+}
+__device__ __forceinline__ void sort_count(const DevP &P, int from)
+{
+    const StBuf &S = P.st[from];
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+        const uint32_t n = P.seg_cnt[seg];
+        const size_t seg_base = (size_t)seg * P.seg_cap;
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            const uint4 s0v = S.S0[seg_base + i];
+            uint32_t r = CELL_NONE;
+            if (s0v.w != CELL_NONE) r = atomicAdd(&P.sort_hist[sort_key(s0v, S.S1[seg_base + i].x)], 1u);
+            P.sort_rank[seg_base + i] = r;
+        }
+    }
+}
+// slice of the histogram that block j scans
+__device__ __forceinline__ void sort_slice(const DevP &P, uint32_t j, uint32_t &b0, uint32_t &b1)
+{
+    const uint32_t per = (P.n_buckets + gridDim.x - 1u) / gridDim.x;
+    b0 = min(j * per, P.n_buckets);
+    b1 = min(b0 + per, P.n_buckets);
+}
+__device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t *wsum)   // all threads; result valid in every thread
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);
+    __syncthreads();
+    if ((threadIdx.x & 31u) == 0u) wsum[threadIdx.x >> 5] = v;
+    __syncthreads();
+    uint32_t tot = 0u;
+    for (uint32_t w = 0; w < (blockDim.x >> 5); w++) tot += wsum[w];
+    return tot;
+}
+__device__ __forceinline__ void sort_partial(const DevP &P, UpdateSmem &sm)
+{
+    uint32_t b0, b1;
+    sort_slice(P, blockIdx.x, b0, b1);
+    uint32_t v = 0u;
+    for (uint32_t b = b0 + threadIdx.x; b < b1; b += blockDim.x) v += P.sort_hist[b];
+    const uint32_t tot = block_sum(v, sm.wsum);
+    if (threadIdx.x == 0u) P.sort_part[blockIdx.x] = tot;
+}
+__device__ __forceinline__ void sort_scan(const DevP &P, UpdateSmem &sm, uint32_t &n_live, uint32_t &per_seg)
+{
+    // offset of this block's slice and the live total, from the per-block sums
+    uint32_t before = 0u, all = 0u;
+    for (uint32_t k = threadIdx.x; k < gridDim.x; k += blockDim.x) {
+        const uint32_t c = P.sort_part[k];
+        all += c;
+        before += k < blockIdx.x ? c : 0u;
+    }
+    all = block_sum(all, sm.wsum);
+    before = block_sum(before, sm.wsum);
+    n_live = all;
+    per_seg = max(1u, (all + P.n_seg - 1u) / P.n_seg);
+    uint32_t b0, b1;
+    sort_slice(P, blockIdx.x, b0, b1);
+    const uint32_t lane_id = threadIdx.x & 31u, warp_id = threadIdx.x >> 5;
+    uint32_t run = before;
+    for (uint32_t base = b0; base < b1; base += blockDim.x) {
+        const uint32_t b = base + threadIdx.x;
+        const uint32_t c = b < b1 ? P.sort_hist[b] : 0u;
+        uint32_t inc = c;   // inclusive scan inside the warp
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+            if (lane_id >= (uint32_t)d) inc += o;
+        }
+        __syncthreads();
+        if (lane_id == 31u) sm.wsum[warp_id] = inc;
+        __syncthreads();
+        uint32_t wpre = 0u, tot = 0u;
+        for (uint32_t w = 0; w < (blockDim.x >> 5); w++) {
+            const uint32_t x = sm.wsum[w];
+            wpre += w < warp_id ? x : 0u;
+            tot += x;
+        }
+        if (b < b1) {
+            const uint32_t off = run + wpre + inc - c;
+            P.sort_hist[b] = off;
+            P.bucket_seg[b] = (off >> 5) % P.n_seg;   // segment of the chunk the bucket's first vehicle goes to
+        }
+        run += tot;
+    }
+}
+__device__ __forceinline__ void sort_scatter(const DevP &P, int from, uint32_t n_live, uint32_t per_seg)
+{
+    const StBuf &S = P.st[from];
+    const StBuf &D = P.st[from ^ 1];
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+        const uint32_t n = P.seg_cnt[seg];
+        const size_t seg_base = (size_t)seg * P.seg_cap;
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            const uint32_t r = P.sort_rank[seg_base + i];
+            if (r == CELL_NONE) continue;
+            const uint4 a0 = S.S0[seg_base + i], a1 = S.S1[seg_base + i], a2 = S.S2[seg_base + i], a3 = S.S3[seg_base + i];
+            const uint32_t g = P.sort_hist[sort_key(a0, a1.x)] + r;
+            // chunks of 32 consecutive vehicles are dealt round-robin: chunk j goes to segment j % n_seg
+            const uint32_t chunk = g >> 5, sd = chunk % P.n_seg;
+            const size_t at = (size_t)sd * P.seg_cap + ((chunk / P.n_seg) << 5) + (g & 31u);
+            D.S0[at] = a0;
+            D.S1[at] = a1;
+            D.S2[at] = a2;
+            D.S3[at] = a3;
+            if (S.acc) D.acc[at] = S.acc[seg_base + i];
+        }
+    }
+    __syncthreads();   // this block has read the old counts of all its segments
+    const uint32_t n_chunks = (n_live + 31u) >> 5;
+    for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x)
+        if (threadIdx.x == 0u) {
+            uint32_t cnt = 0u;
+            if (seg < n_chunks) {
+                const uint32_t mine = (n_chunks - 1u - seg) / P.n_seg + 1u;          // chunks seg, seg + n_seg, ...
+                const bool has_last = (n_chunks - 1u) % P.n_seg == seg;              // only the last chunk can be partial
+                cnt = has_last ? ((mine - 1u) << 5) + (n_live - ((n_chunks - 1u) << 5)) : mine << 5;
+            }
+            P.seg_cnt[seg] = cnt;
+        }
+}
+__device__ __forceinline__ bool sort_due(uint32_t t) { return t != 0u && t % MANTA_SORT_EVERY == 0u; }
 
 // ------------------------------------------------------------------------------------------------ U: R2-R9
-// Second pass: `take` queue entries starting at q0, one per thread, densely packed over the block.
+// A vehicle further than Z_out cells from its edge end cannot reach it in this step (R0: Z_out > vcap dt), so it
+// can be neither an edge-end candidate nor an arrival, whatever its leader.  (R4 allows lane changes only there.)
+__device__ __forceinline__ bool cannot_cross(const DevP &P, const Veh &V) { return V.c + P.Z_out < V.len_c; }
+
+// Look-ahead past the four cached hops (rare: a run of short edges): the cache the vehicle would have four route
+// edges further on is rebuilt from the route store and searched the same way, until the budget of H cells is used
+// up, the route ends or a leader is found.
+__device__ __forceinline__ Hit leader_continue(const DevP &P, const u64 *B, const Veh &V, uint32_t s3z, uint32_t budget_left,
+                                              uint32_t dist_next, uint32_t &n_cells)
+{
+    Hit h;
+    uint32_t cursor = V.cursor, lane = (s3z >> 1) & 7u;
+    for (int rounds = 0; rounds < 16; rounds++) {
+        cursor += 4u;
+        const Hops hp = build_hops(P, cursor, 0u, lane);
+        const int r = leader_window(P, B, V.c, 0u, 0u, 0u, dist_next, budget_left, hp.s2, hp.s3, h, budget_left, dist_next);
+        if (r == WIN_DONE) {
+            n_cells += h.found ? h.dist - V.c : P.H - budget_left;
+            return h;
+        }
+        if (r == WIN_NOFIT) break;
+        lane = (hp.s3.z >> 1) & 7u;
+    }
+    return walk_rows(P, B, V, n_cells);
+}
+
+// Deferred-list entry kinds: 0 / 1 = adjacent-lane evaluation (own-lane leader not found / found, carried in the
+// entry); 2 = look-ahead to be continued past the cached hops (budget_left, dist_next carried); 3 = walk_rows.
 template <bool W256>
-__device__ __forceinline__ void drain_queue(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, uint32_t q0, uint32_t take,
-                                            uint32_t &n_cells)
+__device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, const uint4 &e,
+                                                uint32_t &n_cells)
 {
     const int cur = (int)(t & 1u);
+    const StBuf &S = P.st[sbuf_of(t)];
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
-    if (threadIdx.x >= take) return;
-    const uint4 e = sm.q[q0 + threadIdx.x];
+    const uint32_t slot = e.x & 0x3FFFFFFFu, kind = e.x >> 30;
     Veh V;
-    veh_load(V, P.S0[seg_base + e.x], P.S1[seg_base + e.x]);
-    V.claim = P.S3[seg_base + e.x].w;
+    veh_load(V, S.S0[seg_base + slot], S.S1[seg_base + slot]);
+    V.claim = 0u;
     Lead ld;
-    if (e.w == 2u) {   // the window did not fit the fast search
-        Hit h = walk_rows(P, B, V, n_cells);
+    if (kind >= 2u) {
+        const Hit h = kind == 2u ? leader_continue(P, B, V, e.w, e.y, e.z, n_cells) : walk_rows(P, B, V, n_cells);
         ld = lead_from_hit<W256>(pay, h);
     } else {
-        ld.found = e.w != 0u;
+        ld.found = kind != 0u;
         ld.lead_abs = (int32_t)e.y;
         ld.v_lead = __uint_as_float(e.z);
     }
     pre_lc(P, t, V, ld);
     Outcome O;
     if (V.need_lc) {
-        atomicAdd(&sm.stats[ST_EVAL], 1ull);
+        atomicAdd(&sm.ev[EV_EVAL], 1u);
         O = lane_change_and_finish<W256>(P, t, B, pay, V);
     } else {
         O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
     }
-    write_out(P, t, sm, seg_base, e.x, V, O);
+    write_out(P, t, sm, seg_base, slot, V, O);
 }
 
-// Must be called by ALL threads of the block (contains __syncthreads).
+// Must be called by ALL threads of the block (contains __syncthreads).  Warps take chunks of 32 slots from a
+// shared counter, so a warp that met slow vehicles simply takes fewer chunks.
 template <bool W256>
 __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd)
 {
-    const int cur = (int)(t & 1u);
+    const int cur = (int)(t & 1u), nxt = cur ^ 1;
+    const StBuf &S = P.st[sbuf_of(t)];
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
+    const uint32_t lane_id = threadIdx.x & 31u;
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
-        uint32_t n = P.seg_cnt[seg];
+        const uint32_t n = P.seg_cnt[seg];
         const uint32_t seg_base = seg * P.seg_cap;
         if (threadIdx.x == 0u) {
             sm.xn = 0u;
             sm.qn = 0u;
+            sm.next = blockDim.x;
         }
+        DBG_STAMP(1);
         __syncthreads();
-        if (t % MANTA_COMPACT_EVERY == 0u && n > 0u) {
-            n = compact_segment(P, sm, seg, n);
-            if (threadIdx.x == 0u) P.seg_cnt[seg] = n;
-        }
-        for (uint32_t base = 0u; base < n; base += blockDim.x) {
-            // ---- first pass: everything but the adjacent-lane look-up
-            const uint32_t i = base + threadIdx.x;
-            uint4 s0v = make_uint4(0u, 0u, 0u, CELL_NONE);
-            if (i < n) s0v = P.S0[seg_base + i];
-            if (s0v.w != CELL_NONE) {   // live slot
-                const uint4 s1v = P.S1[seg_base + i];
-                const uint4 s2v = P.S2[seg_base + i];
-                const uint4 s3v = P.S3[seg_base + i];
+        for (uint32_t base = threadIdx.x & ~31u; base < n;) {
+            const uint32_t i = base + lane_id;
+            uint4 s0v = make_uint4(0u, 0u, 0u, CELL_NONE), s1v = s0v, s2v = s0v, s3v = s0v;
+            if (i < n) {
+                s0v = S.S0[seg_base + i];
+                s1v = S.S1[seg_base + i];
+                s2v = S.S2[seg_base + i];
+                s3v = S.S3[seg_base + i];
+            }
+            // the next chunk of this warp (requested now, needed after this one)
+            uint32_t next_base = 0u;
+            if (lane_id == 0u) next_base = atomicAdd(&sm.next, 32u);
+            if (s0v.w == ID_GHOST) {   // the ghost of last step's arrival clears that vehicle's last mark
+                mark_toggle(P.bits[nxt], s0v.z);
+                S.S0[seg_base + i] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);
+            } else if (s0v.w != CELL_NONE) {
                 Veh V;
                 veh_load(V, s0v, s1v);
                 V.claim = s3v.w;
                 n_upd += 1u;
                 Hit h;
-                bool fits;
+                h.found = false;
+                h.cell = 0u;
+                h.dist = 0u;
+                uint32_t budget_left = 0u, dist_next = 0u;
+                int r = WIN_DONE;
                 if (W256) {
-                    fits = leader_cells_fast(P, B, V, s2v, s3v, h, n_cells);
+                    const uint32_t start = V.c + 1u;
+                    const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
+                    r = leader_window(P, B, V.c, V.row0, start, own, V.len_c, P.H, s2v, s3v, h, budget_left, dist_next);
+                    if (r == WIN_DONE) {
+                        n_cells += h.found ? h.dist - V.c : P.H - budget_left;
+                    } else if (!cannot_cross(P, V)) {   // rare: near the edge end and the window does not fit
+                        h = r == WIN_MORE ? leader_continue(P, B, V, s3v.z, budget_left, dist_next, n_cells) : walk_rows(P, B, V, n_cells);
+                        r = WIN_DONE;
+                    }
                 } else {
                     h = walk_rows(P, B, V, n_cells);
-                    fits = true;
                 }
-                uint32_t qkind = 0xFFFFFFFFu;
-                Lead ld;
-                ld.found = false;
-                ld.lead_abs = 0;
-                ld.v_lead = 0.0f;
-                if (fits) {
-                    ld = lead_from_hit<W256>(pay, h);
+                if (r == WIN_DONE) {
+                    const Lead ld = lead_from_hit<W256>(pay, h);
                     pre_lc(P, t, V, ld);
-                    if (V.need_lc) qkind = ld.found ? 1u : 0u;
-                } else {
-                    qkind = 2u;
-                }
-                if (qkind != 0xFFFFFFFFu) {   // parked: the second pass finishes this vehicle
-                    const uint32_t qp = atomicAdd(&sm.qn, 1u);
-                    sm.q[qp] = make_uint4(i, (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), qkind);
-                } else {
-                    const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
-                    write_out(P, t, sm, seg_base, i, V, O);
+                    if (V.need_lc) {   // deferred: must look at the adjacent lane (R5)
+                        P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] =
+                            make_uint4(i | (ld.found ? 1u << 30 : 0u), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
+                    } else {
+                        const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+                        write_out(P, t, sm, seg_base, i, V, O);
+                    }
+                } else {   // deferred: look-ahead to be continued (2) or walked (3)
+                    P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] = make_uint4(i | ((r == WIN_MORE ? 2u : 3u) << 30), budget_left, dist_next, s3v.z);
                 }
             }
-            __syncthreads();
-            const uint32_t qn = sm.qn;
-            if (qn >= blockDim.x) {   // block-uniform
-                drain_queue<W256>(P, t, sm, seg_base, qn - blockDim.x, blockDim.x, n_cells);
-                __syncthreads();
-                if (threadIdx.x == 0u) sm.qn = qn - blockDim.x;
-                __syncthreads();
-            }
+            base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
         }
-        {
-            const uint32_t qn = sm.qn;   // < blockDim.x; visible to all since the last barrier
-            drain_queue<W256>(P, t, sm, seg_base, 0u, qn, n_cells);
-        }
+        __syncthreads();   // the deferred list of this segment is complete (and visible: same block)
+        DBG_STAMP(2);
+        const uint32_t qn = sm.qn;
+        for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) finish_deferred<W256>(P, t, sm, seg_base, P.dlist[seg_base + k], n_cells);
         __syncthreads();
+        DBG_STAMP(3);
         if (threadIdx.x == 0u) P.seg_xn[seg] = sm.xn;
     }
 }
 
-// ------------------------------------------------------------------------------------------------ X: R8, R9
-__device__ __forceinline__ void cross_phase(const DevP &P, uint32_t t)
+// ------------------------------------------------------------------------------------------------ X: R8
+// One thread per cross-list entry: resolve the claim; the winner moves to its next route edge and rebuilds its
+// look-ahead cache, the loser holds at the stop line; both write their time-(t+1) mark and payload.
+__device__ __forceinline__ void second_phase(const DevP &P, uint32_t t)
 {
-    const int cur = (int)(t & 1u), nxt = cur ^ 1;
-    u64 *Bc = P.bits[cur];
+    const int nxt = (int)((t & 1u) ^ 1u);
+    const StBuf &S = P.st[sbuf_of(t)];
     u64 *Bn = P.bits[nxt];
     uint2 *payn = P.pay[nxt];
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
-        const uint32_t n = P.seg_xn[seg];
-        const size_t seg_base = (size_t)seg * P.seg_cap;
-        for (uint32_t k = threadIdx.x; k < n; k += blockDim.x) {
-            const uint4 xl = P.xlist[seg_base + k];     // {slot | XL_DONE, claim word | cell, cursor, id}
-            if (xl.x == XL_DONE) {
-                mark_toggle(Bc, xl.y);    // an arrival leaves no time-(t+1) state to clear its time-t mark later
-                continue;
-            }
-            const size_t at = seg_base + xl.x;
-            uint4 s0 = P.S0[at];
-            const uint4 s1 = P.S1[at];
+        const uint32_t xn = P.seg_xn[seg];
+        const uint32_t seg_base = seg * P.seg_cap;
+        for (uint32_t k = threadIdx.x; k < xn; k += blockDim.x) {
+            const uint4 xl = P.xlist[seg_base + k];     // {slot, claim word, cursor, id}
+            const size_t at = (size_t)seg_base + xl.x;
+            uint4 s0 = S.S0[at];
+            const uint4 s1 = S.S1[at];
             const u64 won = P.claim[xl.y];
             const uint4 rn = P.route[xl.z + 1u];
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)xl.w;
             uint32_t cell;
-            if (won == key) {             // winner crosses (R8)
+            if (won == key) {             // winner crosses
                 const uint32_t lplus = min(GEOM_LANE(s1.y), GEOM_LANES(rn.y) - 1u);
                 const uint32_t geom = (rn.y & GEOM_STATIC_MASK) | (lplus << 28);
                 const uint32_t row = rn.x + lplus * pitch_of(GEOM_LEN(rn.y));
                 const Hops hp = build_hops(P, xl.z + 1u, geom, lplus);
-                P.S1[at] = make_uint4(row, geom, xl.z + 1u, rn.w);
-                P.S2[at] = hp.s2;
-                P.S3[at] = hp.s3;
+                S.S1[at] = make_uint4(row, geom, xl.z + 1u, rn.w);
+                S.S2[at] = hp.s2;
+                S.S3[at] = hp.s3;
                 atomicAdd(&P.edge_entries[rn.z], 1u);
                 cell = row + (s0.x >> 10);
             } else {                      // loser holds at the stop line (G15)
                 s0.x = (GEOM_LEN(s1.y) << 10) - 1u;
                 s0.y = 0u;
-                P.S0[at] = s0;
+                S.S0[at] = s0;
                 cell = s1.x + (s0.x >> 10);
             }
             mark_toggle(Bn, cell);
-            payn[cell] = make_uint2(s0.x & 1023u, s0.y);
+            pay_store(P, payn, cell, s0.x & 1023u, s0.y);
         }
     }
 }
 
-// per-thread counters -> shared -> this block's record (once per kernel)
+// per-thread and per-block counters of this kernel -> this block's record
 __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint32_t n_cells32, uint32_t n_upd32)
 {
     u64 n_cells = n_cells32, n_upd = n_upd32;
@@ -736,19 +867,17 @@ __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint3
         n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
         n_upd += __shfl_down_sync(0xFFFFFFFFu, n_upd, d);
     }
+    BlockStats *b = &P.blk[blockIdx.x];
     if ((threadIdx.x & 31u) == 0u) {
-        if (n_cells) atomicAdd(&sm.stats[ST_CELLS], n_cells);
-        if (n_upd) atomicAdd(&sm.stats[ST_UPD], n_upd);
+        if (n_cells) atomicAdd(&b->cells_examined, n_cells);
+        if (n_upd) atomicAdd(&b->n_updates, n_upd);
     }
     __syncthreads();
     if (threadIdx.x == 0u) {
-        BlockStats *b = &P.blk[blockIdx.x];
-        b->lane_changes += sm.stats[ST_LC];
-        b->cells_examined += sm.stats[ST_CELLS];
-        b->lc_evals += sm.stats[ST_EVAL];
-        b->n_updates += sm.stats[ST_UPD];
-        b->n_done += sm.stats[ST_DONE];
-        b->sum_travel += sm.stats[ST_TRAVEL];
+        if (sm.ev[EV_LC]) atomicAdd(&b->lane_changes, (u64)sm.ev[EV_LC]);
+        if (sm.ev[EV_EVAL]) atomicAdd(&b->lc_evals, (u64)sm.ev[EV_EVAL]);
+        if (sm.ev[EV_DONE]) atomicAdd(&b->n_done, (u64)sm.ev[EV_DONE]);
+        if (sm.ev[EV_TRAVEL]) atomicAdd(&b->sum_travel, (u64)sm.ev[EV_TRAVEL]);
     }
 }
 
@@ -762,14 +891,37 @@ template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, uint32_t t)
 {
     __shared__ UpdateSmem sm;
-    if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
+    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
     __syncthreads();
     uint32_t n_cells = 0u, n_upd = 0u;
     update_phase<W256>(P, t, sm, n_cells, n_upd);
     flush_stats(P, sm, n_cells, n_upd);
 }
 
-__global__ void __launch_bounds__(256) k_cross(const DevP P, uint32_t t) { cross_phase(P, t); }
+__global__ void __launch_bounds__(256) k_second(const DevP P, uint32_t t) { second_phase(P, t); }
+
+// the five stages of the re-sort as kernels (multi-kernel mode); n_live / per_seg travel through sort_part[n_seg..]
+__global__ void __launch_bounds__(MANTA_NT) k_sort_zero(const DevP P) { sort_zero(P); }
+__global__ void __launch_bounds__(MANTA_NT) k_sort_count(const DevP P, int from) { sort_count(P, from); }
+__global__ void __launch_bounds__(MANTA_NT) k_sort_partial(const DevP P)
+{
+    __shared__ UpdateSmem sm;
+    sort_partial(P, sm);
+}
+__global__ void __launch_bounds__(MANTA_NT) k_sort_scan(const DevP P)
+{
+    __shared__ UpdateSmem sm;
+    uint32_t n_live, per_seg;
+    sort_scan(P, sm, n_live, per_seg);
+}
+__global__ void __launch_bounds__(MANTA_NT) k_sort_scatter(const DevP P, int from)
+{
+    __shared__ UpdateSmem sm;
+    uint32_t all = 0u;   // recompute the live total from the per-block sums
+    for (uint32_t k = threadIdx.x; k < gridDim.x; k += blockDim.x) all += P.sort_part[k];
+    all = block_sum(all, sm.wsum);
+    sort_scatter(P, from, all, max(1u, (all + P.n_seg - 1u) / P.n_seg));
+}
 
 // Grid-wide barrier of the persistent kernel: arrival counter + generation word, release / acquire at gpu scope
 // (the fences also invalidate L1, so plain loads after the barrier see the other SMs' writes).  A spin that lasts
@@ -785,22 +937,30 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     __syncthreads();
     if (threadIdx.x == 0u) {
         gen += 1u;
+        unsigned ab = 0u;
         __threadfence();
         const unsigned prev = atomicAdd(&c->bar_count, 1u);
         if (prev + 1u == gen * gridDim.x) {
             asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&c->bar_gen), "r"(gen) : "memory");
         } else {
             const long long t0 = clock64();
+            unsigned spins = 0u;
             while (ld_acquire_u32(&c->bar_gen) < gen) {
-                if (ld_acquire_u32(&c->abort)) break;
-                if (clock64() - t0 > 8000000000ll) {
-                    atomicExch(&c->abort, 1u);
-                    break;
+                if ((++spins & 1023u) == 0u) {   // now and then: has another block given up, or is this taking seconds?
+                    if (ld_acquire_u32(&c->abort)) {
+                        ab = 1u;
+                        break;
+                    }
+                    if (clock64() - t0 > 8000000000ll) {
+                        atomicExch(&c->abort, 1u);
+                        ab = 1u;
+                        break;
+                    }
                 }
             }
         }
         __threadfence();
-        *s_flag = ld_acquire_u32(&c->abort);
+        *s_flag = ab;
     }
     __syncthreads();
     return *s_flag == 0u;
@@ -811,17 +971,35 @@ template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps)
 {
     __shared__ UpdateSmem sm;
-    if (threadIdx.x < 6u) sm.stats[threadIdx.x] = 0ull;
+    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
     unsigned gen = 0u;
     uint32_t n_cells = 0u, n_upd = 0u;
     const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
     for (uint32_t t = t0; t < t0 + n_steps; t++) {
+        if (sort_due(t)) {
+            const int from = sbuf_of(t - 1u);
+            uint32_t n_live, per_seg;
+            sort_zero(P);
+            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+            sort_count(P, from);
+            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+            sort_partial(P, sm);
+            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+            sort_scan(P, sm, n_live, per_seg);
+            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+            sort_scatter(P, from, n_live, per_seg);
+            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+        }
+        DBG_STAMP(0);
         admit_phase(P, t, gtid, gsize);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         update_phase<W256>(P, t, sm, n_cells, n_upd);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-        cross_phase(P, t);
+        DBG_STAMP(4);
+        second_phase(P, t);
+        DBG_STAMP(5);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+        DBG_STAMP(6);
     }
     flush_stats(P, sm, n_cells, n_upd);
 }
@@ -864,34 +1042,36 @@ __global__ void k_mark_last(const uint64_t *route_ptr, uint32_t n_trips, uint4 *
 // route store, mark atlas_0, count the entry.  init = {x_fx, v bits, vehicle id, route cursor}.
 __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init)
 {
+    const StBuf &S = P.st[0];
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_init; i += gridDim.x * blockDim.x) {
         const uint4 iv = init[i];
         const uint4 rr = P.route[iv.w];
         const size_t at = (size_t)(i % P.n_seg) * P.seg_cap + i / P.n_seg;
         const uint32_t geom = rr.y & GEOM_STATIC_MASK;      // lane 0, tag 0
         const Hops hp = build_hops(P, iv.w, geom, 0u);
-        P.S0[at] = make_uint4(iv.x, iv.y, CELL_NONE, iv.z);   // no earlier mark
-        P.S1[at] = make_uint4(rr.x, geom, iv.w, rr.w);
-        P.S2[at] = hp.s2;
-        P.S3[at] = hp.s3;
+        S.S0[at] = make_uint4(iv.x, iv.y, CELL_NONE, iv.z);   // no earlier mark
+        S.S1[at] = make_uint4(rr.x, geom, iv.w, rr.w);
+        S.S2[at] = hp.s2;
+        S.S3[at] = hp.s3;
         const uint32_t cell = rr.x + (iv.x >> 10);
         mark_toggle(P.bits[0], cell);
-        P.pay[0][cell] = make_uint2(iv.x & 1023u, iv.y);
+        pay_store(P, P.pay[0], cell, iv.x & 1023u, iv.y);
         P.admit_step[iv.z] = 0u;
         atomicAdd(&P.edge_entries[rr.z], 1u);
     }
 }
 // Readback: scatter the live slots of the segments into per-trip arrays (caller order).
-__global__ void k_gather_state(const DevP P, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
+__global__ void k_gather_state(const DevP P, int sb, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
                                uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc)
 {
+    const StBuf &S = P.st[sb];
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
         const uint32_t n = P.seg_cnt[seg];
         const size_t seg_base = (size_t)seg * P.seg_cap;
         for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
-            const uint4 s0v = P.S0[seg_base + i];
-            if (s0v.w == CELL_NONE) continue;
-            const uint4 s1v = P.S1[seg_base + i];
+            const uint4 s0v = S.S0[seg_base + i];
+            if (s0v.w >= ID_GHOST) continue;
+            const uint4 s1v = S.S1[seg_base + i];
             const uint32_t tr = trip_of_id[s0v.w];
             status[tr] = 1u;
             route_pos[tr] = s1v.z - P.route_start[s0v.w];
@@ -899,7 +1079,7 @@ __global__ void k_gather_state(const DevP P, const uint32_t *trip_of_id, uint8_t
             tag[tr] = (uint8_t)GEOM_TAG(s1v.y);
             x_fx[tr] = s0v.x;
             v[tr] = __uint_as_float(s0v.y);
-            acc[tr] = P.acc ? P.acc[seg_base + i] : 0.0f;
+            acc[tr] = S.acc ? S.acc[seg_base + i] : 0.0f;
         }
     }
 }

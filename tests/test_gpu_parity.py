@@ -178,3 +178,81 @@ def test_error_codes(binding):
     with pytest.raises(binding.MantaError) as e:
         binding.Sim(net, dict(dt=0.0))
     assert e.value.code == binding.ERR_INVALID_ARG
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Paths of the look-ahead that the configs above rarely take: windows that run past the four route edges cached
+# in the vehicle state (a run of short edges), windows of more than eight occupancy words, H > 256 (generic
+# row walk), vehicles shorter than 4 m (8-byte payload entries), and the periodic spatial re-sort of the slots.
+def short_edge_ring(pattern, lanes, n_veh, n_steps, seed, limit=50 / 3.6):
+    """One-way ring whose edge lengths repeat `pattern` (metres); n_veh vehicles entering over the first steps,
+    each cycling the ring."""
+    lens = np.asarray(pattern, np.float32)
+    n_e = len(lens)
+    tail = np.arange(n_e, dtype=np.int64)
+    net = wl._csr_from_edges(n_e, tail, (tail + 1) % n_e, length_m=lens,
+                             lanes=np.asarray(lanes, np.uint8) if np.ndim(lanes) else np.full(n_e, lanes, np.uint8),
+                             speed_limit=np.full(n_e, limit, np.float32))
+    net["node_ctrl"] = np.zeros(n_e, np.uint8)
+    rng = np.random.default_rng(seed)
+    n_route = int(np.ceil(limit * 0.5 * n_steps / float(lens.min()))) + 4
+    e0 = rng.integers(0, n_e, n_veh)
+    routes = (e0[:, None] + np.arange(n_route)[None, :]) % n_e
+    trips = dict(route_ptr=np.arange(n_veh + 1, dtype=np.uint64) * np.uint64(n_route),
+                 route_edges=routes.astype(np.uint32).ravel(),
+                 depart_time_s=rng.uniform(0.0, 60.0, n_veh).astype(np.float32), init_pos_m=None, init_speed=None)
+    return net, trips
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_look_ahead_past_cached_hops(oracle_mod, binding, flags):
+    """Edges of 12-30 m: a 256-cell window spans 9-20 edges, so nearly every search continues past the cached
+    hops, inline near an edge end and deferred elsewhere; two lanes on some edges give lane changes as well."""
+    rng = np.random.default_rng(11)
+    pattern = rng.integers(12, 31, 60).astype(np.float32)
+    lanes = np.where(rng.random(60) < 0.4, 2, 1)
+    net, trips = short_edge_ring(pattern, lanes, n_veh=7, n_steps=1200, seed=12)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=256), 1200, dense_until=200, every=7,
+                    atlas_every=300, flags=flags)
+    assert s["cells_examined"] > 100 * s["vehicle_updates"]     # i.e. the average window spans five or more edges
+
+
+def test_window_of_more_than_eight_words(oracle_mod, binding):
+    """A 250 m edge followed by 10-12 m edges: from the long edge the window needs up to five own-row words plus
+    one word per short edge -- more than the eight the fast search requests (walk_rows fallback)."""
+    pattern = [250.0] + [11.0, 12.0, 10.0, 12.0, 11.0, 10.0, 12.0] * 3
+    net, trips = short_edge_ring(pattern, 1, n_veh=5, n_steps=900, seed=13)
+    run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=256), 900, dense_until=150, every=5, atlas_every=300)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_long_look_ahead_generic_walk(oracle_mod, binding, flags):
+    """H = 400 > 256: every vehicle takes the generic row walk and the word-by-word scans."""
+    net = wl.grid_network(nx=4, ny=4, lanes=2, ctrl=wl.GREEN)
+    o_, d_ = wl.uniform_od(net, 500, 21)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(500, 0.0, 200.0, 22), n_threads=2)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=400, lookback_cells=150), 900,
+                    dense_until=100, every=9, atlas_every=300, flags=flags)
+    assert s["n_done"] > 100
+
+
+def test_short_vehicles_plain_payload(oracle_mod, binding):
+    """veh_len = 3 m: two vehicles can share an aligned group of four cells, so payload entries are written one by
+    one instead of as whole sectors."""
+    net = wl.grid_network(nx=4, ny=4, lanes=2, ctrl=wl.PRIORITY)
+    o_, d_ = wl.uniform_od(net, 600, 31)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(600, 0.0, 120.0, 32), n_threads=2)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128, veh_len=3.0, s0=1.0), 800,
+                    dense_until=200, every=11, atlas_every=200)
+    assert s["n_done"] > 100
+
+
+def test_full_size_network_peak_window(oracle_mod, binding):
+    """BASELINE.json configs[2] at FULL network size (223,721 nodes, 556,356 directed edges, 1.76e8 atlas cells), in
+    the launch configuration bench.py times (persistent cooperative kernel, 296 segments), with the trips of four
+    minutes of the 07:30 peak: every vehicle's state, per-edge counts and counters bit-exact against the oracle
+    over 700 steps (several spatial re-sorts included)."""
+    net, trips, params, _ = wl.config2(scale=1.0, window=(2.5 * 3600.0, 2.5 * 3600.0 + 240.0), n_threads=8)
+    assert net["n_edges"] > 500000 and len(trips["depart_time_s"]) > 20000
+    s, n_launch = run_both(oracle_mod, binding, net, trips, params, 700, dense_until=0, every=100, flags=0)
+    assert n_launch == 7 and s["vehicle_updates"] > 5_000_000
