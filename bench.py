@@ -123,7 +123,7 @@ def algorithmic_bytes(hbar, flc, lookback):
     payload 8, new mark (8-byte word) 8 + own payload 8, toggling the old mark off 8; a deferred adjacent-lane
     evaluation adds its list entry (16 written + 16 read), the target row's bits ahead and behind and two payloads.
     The whole step adds the cross-list entry and claim of the ~2 % of vehicles at an edge end and the amortised
-    re-sort (128 B per vehicle every MANTA_SORT_EVERY = 32 steps), folded in as 6 B."""
+    re-sort (128 B per vehicle every MANTA_SORT_EVERY = 64 steps), folded in as 6 B."""
     upd = 64.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0 + flc * (32.0 + (hbar + lookback) / 8.0 + 16.0)
     return upd, upd + 6.0
 

@@ -73,7 +73,7 @@ typedef unsigned long long u64;
 #define CELL_NONE 0xFFFFFFFFu
 #define ID_GHOST 0xFFFFFFFEu   // slot of a vehicle that arrived in the previous step: clears its last mark, then dies
 #ifndef MANTA_SORT_EVERY
-#define MANTA_SORT_EVERY 32u      // timesteps between two spatial re-sorts of the vehicle slots
+#define MANTA_SORT_EVERY 64u      // timesteps between two spatial re-sorts of the vehicle slots
 #endif
 #ifndef MANTA_BUCKET_SHIFT
 #define MANTA_BUCKET_SHIFT 8      // sort key = absolute atlas cell >> this

@@ -765,17 +765,22 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             if (s0v.w == ID_GHOST) {   // the ghost of last step's arrival clears that vehicle's last mark
                 mark_toggle(P.bits[nxt], s0v.z);
                 S.S0[seg_base + i] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);
-            } else if (s0v.w != CELL_NONE) {
-                Veh V;
-                veh_load(V, s0v, s1v);
-                V.claim = s3v.w;
+            }
+            // The stages below are separated by __syncwarp() so that the warp runs each of them once, with all its
+            // live lanes, whatever rare side paths single lanes took in the stage before.
+            const bool live = s0v.w < ID_GHOST;
+            Veh V;
+            veh_load(V, s0v, s1v);
+            V.claim = s3v.w;
+            Hit h;
+            h.found = false;
+            h.cell = 0u;
+            h.dist = 0u;
+            uint32_t budget_left = 0u, dist_next = 0u;
+            int r = WIN_DONE;
+            // ---- stage 1: look-ahead (R2)
+            if (live) {
                 n_upd += 1u;
-                Hit h;
-                h.found = false;
-                h.cell = 0u;
-                h.dist = 0u;
-                uint32_t budget_left = 0u, dist_next = 0u;
-                int r = WIN_DONE;
                 if (W256) {
                     const uint32_t start = V.c + 1u;
                     const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
@@ -789,20 +794,32 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
                 } else {
                     h = walk_rows(P, B, V, n_cells);
                 }
-                if (r == WIN_DONE) {
-                    const Lead ld = lead_from_hit<W256>(pay, h);
-                    pre_lc(P, t, V, ld);
-                    if (V.need_lc) {   // deferred: must look at the adjacent lane (R5)
-                        P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] =
-                            make_uint4(i | (ld.found ? 1u << 30 : 0u), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
-                    } else {
-                        const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
-                        write_out(P, t, sm, seg_base, i, V, O);
-                    }
-                } else {   // deferred: look-ahead to be continued (2) or walked (3)
-                    P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] = make_uint4(i | ((r == WIN_MORE ? 2u : 3u) << 30), budget_left, dist_next, s3v.z);
-                }
             }
+            __syncwarp();
+            // ---- stage 2: leader payload, IDM, lane-change pre-tests (R3, R4)
+            const bool searched = live && r == WIN_DONE;
+            Lead ld;
+            ld.found = false;
+            ld.lead_abs = 0;
+            ld.v_lead = 0.0f;
+            V.need_lc = false;
+            if (searched) {
+                ld = lead_from_hit<W256>(pay, h);
+                pre_lc(P, t, V, ld);
+            }
+            __syncwarp();
+            // ---- stage 3: integrate, classify (R7, R8), next state and marks (R9); or defer
+            if (searched && !V.need_lc) {
+                const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+                write_out(P, t, sm, seg_base, i, V, O);
+            } else if (live) {
+                // deferred: must look at the adjacent lane (kinds 0 / 1, R5), or look-ahead to be continued (2) or walked (3)
+                const uint32_t kind = searched ? (ld.found ? 1u : 0u) : (r == WIN_MORE ? 2u : 3u);
+                P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] =
+                    searched ? make_uint4(i | (kind << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u)
+                             : make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
+            }
+            __syncwarp();
             base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
         }
         __syncthreads();   // the deferred list of this segment is complete (and visible: same block)
