@@ -50,6 +50,8 @@ extern "C" {
 /* manta_params.flags */
 #define MANTA_FLAG_MULTI_KERNEL 2u     /* three launches per timestep instead of the persistent cooperative kernel */
 #define MANTA_FLAG_RECORD_ACC 4u       /* keep each vehicle's last acceleration for manta_state.acc (tests)  */
+#define MANTA_FLAG_NO_FUSE 16u         /* admission of step t + 1 as a phase of its own (three grid barriers per step)
+                                          instead of inside the second phase of step t (A/B switch)              */
 #define MANTA_FLAG_NO_L2_PIN 8u        /* do not pin the occupancy planes in L2 (A/B switch; the default sets the
                                           device's cudaLimitPersistingL2CacheSize to the size of the two planes)   */
 

@@ -42,7 +42,9 @@ struct manta_sim {
     // host copies of the network
     uint32_t n_nodes = 0, n_edges = 0;
     std::vector<uint32_t> row_ptr, head, tail, len_c, cell_off;
-    std::vector<uint8_t> lanes;
+    std::vector<uint8_t> lanes, node_prio;
+    uint32_t min_len_c = 0;
+    bool fuse_admit = false;      // admission of step t + 1 runs inside the second phase of step t (two barriers per step)
     double max_limit = 0.0;
     uint64_t n_cells = 0;
     // trips
@@ -260,6 +262,10 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     P.seed_lo = (uint32_t)p.seed; P.seed_hi = (uint32_t)(p.seed >> 32);
     P.n_edges = M; P.flags = p.flags;
 
+    s->node_prio.assign(N, 0);
+    if (net->node_ctrl)
+        for (uint32_t u = 0; u < N; u++) s->node_prio[u] = net->node_ctrl[u] == MANTA_PRIORITY ? 1 : 0;
+    s->min_len_c = *std::min_element(s->len_c.begin(), s->len_c.end());
     // ---- device tables
     std::vector<uint4> et(M);
     for (uint32_t e = 0; e < M; e++) {
@@ -394,9 +400,9 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
                 return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "pre-placed vehicles closer than L on edge %llu", (unsigned long long)(keyx[k].first >> 32)));
     }
     // ---- admission FIFOs: waiting trips grouped by first edge, id order inside (G25)
-    // q_ent = {vehicle id, depart_step, route_start, depart_step of the next entry of the same queue or NONE}
-    std::vector<uint32_t> q_edge, q_ptr, q_next;
-    std::vector<uint4> q_ent, q_row;
+    // q_ent = {vehicle id, depart_step, route cursor, depart_step of the next entry of the same queue or NONE}
+    std::vector<uint32_t> q_edge, q_end;
+    std::vector<uint4> q_ent, q_row, q_state;
     {
         std::vector<uint32_t> cnt(s->n_edges + 1, 0);
         for (uint32_t id = 0; id < n_trips; id++) {
@@ -405,7 +411,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
             cnt[route_edges[route_ptr[tr]] + 1]++;
         }
         for (uint32_t e = 0; e < s->n_edges; e++) cnt[e + 1] += cnt[e];
-        q_ent.resize((size_t)cnt[s->n_edges] + 1);
+        q_ent.assign((size_t)cnt[s->n_edges] + 1, make_uint4(MANTA_NONE, MANTA_NONE, 0u, MANTA_NONE));
         std::vector<uint32_t> fill(cnt.begin(), cnt.end() - 1);
         for (uint32_t id = 0; id < n_trips; id++) {
             const uint32_t tr = trip_of_id[id];
@@ -415,15 +421,18 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         for (uint32_t e = 0; e < s->n_edges; e++)
             if (cnt[e + 1] > cnt[e]) {
                 q_edge.push_back(e);
-                q_ptr.push_back(cnt[e]);
-                q_next.push_back(q_ent[cnt[e]].y);
+                q_end.push_back(cnt[e + 1]);
+                const uint4 h = q_ent[cnt[e]];
+                q_state.push_back(make_uint4(h.y, cnt[e], h.x, h.z));
                 for (uint32_t k = cnt[e]; k + 1 < cnt[e + 1]; k++) q_ent[k].w = q_ent[k + 1].y;
             }
-        q_ptr.push_back(cnt[s->n_edges]);
     }
     // ---- launch geometry and vehicle segments.  A segment is processed by one block per phase; the persistent
     // kernel needs all of its blocks co-resident (cooperative launch), so n_seg = that grid.
     s->w256 = s->prm.lookahead_cells <= 256u && s->prm.lookback_cells <= 128u;
+    // fused admission (see admit_phase): a claim loser's mark (last cell of its row) must lie beyond the entry
+    // window [0, L_c], and a winner's landing cell must fit the first occupancy word
+    s->fuse_admit = !(s->prm.flags & MANTA_FLAG_NO_FUSE) && s->min_len_c >= s->P.L_c + 2u && s->P.Z_out <= 63u;
     {
         int occ = 0, coop = 0;
         if (s->w256)
@@ -441,12 +450,13 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (cap >= 0xFFFFFFFFull) return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
     // ---- upload; expand the route store on the device
     int rc;
-    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qh, *d_qn;
+    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qend;
     uint64_t *d_rp = nullptr;
-    uint4 *d_route, *d_qent, *d_qrow;
+    uint4 *d_route, *d_qent, *d_qrow, *d_qstate;
     for (size_t k = 0; k < q_edge.size(); k++) {
         const uint32_t e = q_edge[k];
-        q_row.push_back(make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16), e, 0u));
+        const uint32_t prio_word = s->node_prio[s->tail[e]] ? s->n_edges * 8u + s->tail[e] : MANTA_NONE;
+        q_row.push_back(make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16), prio_word, e));
     }
     if ((rc = upload(s, &d_re, route_edges, total))) return rollback(rc);
     if ((rc = upload(s, &d_rp, route_ptr, (uint64_t)n_trips + 1))) return rollback(rc);
@@ -463,8 +473,9 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if ((rc = alloc_fill(s, &d_arr, n_trips, 0xFF))) return rollback(rc);
     if ((rc = upload(s, &d_qrow, q_row.data(), q_row.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qent, q_ent.data(), q_ent.size()))) return rollback(rc);
-    if ((rc = upload(s, &d_qh, q_ptr.data(), q_edge.size()))) return rollback(rc);   // heads start at the queue starts
-    if ((rc = upload(s, &d_qn, q_next.data(), q_next.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qend, q_end.data(), q_end.size()))) return rollback(rc);
+    if ((rc = upload(s, &d_qstate, q_state.data(), q_state.size()))) return rollback(rc);
+    if ((rc = alloc_fill(s, &P.cand_info, n_trips, 0))) return rollback(rc);
     for (int k = 0; k < 2; k++) {
         uint4 **arr[4] = {&P.st[k].S0, &P.st[k].S1, &P.st[k].S2, &P.st[k].S3};
         for (int a = 0; a < 4; a++) {
@@ -492,7 +503,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     P.dlist = (uint4 *)dev_alloc(s, cap * sizeof(uint4));
     if (!P.xlist || !P.dlist) return rollback(fail(s, MANTA_ERR_OOM, "vehicle array allocation failed"));
     P.route = d_route; P.route_start = d_rs; P.admit_step = d_adm; P.arrive_step = d_arr;
-    P.q_row = d_qrow; P.q_ent = d_qent; P.q_head = d_qh; P.q_next = d_qn; P.q_ptr = nullptr;
+    P.q_row = d_qrow; P.q_ent = d_qent; P.q_end = d_qend; P.q_state = d_qstate;
     P.n_queues = (uint32_t)q_edge.size();
     const uint32_t n_init = (uint32_t)init_a0.size();
     if (n_init) {
@@ -562,26 +573,43 @@ cudaError_t launch_k(const manta_sim *s, void (*kern)(KArgs...), int grid, int b
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-// three launches per timestep (MANTA_FLAG_MULTI_KERNEL, manta_step_timed, devices without cooperative launch)
-void launch_step_multi(manta_sim *s, uint32_t t, cudaEvent_t *ev)
+void launch_sort(manta_sim *s, uint32_t t)   // spatial re-sort of the vehicle slots before step t (five stages)
 {
-    if (t != 0u && t % MANTA_SORT_EVERY == 0u) {   // spatial re-sort of the vehicle slots (five stages)
-        const int from = (int)(((t - 1u) / MANTA_SORT_EVERY) & 1u);
-        launch_k(s, k_sort_zero, s->grid_step, MANTA_NT, false, s->P);
-        launch_k(s, k_sort_count, s->grid_step, MANTA_NT, false, s->P, from);
-        launch_k(s, k_sort_partial, s->grid_step, MANTA_NT, false, s->P);
-        launch_k(s, k_sort_scan, s->grid_step, MANTA_NT, false, s->P);
-        launch_k(s, k_sort_scatter, s->grid_step, MANTA_NT, false, s->P, from);
-        s->launches += 5;
-    }
+    const int from = (int)(((t - 1u) / MANTA_SORT_EVERY) & 1u);
+    launch_k(s, k_sort_zero, s->grid_step, MANTA_NT, false, s->P);
+    launch_k(s, k_sort_count, s->grid_step, MANTA_NT, false, s->P, from);
+    launch_k(s, k_sort_partial, s->grid_step, MANTA_NT, false, s->P);
+    launch_k(s, k_sort_scan, s->grid_step, MANTA_NT, false, s->P);
+    launch_k(s, k_sort_scatter, s->grid_step, MANTA_NT, false, s->P, from);
+    s->launches += 5;
+}
+bool sort_due_host(uint32_t t) { return t != 0u && t % MANTA_SORT_EVERY == 0u; }
+
+// Kernel-per-phase stepping (MANTA_FLAG_MULTI_KERNEL, manta_step_timed, devices without cooperative launch):
+// step t of a call whose last step is t_last.  The admission of step t + 1 rides in the second-phase launch of
+// step t when fused; the first step of a call always admits on its own.
+void launch_step_multi(manta_sim *s, uint32_t t, bool first, bool last, cudaEvent_t *ev)
+{
     if (ev) cudaEventRecord(ev[0], s->stream);
-    launch_k(s, k_admit, s->grid_admit, 256, false, s->P, t);
+    if (first) {
+        if (sort_due_host(t)) launch_sort(s, t);
+        launch_k(s, k_admit, s->grid_admit, 256, false, s->P, t);
+        s->launches += 1;
+    }
     if (ev) cudaEventRecord(ev[1], s->stream);
     launch_k(s, s->w256 ? k_update<true> : k_update<false>, s->grid_step, MANTA_NT, false, s->P, t);
     if (ev) cudaEventRecord(ev[2], s->stream);
-    launch_k(s, k_second, s->grid_step, 256, false, s->P, t);
+    const int admit_next = (!last && s->fuse_admit) ? 1 : 0;
+    launch_k(s, k_second, s->grid_step, 256, false, s->P, t, admit_next);
+    s->launches += 2;
+    if (!last) {
+        if (sort_due_host(t + 1u)) launch_sort(s, t + 1u);
+        if (!admit_next) {
+            launch_k(s, k_admit, s->grid_admit, 256, false, s->P, t + 1u);
+            s->launches += 1;
+        }
+    }
     if (ev) cudaEventRecord(ev[3], s->stream);
-    s->launches += 3;
 }
 
 }  // namespace
@@ -592,13 +620,13 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
     if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
     if ((s->prm.flags & MANTA_FLAG_MULTI_KERNEL) || s->grid_persist == 0) {
-        for (uint32_t k = 0; k < n_steps; k++) launch_step_multi(s, s->t++, nullptr);
+        for (uint32_t k = 0; k < n_steps; k++, s->t++) launch_step_multi(s, s->t, k == 0, k + 1 == n_steps, nullptr);
     } else {
         // one cooperative launch per chunk of timesteps; the grid barrier words restart from zero every launch
         for (uint32_t done = 0; done < n_steps;) {
             uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s->t;
             CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 33 * sizeof(unsigned int), s->stream));   // bar_count .. bar_gen
-            CUDA_TRY(s, launch_k(s, s->w256 ? k_persistent<true> : k_persistent<false>, s->grid_persist, MANTA_NT, true, s->P, t0, m));
+            CUDA_TRY(s, launch_k(s, s->w256 ? k_persistent<true> : k_persistent<false>, s->grid_persist, MANTA_NT, true, s->P, t0, m, s->fuse_admit ? 1 : 0));
             s->launches += 1;
             s->t += m;
             done += m;
@@ -619,7 +647,7 @@ int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
     for (auto &e : ev) CUDA_TRY(s, cudaEventCreate(&e));
     for (uint32_t done = 0; done < n_steps;) {
         const uint32_t m = std::min(CH, n_steps - done);
-        for (uint32_t k = 0; k < m; k++) launch_step_multi(s, s->t++, &ev[4 * k]);
+        for (uint32_t k = 0; k < m; k++, s->t++) launch_step_multi(s, s->t, done + k == 0, done + k + 1 == n_steps, &ev[4 * k]);
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
         for (uint32_t k = 0; k < m; k++)
             for (int ph = 0; ph < 3; ph++) {

@@ -51,7 +51,8 @@ typedef unsigned long long u64;
 //          (lane clamped hop by hop, R2) }
 //   S3 = { len_c of edges +1 | +2 << 16, len_c of edges +3 | +4 << 16 (0 = the route ended before),
 //          bit 0: the route goes on past edge +4, bits 1-3: the (clamped) lane the look-ahead is in on edge +4,
-//          claim word of R8 for this edge's end }
+//          bits 4-31: head node of this edge if it is a PRIORITY node (its claim word of R8),
+//          lane entry (e+ * 8 + lanes(e+) - 1) the vehicle heads for at this edge's end }
 // A stayer rewrites S0 only (S1 when its tag or lane changed, S2/S3 when its lane changed).  A vehicle that
 // arrives leaves a GHOST in its slot for one step, which toggles the vehicle's last mark off (that mark is in the
 // plane everybody reads during the arrival step, so it cannot be cleared earlier) and then frees the slot.
@@ -132,11 +133,11 @@ struct DevP {
     uint32_t *admit_step;
     uint32_t *arrive_step;
     // admission queues: one FIFO per origin edge (reading G25), entries in vehicle-id order
-    const uint4 *q_row;          // [n_queues] edge_tab record of the origin edge
-    const uint32_t *q_ptr;       // [n_queues + 1]
-    const uint4 *q_ent;          // [waiting trips] {vehicle id, depart_step, route_start, edge id}
-    uint32_t *q_head;            // [n_queues]
-    uint32_t *q_next;            // [n_queues] depart_step of the head entry (NONE when the queue is exhausted)
+    const uint4 *q_row;          // [n_queues] {cell_off, len_c | lanes << 16, claim word of the tail node if it is PRIORITY else NONE, edge id}
+    const uint4 *q_ent;          // [waiting trips + 1] {vehicle id, depart_step, route cursor, depart_step of the next entry}
+    const uint32_t *q_end;       // [n_queues] index in q_ent one past the queue's last entry
+    uint4 *q_state;              // [n_queues] head of the FIFO: {its depart_step (NONE: exhausted), index in q_ent, vehicle id, route cursor}
+    uint2 *cand_info;            // [n_trips] written by an edge-end candidate: {lane entry e+ * 8 + l+ it heads for, cell it would land in}
     // claims, counters, tables
     u64 *claim;                  // [n_edges * 8 + n_nodes]
     uint32_t *edge_entries;
@@ -362,16 +363,16 @@ __device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint3
         l = ended ? l : lk;
         ended = ended || GEOM_LAST(g) != 0u;
     }
-    uint32_t word = 0u;
+    // lane entry (e+, l+) the vehicle heads for at the end of this edge; the low 3 bits hold lanes(e+) - 1 until l'
+    // is known.  Behind a PRIORITY node the claim word of R8 is the node instead: its id goes into S3.z.
+    uint32_t word = 0u, node = 0u;
     if (!GEOM_LAST(geom_cur)) {
-        if (GEOM_PRIO(geom_cur))       // PRIORITY: the claim word is the head node of this edge (R8)
-            word = P.n_edges * 8u + P.edge_tab[rp[0].z].z;
-        else                           // GREEN: lane entry (e+, l+); the low 3 bits hold lanes(e+) - 1 until l' is known
-            word = r[0].z * 8u + (GEOM_LANES(r[0].y) - 1u);
+        word = r[0].z * 8u + (GEOM_LANES(r[0].y) - 1u);
+        if (GEOM_PRIO(geom_cur)) node = P.edge_tab[rp[0].z].z;
     }
     Hops h;
     h.s2 = make_uint4(roww[0], roww[1], roww[2], roww[3]);
-    h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), (ended ? 0u : 1u) | (l << 1), word);
+    h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), (ended ? 0u : 1u) | (l << 1) | (node << 4), word);
     return h;
 }
 

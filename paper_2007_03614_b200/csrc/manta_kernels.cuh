@@ -57,6 +57,7 @@ struct Veh {
     uint32_t len_c, n, l, c, pitch;
     bool last;
     uint32_t claim;     // S3.w
+    uint32_t hopz;      // S3.z
     // after pre_lc
     float acc_cur;
     int32_t bound;
@@ -437,7 +438,9 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
             S.S0[at] = make_uint4(0u, 0u, cur_abs, ID_GHOST);   // the ghost clears the time-t mark in the next step
         } else {
             // smallest id wins; the key carries ~t in the high word so claim words never need a reset
-            const uint32_t word = GEOM_PRIO(V.geom) ? V.claim : (V.claim & ~7u) + min(O.l_new, V.claim & 7u);
+            const uint32_t target = (V.claim & ~7u) + min(O.l_new, V.claim & 7u);   // lane entry (e+, l+)
+            const uint32_t word = GEOM_PRIO(V.geom) ? P.n_edges * 8u + (V.hopz >> 4) : target;
+            P.cand_info[V.id] = make_uint2(target, O.nx >> 10);
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)V.id;
             atomicMin(&P.claim[word], key);
             P.xlist[seg_base + atomicAdd(&sm.xn, 1u)] = make_uint4(slot, word, V.cursor, V.id);
@@ -481,35 +484,63 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
 }
 
 // ------------------------------------------------------------------------------------------------ A: R1
-// Departure admission (G17, G25).  Thread k owns the FIFO of one origin edge; trips in it are in
-// vehicle-id (= departure) order, so the head is the smallest waiting id on that edge.
-__device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t gtid, uint32_t gsize)
+// Departure admission (G17, G25) for step t.  Thread k owns the FIFO of one origin edge; trips in it
+// are in vehicle-id (= departure) order, so the head is the smallest waiting id on that edge.  New vehicles go
+// into state buffer sb.
+// FUSED = false: runs between two grid barriers; atlas_t is complete.
+// FUSED = true : runs in the same phase as second_phase(t - 1), whose winners may be writing their marks into the
+// entry windows tested here.  The only marks of that phase that can fall into a window [0, L_c] are those of claim
+// winners (losers hold in the last cell of a row, which lies beyond the window: the host fuses only if every edge
+// has at least L_c + 2 cells), at most one per lane entry, and which vehicle wins and where it lands can be read
+// from the claim word and cand_info: the winner's bit is ORed into the word, whether its toggle has landed or not.
+template <bool FUSED>
+__device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb, uint32_t gtid, uint32_t gsize)
 {
     const int cur = (int)(t & 1u);
-    const StBuf &S = P.st[sbuf_of(t)];
+    const StBuf &S = P.st[sb];
     u64 *B = P.bits[cur];
     uint2 *pay = P.pay[cur];
     const u64 window = bits_below(P.L_c + 1u);
     for (uint32_t k = gtid; k < P.n_queues; k += gsize) {
-        if (P.q_next[k] > t) continue;                 // idle (or exhausted: NONE) queue
-        const uint32_t h = P.q_head[k];
+        const uint4 qs = P.q_state[k];                 // {depart_step, index in q_ent, vehicle id, route cursor} of the head
+        if (qs.x > t) continue;                        // idle (or exhausted: NONE) queue
         const uint4 er = P.q_row[k];
-        const uint4 ent = P.q_ent[h];                  // {id, depart_step, route_start, depart_step of the next entry}
+        const uint4 nx = P.q_ent[qs.y + 1u];           // the entry that becomes the head (padding entry after the last)
+        const uint32_t id = qs.z, cursor = qs.w;
+        const uint4 rr = P.route[cursor];
         const uint32_t len = GEOM_LEN(er.y), lanes = GEOM_LANES(er.y), pitch = pitch_of(len);
+        uint32_t seg = P.bucket_seg[er.x >> MANTA_BUCKET_SHIFT];   // the segment whose vehicles are in this stretch of the atlas
         u64 w[MANTA_MAX_LANES_DEV];
 #pragma unroll
         for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++) w[l] = l < lanes ? B[(er.x + l * pitch) >> 6] : ~0ull;
+        if (FUSED) {
+            const uint32_t stamp = 0xFFFFFFFFu - (t - 1u);   // claims of the step whose second phase is running
+            u64 key[MANTA_MAX_LANES_DEV];
+#pragma unroll
+            for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++) {
+                key[l] = ~0ull;
+                if (er.z != CELL_NONE) {               // PRIORITY tail node: one claim word for all entries
+                    if (l == 0u) key[l] = P.claim[er.z];
+                } else if (l < lanes) {
+                    key[l] = P.claim[er.w * 8u + l];
+                }
+            }
+#pragma unroll
+            for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++)
+                if ((uint32_t)(key[l] >> 32) == stamp && (uint32_t)key[l] != CELL_NONE) {   // (never-claimed words are all ones)
+                    const uint2 ci = P.cand_info[(uint32_t)key[l]];   // {lane entry it heads for, landing cell}
+#pragma unroll
+                    for (uint32_t m = 0; m < MANTA_MAX_LANES_DEV; m++)
+                        if (ci.x == er.w * 8u + m) w[m] |= 1ull << (ci.y & 63u);
+                }
+        }
         uint32_t l_sel = 0xFFFFFFFFu;
 #pragma unroll
         for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++)
             if (l_sel == 0xFFFFFFFFu && !(w[l] & window)) l_sel = l;   // first lane whose window [0, L_c] is free
         if (l_sel == 0xFFFFFFFFu) continue;
-        const uint32_t id = ent.x, cursor = ent.z;
-        const uint4 rr = P.route[cursor];
         const uint32_t geom = (rr.y & GEOM_STATIC_MASK) | (l_sel << 28);
         const Hops hp = build_hops(P, cursor, geom, l_sel);
-        // the segment that currently holds the vehicles of this stretch of the atlas (see the re-sort)
-        uint32_t seg = P.bucket_seg[er.x >> MANTA_BUCKET_SHIFT];
         uint32_t slot;
         for (;;) {
             slot = atomicAdd(&P.seg_cnt[seg], 1u);
@@ -528,8 +559,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, uint32_t 
         pay_store(P, pay, row, 0u, 0u);
         P.admit_step[id] = t;
         atomicAdd(&P.edge_entries[rr.z], 1u);
-        P.q_head[k] = h + 1u;
-        P.q_next[k] = ent.w;
+        P.q_state[k] = make_uint4(qs.y + 1u < P.q_end[k] ? nx.y : CELL_NONE, qs.y + 1u, nx.x, nx.z);
     }
 }
 
@@ -709,7 +739,8 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     const uint32_t slot = e.x & 0x3FFFFFFFu, kind = e.x >> 30;
     Veh V;
     veh_load(V, S.S0[seg_base + slot], S.S1[seg_base + slot]);
-    V.claim = 0u;
+    V.claim = 0u;   // a deferred vehicle cannot reach its edge end
+    V.hopz = 0u;
     Lead ld;
     if (kind >= 2u) {
         const Hit h = kind == 2u ? leader_continue(P, B, V, e.w, e.y, e.z, n_cells) : walk_rows(P, B, V, n_cells);
@@ -772,6 +803,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             Veh V;
             veh_load(V, s0v, s1v);
             V.claim = s3v.w;
+            V.hopz = s3v.z;
             Hit h;
             h.found = false;
             h.cell = 0u;
@@ -901,7 +933,7 @@ __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint3
 // ------------------------------------------------------------------------------------------------ kernels
 __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 {
-    admit_phase(P, t, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    admit_phase<false>(P, t, sbuf_of(t), blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
 template <bool W256>
@@ -915,7 +947,12 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, u
     flush_stats(P, sm, n_cells, n_upd);
 }
 
-__global__ void __launch_bounds__(256) k_second(const DevP P, uint32_t t) { second_phase(P, t); }
+// second phase of step t; with admit_next, the admission of step t + 1 runs in the same launch (fused, see admit_phase)
+__global__ void __launch_bounds__(256) k_second(const DevP P, uint32_t t, int admit_next)
+{
+    if (admit_next) admit_phase<true>(P, t + 1u, sbuf_of(t), blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    second_phase(P, t);
+}
 
 // the five stages of the re-sort as kernels (multi-kernel mode); n_live / per_seg travel through sort_part[n_seg..]
 __global__ void __launch_bounds__(MANTA_NT) k_sort_zero(const DevP P) { sort_zero(P); }
@@ -983,40 +1020,54 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     return *s_flag == 0u;
 }
 
-// One cooperative launch = n_steps timesteps; the host is not involved between steps.
+__device__ __forceinline__ bool sort_all(const DevP &P, UpdateSmem &sm, int from, unsigned &gen)
+{
+    uint32_t n_live, per_seg;
+    sort_zero(P);
+    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    sort_count(P, from);
+    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    sort_partial(P, sm);
+    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    sort_scan(P, sm, n_live, per_seg);
+    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    sort_scatter(P, from, n_live, per_seg);
+    return grid_barrier(P.ctr, gen, &sm.flag);
+}
+
+// One cooperative launch = n_steps timesteps; the host is not involved between steps.  Two grid barriers per
+// timestep when the admission of step t + 1 is fused into the second phase of step t (fuse != 0), else three.
 template <bool W256>
-__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps)
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps, int fuse)
 {
     __shared__ UpdateSmem sm;
     if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
     unsigned gen = 0u;
     uint32_t n_cells = 0u, n_upd = 0u;
     const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
-    for (uint32_t t = t0; t < t0 + n_steps; t++) {
-        if (sort_due(t)) {
-            const int from = sbuf_of(t - 1u);
-            uint32_t n_live, per_seg;
-            sort_zero(P);
-            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-            sort_count(P, from);
-            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-            sort_partial(P, sm);
-            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-            sort_scan(P, sm, n_live, per_seg);
-            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-            sort_scatter(P, from, n_live, per_seg);
-            if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
-        }
+    const uint32_t t_end = t0 + n_steps;
+    // the first step of a launch: re-sort if due, admission on its own
+    if (sort_due(t0) && !sort_all(P, sm, sbuf_of(t0 - 1u), gen)) return;
+    admit_phase<false>(P, t0, sbuf_of(t0), gtid, gsize);
+    if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+    for (uint32_t t = t0; t < t_end; t++) {
         DBG_STAMP(0);
-        admit_phase(P, t, gtid, gsize);
-        if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         update_phase<W256>(P, t, sm, n_cells, n_upd);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(4);
+        const bool more = t + 1u < t_end;
+        if (more && fuse) admit_phase<true>(P, t + 1u, sbuf_of(t), gtid, gsize);   // the longer dependent chain first
         second_phase(P, t);
         DBG_STAMP(5);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(6);
+        if (more) {
+            if (sort_due(t + 1u) && !sort_all(P, sm, sbuf_of(t), gen)) return;
+            if (!fuse) {
+                admit_phase<false>(P, t + 1u, sbuf_of(t + 1u), gtid, gsize);
+                if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
+            }
+        }
     }
     flush_stats(P, sm, n_cells, n_upd);
 }

@@ -256,3 +256,17 @@ def test_full_size_network_peak_window(oracle_mod, binding):
     assert net["n_edges"] > 500000 and len(trips["depart_time_s"]) > 20000
     s, n_launch = run_both(oracle_mod, binding, net, trips, params, 700, dense_until=0, every=100, flags=0)
     assert n_launch == 7 and s["vehicle_updates"] > 5_000_000
+
+
+@pytest.mark.parametrize("flags", [0, 2, 16, 18])
+@pytest.mark.parametrize("ctrl", [wl.GREEN, wl.PRIORITY])
+def test_admission_fused_with_second_phase(oracle_mod, binding, ctrl, flags):
+    """Heavy demand on a small grid of short edges, compared every 3 steps: inside a manta_step call the admission of
+    step t + 1 runs in the same phase as the claim resolution of step t (flags 0 / 2), so claim winners land in the
+    very entry windows that admission is testing; flags 16 / 18 (MANTA_FLAG_NO_FUSE) keep the phase of its own."""
+    net = wl.grid_network(nx=4, ny=3, edge_len=40.0, lanes=2, ctrl=ctrl)
+    o_, d_ = wl.uniform_od(net, 1500, 41)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(1500, 0.0, 150.0, 42), n_threads=2)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1200, dense_until=0, every=3,
+                    atlas_every=300, flags=flags)
+    assert s["n_done"] > 300
