@@ -524,7 +524,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
-    s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, (uint32_t)s->sm_count * 8u));
+    s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, (uint32_t)s->sm_count * 8u));   // k_admit alone
     return MANTA_OK;
 }
 

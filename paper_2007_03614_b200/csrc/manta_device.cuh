@@ -346,34 +346,48 @@ __device__ __forceinline__ bool last_set_w(const u64 *B, uint32_t row, uint32_t 
 struct Hops {
     uint4 s2, s3;
 };
-__device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint32_t geom_cur, uint32_t l)
+struct HopRecs {
+    uint4 r[4];   // RouteRecs cursor + 1 .. cursor + 4
+};
+// the loads, separated from the arithmetic so that callers can issue them together with their other gathers
+__device__ __forceinline__ HopRecs load_hop_recs(const DevP &P, uint32_t cursor)
 {
+    HopRecs R;
     const uint4 *rp = P.route + cursor;
-    uint4 r[4];
 #pragma unroll
-    for (int k = 0; k < 4; k++) r[k] = rp[k + 1];
+    for (int k = 0; k < 4; k++) R.r[k] = rp[k + 1];
+    return R;
+}
+// node: head node of the current edge if it is a PRIORITY node (GEOM_PRIO(geom_cur)), else ignored
+__device__ __forceinline__ Hops make_hops(const HopRecs &R, uint32_t geom_cur, uint32_t l, uint32_t node)
+{
     bool ended = GEOM_LAST(geom_cur) != 0u;
     uint32_t roww[4], len[4];
 #pragma unroll
     for (int k = 0; k < 4; k++) {
-        const uint32_t g = r[k].y;
+        const uint32_t g = R.r[k].y;
         const uint32_t lk = min(l, GEOM_LANES(g) - 1u);
-        roww[k] = ended ? 0u : (r[k].x + lk * pitch_of(GEOM_LEN(g))) >> 6;
+        roww[k] = ended ? 0u : (R.r[k].x + lk * pitch_of(GEOM_LEN(g))) >> 6;
         len[k] = ended ? 0u : GEOM_LEN(g);
         l = ended ? l : lk;
         ended = ended || GEOM_LAST(g) != 0u;
     }
     // lane entry (e+, l+) the vehicle heads for at the end of this edge; the low 3 bits hold lanes(e+) - 1 until l'
     // is known.  Behind a PRIORITY node the claim word of R8 is the node instead: its id goes into S3.z.
-    uint32_t word = 0u, node = 0u;
-    if (!GEOM_LAST(geom_cur)) {
-        word = r[0].z * 8u + (GEOM_LANES(r[0].y) - 1u);
-        if (GEOM_PRIO(geom_cur)) node = P.edge_tab[rp[0].z].z;
-    }
+    uint32_t word = 0u;
+    if (!GEOM_LAST(geom_cur)) word = R.r[0].z * 8u + (GEOM_LANES(R.r[0].y) - 1u);
+    if (GEOM_LAST(geom_cur) || !GEOM_PRIO(geom_cur)) node = 0u;
     Hops h;
     h.s2 = make_uint4(roww[0], roww[1], roww[2], roww[3]);
     h.s3 = make_uint4(len[0] | (len[1] << 16), len[2] | (len[3] << 16), (ended ? 0u : 1u) | (l << 1) | (node << 4), word);
     return h;
+}
+__device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint32_t geom_cur, uint32_t l)
+{
+    const HopRecs R = load_hop_recs(P, cursor);
+    uint32_t node = 0u;
+    if (!GEOM_LAST(geom_cur) && GEOM_PRIO(geom_cur)) node = P.edge_tab[P.route[cursor].z].z;
+    return make_hops(R, geom_cur, l, node);
 }
 
 }  // namespace manta

@@ -494,8 +494,12 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
 // has at least L_c + 2 cells), at most one per lane entry, and which vehicle wins and where it lands can be read
 // from the claim word and cand_info: the winner's bit is ORed into the word, whether its toggle has landed or not.
 template <bool FUSED>
-__device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb, uint32_t gtid, uint32_t gsize)
+__device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb)
 {
+    // queue k is served by block k % gridDim, counted down from the block's LAST thread: the queues are spread over
+    // all blocks, away from the low threads that carry the cross-list entries of the same phase
+    const uint32_t gsize = gridDim.x * blockDim.x;
+    const uint32_t gtid = blockIdx.x + gridDim.x * (blockDim.x - 1u - threadIdx.x);
     const int cur = (int)(t & 1u);
     const StBuf &S = P.st[sb];
     u64 *B = P.bits[cur];
@@ -505,9 +509,12 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb, u
         const uint4 qs = P.q_state[k];                 // {depart_step, index in q_ent, vehicle id, route cursor} of the head
         if (qs.x > t) continue;                        // idle (or exhausted: NONE) queue
         const uint4 er = P.q_row[k];
+        const uint32_t q_end = P.q_end[k];
         const uint4 nx = P.q_ent[qs.y + 1u];           // the entry that becomes the head (padding entry after the last)
         const uint32_t id = qs.z, cursor = qs.w;
         const uint4 rr = P.route[cursor];
+        const HopRecs hr = load_hop_recs(P, cursor);   // all gathers of this admission are requested here, together
+        const uint32_t head_node = P.edge_tab[er.w].z;
         const uint32_t len = GEOM_LEN(er.y), lanes = GEOM_LANES(er.y), pitch = pitch_of(len);
         uint32_t seg = P.bucket_seg[er.x >> MANTA_BUCKET_SHIFT];   // the segment whose vehicles are in this stretch of the atlas
         u64 w[MANTA_MAX_LANES_DEV];
@@ -540,7 +547,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb, u
             if (l_sel == 0xFFFFFFFFu && !(w[l] & window)) l_sel = l;   // first lane whose window [0, L_c] is free
         if (l_sel == 0xFFFFFFFFu) continue;
         const uint32_t geom = (rr.y & GEOM_STATIC_MASK) | (l_sel << 28);
-        const Hops hp = build_hops(P, cursor, geom, l_sel);
+        const Hops hp = make_hops(hr, geom, l_sel, head_node);
         uint32_t slot;
         for (;;) {
             slot = atomicAdd(&P.seg_cnt[seg], 1u);
@@ -559,7 +566,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb, u
         pay_store(P, pay, row, 0u, 0u);
         P.admit_step[id] = t;
         atomicAdd(&P.edge_entries[rr.z], 1u);
-        P.q_state[k] = make_uint4(qs.y + 1u < P.q_end[k] ? nx.y : CELL_NONE, qs.y + 1u, nx.x, nx.z);
+        P.q_state[k] = make_uint4(qs.y + 1u < q_end ? nx.y : CELL_NONE, qs.y + 1u, nx.x, nx.z);
     }
 }
 
@@ -883,13 +890,16 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t)
             const uint4 s1 = S.S1[at];
             const u64 won = P.claim[xl.y];
             const uint4 rn = P.route[xl.z + 1u];
+            const HopRecs hr = load_hop_recs(P, xl.z + 1u);   // requested with the other gathers; used by the winner
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)xl.w;
             uint32_t cell;
             if (won == key) {             // winner crosses
                 const uint32_t lplus = min(GEOM_LANE(s1.y), GEOM_LANES(rn.y) - 1u);
                 const uint32_t geom = (rn.y & GEOM_STATIC_MASK) | (lplus << 28);
                 const uint32_t row = rn.x + lplus * pitch_of(GEOM_LEN(rn.y));
-                const Hops hp = build_hops(P, xl.z + 1u, geom, lplus);
+                uint32_t node = 0u;
+                if (!GEOM_LAST(geom) && GEOM_PRIO(geom)) node = P.edge_tab[rn.z].z;
+                const Hops hp = make_hops(hr, geom, lplus, node);
                 S.S1[at] = make_uint4(row, geom, xl.z + 1u, rn.w);
                 S.S2[at] = hp.s2;
                 S.S3[at] = hp.s3;
@@ -933,7 +943,7 @@ __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint3
 // ------------------------------------------------------------------------------------------------ kernels
 __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 {
-    admit_phase<false>(P, t, sbuf_of(t), blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    admit_phase<false>(P, t, sbuf_of(t));
 }
 
 template <bool W256>
@@ -950,7 +960,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, u
 // second phase of step t; with admit_next, the admission of step t + 1 runs in the same launch (fused, see admit_phase)
 __global__ void __launch_bounds__(256) k_second(const DevP P, uint32_t t, int admit_next)
 {
-    if (admit_next) admit_phase<true>(P, t + 1u, sbuf_of(t), blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    if (admit_next) admit_phase<true>(P, t + 1u, sbuf_of(t));
     second_phase(P, t);
 }
 
@@ -1044,11 +1054,10 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
     if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
     unsigned gen = 0u;
     uint32_t n_cells = 0u, n_upd = 0u;
-    const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
     const uint32_t t_end = t0 + n_steps;
     // the first step of a launch: re-sort if due, admission on its own
     if (sort_due(t0) && !sort_all(P, sm, sbuf_of(t0 - 1u), gen)) return;
-    admit_phase<false>(P, t0, sbuf_of(t0), gtid, gsize);
+    admit_phase<false>(P, t0, sbuf_of(t0));
     if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     for (uint32_t t = t0; t < t_end; t++) {
         DBG_STAMP(0);
@@ -1056,7 +1065,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(4);
         const bool more = t + 1u < t_end;
-        if (more && fuse) admit_phase<true>(P, t + 1u, sbuf_of(t), gtid, gsize);   // the longer dependent chain first
+        if (more && fuse) admit_phase<true>(P, t + 1u, sbuf_of(t));   // the longer dependent chain first
         second_phase(P, t);
         DBG_STAMP(5);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
@@ -1064,7 +1073,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
         if (more) {
             if (sort_due(t + 1u) && !sort_all(P, sm, sbuf_of(t), gen)) return;
             if (!fuse) {
-                admit_phase<false>(P, t + 1u, sbuf_of(t + 1u), gtid, gsize);
+                admit_phase<false>(P, t + 1u, sbuf_of(t + 1u));
                 if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
             }
         }
