@@ -120,8 +120,7 @@ struct DevP {
     uint32_t *seg_cnt;
     uint4 *xlist;                // cross list of segment s at [s * seg_cap, ...): {slot, claim word, cursor, id}
     uint4 *dlist;                // deferred list of segment s, same place: {slot, lead_abs, v_lead bits, 0 | 1 found | 2 search to do}
-    uint32_t *seg_xn;            // cross-list entries of each segment (written by the update phase)
-    uint32_t *seg_qn;            // (unused)
+    uint32_t *seg_xn, *seg_qn;   // entries of the two lists of each segment (written by the update phase)
     // spatial re-sort (every MANTA_SORT_EVERY steps): counting sort of the live slots by atlas bucket
     uint32_t n_buckets;          // buckets of 2^MANTA_BUCKET_SHIFT atlas cells
     uint32_t *sort_hist;         // [n_buckets + 1] counts, then exclusive offsets
@@ -347,7 +346,8 @@ struct Hops {
     uint4 s2, s3;
 };
 struct HopRecs {
-    uint4 r[4];   // RouteRecs cursor + 1 .. cursor + 4
+    uint2 r[4];   // {cell_off, geom} of RouteRecs cursor + 1 .. cursor + 4
+    uint32_t e1;  // edge id of RouteRec cursor + 1
 };
 // the loads, separated from the arithmetic so that callers can issue them together with their other gathers
 __device__ __forceinline__ HopRecs load_hop_recs(const DevP &P, uint32_t cursor)
@@ -355,7 +355,8 @@ __device__ __forceinline__ HopRecs load_hop_recs(const DevP &P, uint32_t cursor)
     HopRecs R;
     const uint4 *rp = P.route + cursor;
 #pragma unroll
-    for (int k = 0; k < 4; k++) R.r[k] = rp[k + 1];
+    for (int k = 0; k < 4; k++) R.r[k] = *reinterpret_cast<const uint2 *>(rp + k + 1);
+    R.e1 = rp[1].z;
     return R;
 }
 // node: head node of the current edge if it is a PRIORITY node (GEOM_PRIO(geom_cur)), else ignored
@@ -375,7 +376,7 @@ __device__ __forceinline__ Hops make_hops(const HopRecs &R, uint32_t geom_cur, u
     // lane entry (e+, l+) the vehicle heads for at the end of this edge; the low 3 bits hold lanes(e+) - 1 until l'
     // is known.  Behind a PRIORITY node the claim word of R8 is the node instead: its id goes into S3.z.
     uint32_t word = 0u;
-    if (!GEOM_LAST(geom_cur)) word = R.r[0].z * 8u + (GEOM_LANES(R.r[0].y) - 1u);
+    if (!GEOM_LAST(geom_cur)) word = R.e1 * 8u + (GEOM_LANES(R.r[0].y) - 1u);
     if (GEOM_LAST(geom_cur) || !GEOM_PRIO(geom_cur)) node = 0u;
     Hops h;
     h.s2 = make_uint4(roww[0], roww[1], roww[2], roww[3]);
