@@ -230,7 +230,9 @@ def main():
     dev_bytes = sim.device_bytes
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     ev[0].record(stream)
+    sim.set_multi_kernel(False)                           # the untimed fast-forward always runs in the persistent kernel
     sim.step_async(args.start_step)                       # initialisation: advance to the peak (untimed region)
+    sim.set_multi_kernel(bool(args.flags & 2))
     ev[1].record(stream)
     sim.step(W)                                           # warm-up steps
     s0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
@@ -259,6 +261,7 @@ def main():
 
     # ---- roofline of the update-phase kernel: per-phase CUDA events on the launching stream ---------------
     sim = binding.Sim(net, params, trips, device=local, stream=stream)
+    sim.set_multi_kernel(False)
     sim.step(args.start_step + W)
     r0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
     Kp = min(K, 1200)

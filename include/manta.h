@@ -158,6 +158,10 @@ uint64_t manta_atlas_cells(const manta_sim *sim);
 int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch);
 
 int manta_set_stream(manta_sim *sim, void *cuda_stream);   /* cudaStream_t; work already enqueued is not moved */
+/* Switches between the persistent kernel and kernel-per-phase stepping for the following manta_step calls
+ * (on != 0: as if MANTA_FLAG_MULTI_KERNEL had been given).  Results are identical either way; profilers use it to
+ * advance a simulation in one launch and then look at single phases. */
+int manta_set_multi_kernel(manta_sim *sim, int on);
 uint64_t manta_launch_count(const manta_sim *sim);         /* kernels launched by this simulation so far   */
 uint64_t manta_device_bytes(const manta_sim *sim);         /* device memory held                           */
 void manta_destroy(manta_sim *sim);

@@ -20,7 +20,8 @@ FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_timed",
-           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_launch_count",
+           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_multi_kernel",
+           "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error")
 
 
@@ -86,6 +87,7 @@ def load_library():
     L.manta_atlas_cells.restype = C.c_uint64
     L.manta_readback_atlas.argtypes = [C.c_void_p] * 5
     L.manta_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    L.manta_set_multi_kernel.argtypes = [C.c_void_p, C.c_int]
     L.manta_launch_count.argtypes = [C.c_void_p]
     L.manta_launch_count.restype = C.c_uint64
     L.manta_device_bytes.argtypes = [C.c_void_p]
@@ -173,6 +175,9 @@ class Sim:
 
     def step(self, n=1):
         self._check(load_library().manta_step(self.h, int(n)))
+
+    def set_multi_kernel(self, on):
+        self._check(load_library().manta_set_multi_kernel(self.h, int(bool(on))))
 
     def step_async(self, n=1):
         self._check(load_library().manta_step_async(self.h, int(n)))

@@ -178,6 +178,16 @@ int manta_set_stream(manta_sim *sim, void *cuda_stream)
     return MANTA_OK;
 }
 
+int manta_set_multi_kernel(manta_sim *sim, int on)
+{
+    if (!sim) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (on)
+        sim->prm.flags |= MANTA_FLAG_MULTI_KERNEL;
+    else
+        sim->prm.flags &= ~MANTA_FLAG_MULTI_KERNEL;
+    return MANTA_OK;
+}
+
 int manta_create(const manta_network *net, const manta_params *prm, int cuda_device, manta_sim **out)
 {
     if (!net || !prm || !out) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null argument");
