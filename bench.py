@@ -183,6 +183,21 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def aggregate(ms, updates, world, device="cpu"):
+    """Whole-job figures of N independent replicas: MAX over ranks of the device time of the
+    timed region, SUM over ranks of the vehicle-updates processed in it; value = SUM / MAX.  These two reductions
+    (and the barriers around the timed region) are the only collectives of a multi-GPU run."""
+    import torch
+    import torch.distributed as dist
+    t_ms = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    t_upd = torch.tensor([float(updates)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(t_upd, op=dist.ReduceOp.SUM)
+    ms_max, upd_all = float(t_ms.item()), float(t_upd.item())
+    return ms_max, upd_all, upd_all / (ms_max * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -250,13 +265,7 @@ def main():
     s1 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
     launches = sim.launch_count - launches0
     upd = s1["vehicle_updates"] - s0["vehicle_updates"]
-    t_ms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    t_upd = torch.tensor([float(upd)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(t_upd, op=dist.ReduceOp.SUM)
-    ms_max, upd_all = float(t_ms.item()), float(t_upd.item())
-    value = upd_all / (ms_max * 1e-3)
+    ms_max, upd_all, value = aggregate(ms, upd, world, "cuda")
     sim.close()
 
     # ---- roofline of the update-phase kernel: per-phase CUDA events on the launching stream ---------------

@@ -37,7 +37,8 @@ def build_cuda(force=False, verbose=False):
     if res.returncode != 0:
         raise RuntimeError("nvcc failed")
     with open(os.path.join(_HERE, "libmanta.ptxas.txt"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+        log = "".join(l for l in (res.stdout + res.stderr).splitlines(True) if "Compile time" not in l)
+        f.write(" ".join(cmd) + "\n" + log)
     return LIB
 
 
