@@ -336,6 +336,48 @@ __device__ __forceinline__ bool last_set_w(const u64 *B, uint32_t row, uint32_t 
     return false;
 }
 
+// R5 in one round of loads (H <= 256, lookback <= 128): lead = first occupied cell in [c, end) and lag = last occupied
+// cell in [b0, c) of the row; the up-to-five words ahead and up-to-three words behind are requested together.
+__device__ __forceinline__ void lead_lag_w(const u64 *B, uint32_t row, uint32_t c, uint32_t end, uint32_t b0, bool &has_a, uint32_t &ja,
+                                           bool &has_b, uint32_t &jb)
+{
+    const u64 *p = B + (row >> 6);
+    const uint32_t w0 = c >> 6, wl = (end - 1u) >> 6;        // c < end: R4 allows lane changes only before len_c - Z_out
+    const uint32_t v0 = b0 >> 6, vl = (c - 1u) >> 6;         // used only when c > b0
+    const bool back = c > b0;
+    u64 m[5], k[3];
+#pragma unroll
+    for (uint32_t i = 0; i < 5u; i++) m[i] = (w0 + i <= wl) ? p[w0 + i] : 0ull;
+#pragma unroll
+    for (uint32_t i = 0; i < 3u; i++) k[i] = (back && vl >= v0 + i) ? p[vl - i] : 0ull;
+    m[0] &= ~0ull << (c & 63u);
+    const u64 tail = bits_below(end - (wl << 6));
+    has_a = false;
+#pragma unroll
+    for (int i = 4; i >= 0; i--) {
+        if (w0 + (uint32_t)i == wl) m[i] &= tail;
+        if (m[i]) {
+            ja = ((w0 + (uint32_t)i) << 6) + (uint32_t)__ffsll((long long)m[i]) - 1u;
+            has_a = true;
+        }
+    }
+    has_b = false;
+    if (back) {
+        k[0] &= bits_below(c - (vl << 6));
+        const u64 head = ~0ull << (b0 & 63u);
+#pragma unroll
+        for (int i = 2; i >= 0; i--) {
+            if (vl >= v0 + (uint32_t)i) {
+                if (vl - (uint32_t)i == v0) k[i] &= head;
+                if (k[i]) {
+                    jb = ((vl - (uint32_t)i) << 6) + 63u - (uint32_t)__clzll((long long)k[i]);
+                    has_b = true;
+                }
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------- look-ahead cache
 // What R2 needs of the four route edges after the current one, for a vehicle at RouteRec `cursor` in lane l:
 // the word index of the row it would continue in (lane clamped hop by hop: "the lane index carried on is the

@@ -31,6 +31,15 @@ namespace manta {
 #ifndef MANTA_MINB
 #define MANTA_MINB 2      // blocks per SM the step kernels are compiled for
 #endif
+#ifndef MANTA_BAR
+#define MANTA_BAR 1       // grid barrier: 1 = release reduction + polling the arrival counter, 0 = atomicAdd + generation word
+#endif
+#ifndef MANTA_DQ
+#define MANTA_DQ 0        // deferred-list entries a block keeps in shared memory (0: all in P.dlist)
+#endif
+#ifndef MANTA_PF
+#define MANTA_PF 3        // state records requested ahead: 1 = next chunk into L2, 2 = into L1, 3 = 1 + the first chunks of step t + 1 before the grid barrier
+#endif
 #define MANTA_NW (MANTA_NT / 32)
 #define MANTA_NS 8        // occupancy words the fast look-ahead search requests per vehicle
 #define MANTA_MAX_LANES_DEV 8u
@@ -43,6 +52,14 @@ __device__ __forceinline__ u64 gtimer() { u64 v; asm volatile("mov.u64 %0, %glob
 #else
 #define DBG_STAMP(k) do { } while (0)
 #endif
+__device__ __forceinline__ void prefetch_line(const void *p)
+{
+#if MANTA_PF == 2
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#else
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
 struct Lead {
     bool found;
     int32_t lead_abs;   // leader position in the follower's frame, Q22.10 (R2)
@@ -75,6 +92,9 @@ struct UpdateSmem {
     uint32_t ev[4];               // event counters of this kernel: lane changes, lane-change evaluations, arrivals, travel steps
     uint32_t xn, qn, flag, next;  // per segment: cross-list / deferred-list entries, next unclaimed chunk; barrier flag
     uint32_t wsum[MANTA_NW];      // re-sort: per-warp partial sums
+#if MANTA_DQ
+    uint4 dq[MANTA_DQ][3];        // deferred entries with their vehicle records {S0, S1, entry}; the overflow goes to P.dlist
+#endif
 };
 enum { EV_LC = 0, EV_EVAL = 1, EV_DONE = 2, EV_TRAVEL = 3 };
 
@@ -465,8 +485,13 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
     const uint32_t rowt = V.lt > V.l ? V.row0 + V.pitch : V.row0 - V.pitch;
     uint32_t ja = 0u, jb = 0u;
     const uint32_t b0 = V.c > P.lookback ? V.c - P.lookback : 0u;
-    const bool has_a = scan_fwd<W256>(B, rowt, V.c, min(V.len_c, V.c + P.H), ja);
-    const bool has_b = V.c > b0 && scan_bwd<W256>(B, rowt, b0, V.c, jb);
+    bool has_a, has_b;
+    if (W256) {
+        lead_lag_w(B, rowt, V.c, min(V.len_c, V.c + P.H), b0, has_a, ja, has_b, jb);
+    } else {
+        has_a = scan_fwd<W256>(B, rowt, V.c, min(V.len_c, V.c + P.H), ja);
+        has_b = V.c > b0 && scan_bwd<W256>(B, rowt, b0, V.c, jb);
+    }
     int32_t x_a = 0, x_b = 0;
     float v_a = 0.0f, v_b = 0.0f;
     uint2 pa = make_uint2(0u, 0u), pb = pa;
@@ -736,7 +761,7 @@ __device__ __forceinline__ Hit leader_continue(const DevP &P, const u64 *B, cons
 // Deferred-list entry kinds: 0 / 1 = adjacent-lane evaluation (own-lane leader not found / found, carried in the
 // entry); 2 = look-ahead to be continued past the cached hops (budget_left, dist_next carried); 3 = walk_rows.
 template <bool W256>
-__device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, const uint4 &e,
+__device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t seg_base, const uint4 &e, const uint4 &s0v, const uint4 &s1v,
                                                 uint32_t &n_cells)
 {
     const int cur = (int)(t & 1u);
@@ -745,7 +770,11 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     const uint2 *pay = P.pay[cur];
     const uint32_t slot = e.x & 0x3FFFFFFFu, kind = e.x >> 30;
     Veh V;
-    veh_load(V, S.S0[seg_base + slot], S.S1[seg_base + slot]);
+    veh_load(V, s0v, s1v);
+    if (kind < 2u) {   // a lane change rebuilds the look-ahead cache from these route records: on their way now
+        prefetch_line(P.route + V.cursor + 1u);
+        prefetch_line(P.route + V.cursor + 4u);
+    }
     V.claim = 0u;   // a deferred vehicle cannot reach its edge end
     V.hopz = 0u;
     Lead ld;
@@ -800,6 +829,16 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             // the next chunk of this warp (requested now, needed after this one)
             uint32_t next_base = 0u;
             if (lane_id == 0u) next_base = atomicAdd(&sm.next, 32u);
+#if MANTA_PF
+            next_base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
+            if (next_base + lane_id < n) {   // its state records, requested a whole chunk ahead
+                const uint32_t at = seg_base + next_base + lane_id;
+                prefetch_line(&S.S0[at]);
+                prefetch_line(&S.S1[at]);
+                prefetch_line(&S.S2[at]);
+                prefetch_line(&S.S3[at]);
+            }
+#endif
             if (s0v.w == ID_GHOST) {   // the ghost of last step's arrival clears that vehicle's last mark
                 mark_toggle(P.bits[nxt], s0v.z);
                 S.S0[seg_base + i] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);
@@ -854,17 +893,39 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             } else if (live) {
                 // deferred: must look at the adjacent lane (kinds 0 / 1, R5), or look-ahead to be continued (2) or walked (3)
                 const uint32_t kind = searched ? (ld.found ? 1u : 0u) : (r == WIN_MORE ? 2u : 3u);
-                P.dlist[seg_base + atomicAdd(&sm.qn, 1u)] =
-                    searched ? make_uint4(i | (kind << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u)
-                             : make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
+                const uint4 e = searched ? make_uint4(i | (kind << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u)
+                                         : make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
+                const uint32_t k = atomicAdd(&sm.qn, 1u);
+#if MANTA_DQ
+                if (k < (uint32_t)MANTA_DQ) {
+                    sm.dq[k][0] = s0v;
+                    sm.dq[k][1] = s1v;
+                    sm.dq[k][2] = e;
+                } else
+#endif
+                    P.dlist[seg_base + k] = e;
             }
             __syncwarp();
+#if MANTA_PF
+            base = next_base;
+#else
             base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
+#endif
         }
         __syncthreads();   // the deferred list of this segment is complete (and visible: same block)
         DBG_STAMP(2);
         const uint32_t qn = sm.qn;
-        for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) finish_deferred<W256>(P, t, sm, seg_base, P.dlist[seg_base + k], n_cells);
+        for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) {
+#if MANTA_DQ
+            if (k < (uint32_t)MANTA_DQ) {
+                finish_deferred<W256>(P, t, sm, seg_base, sm.dq[k][2], sm.dq[k][0], sm.dq[k][1], n_cells);
+                continue;
+            }
+#endif
+            const uint4 e = P.dlist[seg_base + k];
+            const uint32_t slot = e.x & 0x3FFFFFFFu;
+            finish_deferred<W256>(P, t, sm, seg_base, e, S.S0[seg_base + slot], S.S1[seg_base + slot], n_cells);
+        }
         __syncthreads();
         DBG_STAMP(3);
         if (threadIdx.x == 0u) P.seg_xn[seg] = sm.xn;
@@ -1002,6 +1063,15 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     if (threadIdx.x == 0u) {
         gen += 1u;
         unsigned ab = 0u;
+#if MANTA_BAR == 1
+        // arrival = one release reduction (no round trip); everybody polls the arrival counter itself
+        const unsigned target = gen * gridDim.x;
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&c->bar_count) : "memory");
+        {
+            const long long t0 = clock64();
+            unsigned spins = 0u;
+            while (ld_acquire_u32(&c->bar_count) < target) {
+#else
         __threadfence();
         const unsigned prev = atomicAdd(&c->bar_count, 1u);
         if (prev + 1u == gen * gridDim.x) {
@@ -1010,6 +1080,7 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
             const long long t0 = clock64();
             unsigned spins = 0u;
             while (ld_acquire_u32(&c->bar_gen) < gen) {
+#endif
                 if ((++spins & 1023u) == 0u) {   // now and then: has another block given up, or is this taking seconds?
                     if (ld_acquire_u32(&c->abort)) {
                         ab = 1u;
@@ -1067,6 +1138,20 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
         const bool more = t + 1u < t_end;
         if (more && fuse) admit_phase<true>(P, t + 1u, sbuf_of(t));   // the longer dependent chain first
         second_phase(P, t);
+#if MANTA_PF >= 3
+        if (more) {   // the state records of this block's first chunks of step t + 1: on their way while the barrier completes
+            const StBuf &Sn = P.st[sbuf_of(t + 1u)];
+            for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
+                const uint32_t at = seg * P.seg_cap + threadIdx.x;
+                if (threadIdx.x < P.seg_cnt[seg]) {
+                    prefetch_line(&Sn.S0[at]);
+                    prefetch_line(&Sn.S1[at]);
+                    prefetch_line(&Sn.S2[at]);
+                    prefetch_line(&Sn.S3[at]);
+                }
+            }
+        }
+#endif
         DBG_STAMP(5);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(6);
