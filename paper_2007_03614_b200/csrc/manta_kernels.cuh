@@ -32,7 +32,7 @@ namespace manta {
 #define MANTA_MINB 2      // blocks per SM the step kernels are compiled for
 #endif
 #ifndef MANTA_BAR
-#define MANTA_BAR 1       // grid barrier: 1 = release reduction + polling the arrival counter, 0 = atomicAdd + generation word
+#define MANTA_BAR 1       // grid barrier: 1 = release reduction + acquire polling of the arrival counter, 0 = atomicAdd + generation word
 #endif
 #ifndef MANTA_DQ
 #define MANTA_DQ 0        // deferred-list entries a block keeps in shared memory (0: all in P.dlist)
@@ -1048,9 +1048,12 @@ __global__ void __launch_bounds__(MANTA_NT) k_sort_scatter(const DevP P, int fro
     sort_scatter(P, from, all, max(1u, (all + P.n_seg - 1u) / P.n_seg));
 }
 
-// Grid-wide barrier of the persistent kernel: arrival counter + generation word, release / acquire at gpu scope
-// (the fences also invalidate L1, so plain loads after the barrier see the other SMs' writes).  A spin that lasts
-// longer than ~4 s sets the abort flag; every block then leaves the kernel and manta_step reports the failure.
+// Grid-wide barrier of the persistent kernel.  Arrival: bar.sync, then thread 0 adds 1 to the arrival counter with
+// red.release.gpu (MEMBAR.ALL.GPU + REDG: the block's writes are performed before the count moves; no round trip).
+// Departure: thread 0 polls the counter with ld.acquire.gpu until it reaches generation x grid size (each polling
+// load is LDG.STRONG.GPU + CCTL.IVALL, so the SM's L1 holds nothing stale when the other threads are let through
+// bar.sync and read the other SMs' writes with plain loads).  The counter is never reset inside a launch.  A spin
+// that lasts longer than ~4 s sets the abort flag; every block then leaves the kernel and manta_step reports it.
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
 {
     unsigned v;
@@ -1063,7 +1066,7 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     if (threadIdx.x == 0u) {
         gen += 1u;
         unsigned ab = 0u;
-#if MANTA_BAR == 1
+#if MANTA_BAR >= 1
         // arrival = one release reduction (no round trip); everybody polls the arrival counter itself
         const unsigned target = gen * gridDim.x;
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&c->bar_count) : "memory");
@@ -1094,7 +1097,9 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
                 }
             }
         }
+#if MANTA_BAR == 0
         __threadfence();
+#endif
         *s_flag = ab;
     }
     __syncthreads();
