@@ -49,9 +49,14 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def make_workload(scale, n_threads=None, cache=True):
+CONFIGS = {2: ("configs[2] Bay-Area-shaped synthetic morning", 50400),
+           3: ("configs[3] congestion stress (lane-reduced configs[2] network, 2 x demand in 06:00-09:00)", 43200),
+           4: ("configs[4] 2 x 2 tiled configs[2] network, 4 x demand", 50400)}
+
+
+def make_workload(scale, n_threads=None, cache=True, config=2):
     from paper_2007_03614_b200 import workloads as wl
-    tag = "/tmp/manta_cfg2_%g_v3.npz" % scale
+    tag = "/tmp/manta_cfg%d_%g_v3.npz" % (config, scale)
     if cache and os.path.exists(tag):
         try:
             z = np.load(tag, allow_pickle=False)
@@ -59,10 +64,11 @@ def make_workload(scale, n_threads=None, cache=True):
             net["n_nodes"], net["n_edges"] = int(net["n_nodes"]), int(net["n_edges"])
             trips = {k[5:]: z[k] for k in z.files if k.startswith("trip_")}
             trips["init_pos_m"] = trips["init_speed"] = None
-            return net, trips, dict(lookahead_cells=256), 50400
+            return net, trips, dict(lookahead_cells=256), CONFIGS[config][1]
         except Exception:
             pass
-    net, trips, params, n_steps = wl.config2(scale=scale, n_threads=n_threads)
+    gen = {2: wl.config2, 3: wl.config3, 4: wl.config4}[config]
+    net, trips, params, n_steps = gen(scale=scale, n_threads=n_threads)
     if cache:
         try:
             keep = ("n_nodes", "n_edges", "row_ptr", "head", "length_m", "lanes", "speed_limit", "node_ctrl")
@@ -159,7 +165,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    net, trips, params, _ = make_workload(args.scale)
+    net, trips, params, _ = make_workload(args.scale, config=args.config)
     K, W = args.steps, args.warmup
     # sample sized so that W + K oracle steps end within ~2 minutes (about 1.5 us per update on one core)
     n_sample = int(min(200000, max(2000, 100.0 / ((K + W) * 1.5e-6))))
@@ -170,12 +176,12 @@ def run_reference(args):
     upd_0, wall_0, _, _ = oracle_sample(net, trips, params, args.start_step, n_sample, W) if W else (0, 0.0, 0, 0)
     upd, wall = upd_w - upd_0, max(wall_w - wall_0, 1e-9)
     val = upd / wall
-    sample = ("first %d trips departing from step %d of configs[2] (scale %g), run %d timesteps from their first "
-              "departure" % (n_tr, args.start_step, args.scale, K))
+    sample = ("first %d trips departing from step %d of configs[%d] (scale %g), run %d timesteps from their first "
+              "departure" % (n_tr, args.start_step, args.config, args.scale, K))
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
            "warmup": W, "ms_per_step": wall / K * 1e3, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": "configs[2] Bay-Area-shaped synthetic morning, scale %g" % args.scale,
+           "config": {"workload": "%s, scale %g" % (CONFIGS[args.config][0], args.scale),
                       "sample": sample, "l2": "n/a (CPU)"},
            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -205,11 +211,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scale", type=float, default=1.0, help="configs[2] size factor (1.0 = the named workload)")
-    ap.add_argument("--start-step", type=int, default=18000, help="timestep at which the timed window starts (07:30)")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4],
+                    help="BASELINE.json config: 2 = the workload the metric is quoted on (default); 3, 4 = the larger cases")
+    ap.add_argument("--start-step", type=int, default=None,
+                    help="timestep at which the timed window starts (default: 07:30 = step 18000; configs[3]: 07:00 = step 7200)")
     ap.add_argument("--flags", type=int, default=0, help="manta_params.flags (A/B switches)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
+    if args.start_step is None:
+        args.start_step = 7200 if args.config == 3 else 18000
     if args.impl == "reference":
         return run_reference(args)
 
@@ -227,7 +238,7 @@ def main():
     binding.load_library()
     K, W = args.steps, max(args.warmup, 3)
     t0 = time.time()
-    net, trips, params, n_total = make_workload(args.scale)
+    net, trips, params, n_total = make_workload(args.scale, config=args.config)
     params = dict(params, flags=args.flags)
     n_trips = len(trips["depart_time_s"])
     log("[bench] workload ready in %.1f s: %d nodes %d edges %d trips %d route entries" % (
@@ -297,9 +308,9 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
-           "config": {"workload": "configs[2] Bay-Area-shaped synthetic morning, scale %g: %d nodes, %d directed edges, "
-                                  "%d trips, dt 0.5 s" % (args.scale, net["n_nodes"], net["n_edges"], n_trips),
-                      "timed_window": "timesteps %d..%d (07:30 + %d steps of 0.5 s)" % (args.start_step + W, args.start_step + W + K, K),
+           "config": {"workload": "%s, scale %g: %d nodes, %d directed edges, %d trips, dt 0.5 s" % (
+                          CONFIGS[args.config][0], args.scale, net["n_nodes"], net["n_edges"], n_trips),
+                      "timed_window": "timesteps %d..%d (%d steps of 0.5 s)" % (args.start_step + W, args.start_step + W + K, K),
                       "parallelism": "replicas x%d" % world, "flags": args.flags,
                       "l2": "inputs larger than L2 (%.1f GB device-resident), no flush" % (dev_bytes / 1e9)},
            "clocks": clk, "gpu_launches": launches, "roofline": roofline,

@@ -417,3 +417,35 @@ def config2(scale=1.0, n_trips=None, seed=SEED_DEMAND, net=None, window=None, n_
         sel = (dep >= window[0]) & (dep < window[1])
         o, d, dep = o[sel], d[sel], dep[sel] - np.float32(window[0])
     return net, make_trips(net, o, d, dep, n_threads=n_threads, weight=weight), dict(lookahead_cells=256), 50400
+
+
+def config3(scale=1.0, seed=SEED_DEMAND + 100, window=None, n_threads=None):
+    """BASELINE.json configs[3], congestion stress: the configs[2] network with 20 % of its >= 2-lane edges reduced
+    to one lane, demand x 2 (6.4 M trips at scale 1) compressed into 06:00-09:00 (same bimodal law squeezed into
+    the three hours), same gravity OD; runs until all trips are done or 43,200 steps (6 simulated hours).
+    Times are seconds after 06:00."""
+    side = np.sqrt(scale)
+    net = reduce_lanes(bay_network(nx=max(12, int(round(492 * side))), ny=max(12, int(round(490 * side)))))
+    n_trips = int(round(6_400_000 * scale))
+    dep = depart_bimodal(n_trips, seed + 1, t_open=6 * 3600.0, t_close=9 * 3600.0,
+                         peaks=((0.55, 7.25 * 3600.0, 20 * 60.0), (0.45, 7.9 * 3600.0, 20 * 60.0)))
+    o, d = gravity_od(net, n_trips, seed, n_origins=max(64, int(16384 * scale)))
+    if window is not None:
+        sel = (dep >= window[0]) & (dep < window[1])
+        o, d, dep = o[sel], d[sel], dep[sel] - np.float32(window[0])
+    return net, make_trips(net, o, d, dep, n_threads=n_threads, weight="time"), dict(lookahead_cells=256), 43200
+
+
+def config4(scale=1.0, seed=SEED_DEMAND + 200, window=None, n_threads=None):
+    """BASELINE.json configs[4], scale-out on one GPU: 2 x 2 tiling of the configs[2] network joined by seam edges
+    (~ 900 k nodes, ~ 2.2 M directed edges at scale 1) with 12.8 M trips of the same distributions (gravity OD over
+    the whole tiled network, bimodal departures 05:00-12:00); 50,400 steps (7 simulated hours)."""
+    side = np.sqrt(scale)
+    net = tile_network(bay_network(nx=max(12, int(round(492 * side))), ny=max(12, int(round(490 * side)))), 2, 2)
+    n_trips = int(round(12_800_000 * scale))
+    dep = depart_bimodal(n_trips, seed + 1)
+    o, d = gravity_od(net, n_trips, seed, n_origins=max(64, int(65536 * scale)))
+    if window is not None:
+        sel = (dep >= window[0]) & (dep < window[1])
+        o, d, dep = o[sel], d[sel], dep[sel] - np.float32(window[0])
+    return net, make_trips(net, o, d, dep, n_threads=n_threads, weight="time"), dict(lookahead_cells=256), 50400

@@ -136,6 +136,27 @@ def test_config2_shaped_small_bit_exact(oracle_mod, binding, flags):
     assert s["n_done"] > 500 and s["lane_changes"] > 20
 
 
+@pytest.mark.parametrize("flags", [0, 2])
+def test_config3_shaped_congestion_bit_exact(oracle_mod, binding, flags):
+    """BASELINE.json configs[3] shape at 1/64 scale (20 % of the multi-lane edges cut to one lane, doubled demand
+    squeezed into three hours), the densest 20 minutes: spill-back, refused admissions, claims lost at full entry
+    windows -- every vehicle bit-exact against the oracle."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5400.0), n_threads=4)
+    assert len(trips["depart_time_s"]) > 15000
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 2400, dense_until=0, every=40, atlas_every=1200,
+                    flags=flags)
+    assert s["n_done"] > 2000 and s["lane_changes"] > 1000
+
+
+def test_config4_shaped_tiled_bit_exact(oracle_mod, binding):
+    """BASELINE.json configs[4] shape at 1/64 scale: 2 x 2 tiling of the Bay-Area-shaped network joined by seam
+    edges, trips crossing between tiles; 10 minutes of peak demand, 2,400 steps, bit-exact against the oracle."""
+    net, trips, params, _ = wl.config4(scale=1 / 64.0, window=(9000.0, 9600.0), n_threads=4)
+    assert len(trips["depart_time_s"]) > 8000 and net["n_edges"] > 30000
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 2400, dense_until=0, every=60, atlas_every=1200)
+    assert s["n_done"] > 1000
+
+
 def test_edge_cases(oracle_mod, binding):
     # a single trip on a single edge; trips that depart after the horizon; route of one edge
     net = wl.straight_road(n_edges=2, length_m=50.0, lanes=1)
