@@ -134,6 +134,13 @@ def algorithmic_bytes(hbar, flc, lookback):
     return upd, upd + 6.0
 
 
+# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01c_inplace_state.md):
+# dram__bytes_read.sum + dram__bytes_write.sum = 76.4 MB + 9.6 MB for a launch of 383,948 vehicle-updates with the
+# L2 flushed before the launch (ncu's default cache control), i.e. 224 B per update.  bench.py reports it scaled to
+# the updates per launch of its own timed window.
+NCU_TRAFFIC_BYTES_PER_UPDATE = (76.366336e6 + 9.636352e6) / 383948.0
+
+
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
     """Bounded sample of the same workload for the CPU oracle: the first n_sample_trips trips departing at or
     after start_step, their departures shifted so the earliest leaves at t = 0; run n_steps timesteps."""
@@ -298,7 +305,10 @@ def main():
     t_update = ph[1] / Kp * 1e-3
     achieved = bytes_update * upd_per_launch / t_update / 1e9
     roofline = {"bound": "hbm", "kernel": "k_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_UPDATE * upd_per_launch,
+                "traffic_source": "ncu --set full (profiles/r01c_inplace_state.md): %.0f B per update, L2 flushed; "
+                                  "scaled to this run's updates per launch" % NCU_TRAFFIC_BYTES_PER_UPDATE,
+                "peak_source": peak_src,
                 "bytes_per_update": bytes_update, "updates_per_launch": upd_per_launch,
                 "avg_launch_us": t_update * 1e6, "hbar_cells": hbar, "f_lc": flc,
                 "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp},

@@ -327,8 +327,9 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
             }
         }
     }
+    P.pay_shift = P.L_fx >= 4096 ? 2u : 0u;   // one payload entry per aligned group of four cells when L >= 4 m
     for (int k = 0; k < 2; k++)
-        if ((rc = alloc_fill(s, &P.pay[k], cells + 64, 0))) return bail(rc);
+        if ((rc = alloc_fill(s, &P.pay[k], (cells >> P.pay_shift) + 64, 0))) return bail(rc);
     P.edge_tab = d_et; P.P_mlc = d_pm; P.edge_entries = d_ee; P.claim = d_claim; P.ctr = d_ctr;
     P.blk = d_blk;
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(s, MANTA_ERR_CUDA, "upload failed: %s", cudaGetErrorString(cudaGetLastError())));
@@ -778,7 +779,7 @@ int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell
         float *d_spd = (float *)buf;
         uint16_t *d_occ = (uint16_t *)(buf + n * 4);
         k_export_atlas<<<(unsigned)std::min<uint64_t>((n + 255) / 256, 65535ull), 256, 0, s->stream>>>(
-            s->P.bits[s->t & 1u], s->P.pay[s->t & 1u], n, d_occ, d_spd);
+            s->P.bits[s->t & 1u], s->P.pay[s->t & 1u], s->P.pay_shift, n, d_occ, d_spd);
         CUDA_TRY(s, cudaGetLastError());
         if (occ) CUDA_TRY(s, cudaMemcpyAsync(occ, d_occ, n * 2, cudaMemcpyDeviceToHost, s->stream));
         if (spd) CUDA_TRY(s, cudaMemcpyAsync(spd, d_spd, n * 4, cudaMemcpyDeviceToHost, s->stream));

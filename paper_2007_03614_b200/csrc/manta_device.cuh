@@ -113,6 +113,7 @@ struct DevP {
     // atlas
     u64 *bits[2];
     uint2 *pay[2];
+    uint32_t pay_shift;          // payload entry of a cell = pay[cell >> pay_shift]: 2 (one entry per aligned group of four cells) if L >= 4 m, else 0
     // routes
     const uint4 *route;
     // vehicles: segment s occupies slots [s * seg_cap, s * seg_cap + seg_cnt[s]) (live and dead slots)
@@ -269,28 +270,13 @@ __device__ __forceinline__ void mark_move(u64 *B, uint32_t cell_old, uint32_t ce
     }
 }
 
-// Payload of the vehicle in `cell`: written as the whole aligned 32-byte sector (four cells).  Vehicles in one row
-// are at least L >= 4 m apart, so no second vehicle can be in the same aligned group of four cells at the same
-// time: the other three entries are nobody's, and a full-sector store needs no read-modify-write in L2 / DRAM.
+// Payload of the vehicle in `cell`.  Vehicles in one row are at least L apart; for L >= 4 m an aligned group of
+// four cells never holds two of them at the same time, so the plane keeps ONE 8-byte entry per group (pay_shift = 2:
+// 2 bytes per cell instead of 8; the reader knows the occupant's cell from the occupancy bit).  Shorter vehicles get
+// one entry per cell (pay_shift = 0).
 __device__ __forceinline__ void pay_store(const DevP &P, uint2 *pay, uint32_t cell, uint32_t frac, uint32_t vbits)
 {
-    if (P.L_fx < 4096) {   // vehicles shorter than 4 m: plain 8-byte entry
-        pay[cell] = make_uint2(frac, vbits);
-        return;
-    }
-    const uint32_t k = cell & 3u;
-    uint4 lo, hi;
-    lo.x = k == 0u ? frac : 0u;
-    lo.y = k == 0u ? vbits : 0u;
-    lo.z = k == 1u ? frac : 0u;
-    lo.w = k == 1u ? vbits : 0u;
-    hi.x = k == 2u ? frac : 0u;
-    hi.y = k == 2u ? vbits : 0u;
-    hi.z = k == 3u ? frac : 0u;
-    hi.w = k == 3u ? vbits : 0u;
-    uint4 *p = reinterpret_cast<uint4 *>(pay + (cell & ~3u));
-    p[0] = lo;
-    p[1] = hi;
+    pay[cell >> P.pay_shift] = make_uint2(frac, vbits);
 }
 
 // first occupied cell j in [start, end) of a row, for windows of at most 256 cells (H <= 256): the up-to-five words

@@ -254,14 +254,14 @@ __device__ __forceinline__ int leader_window(const DevP &P, const u64 *B, uint32
 }
 
 template <bool W256>
-__device__ __forceinline__ Lead lead_from_hit(const uint2 *pay, const Hit &h)
+__device__ __forceinline__ Lead lead_from_hit(const uint2 *pay, uint32_t pay_shift, const Hit &h)
 {
     Lead L;
     L.found = h.found;
     L.lead_abs = 0;
     L.v_lead = 0.0f;
     if (h.found) {
-        const uint2 pc = pay[h.cell];
+        const uint2 pc = pay[h.cell >> pay_shift];
         L.lead_abs = (int32_t)((h.dist << 10) | pc.x);
         L.v_lead = __uint_as_float(pc.y);
     }
@@ -495,8 +495,8 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
     int32_t x_a = 0, x_b = 0;
     float v_a = 0.0f, v_b = 0.0f;
     uint2 pa = make_uint2(0u, 0u), pb = pa;
-    if (has_a) pa = pay[(size_t)rowt + ja];
-    if (has_b) pb = pay[(size_t)rowt + jb];
+    if (has_a) pa = pay[(rowt + ja) >> P.pay_shift];
+    if (has_b) pb = pay[(rowt + jb) >> P.pay_shift];
     if (has_a) {
         x_a = (int32_t)((ja << 10) | pa.x);
         v_a = __uint_as_float(pa.y);
@@ -780,7 +780,7 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     Lead ld;
     if (kind >= 2u) {
         const Hit h = kind == 2u ? leader_continue(P, B, V, e.w, e.y, e.z, n_cells) : walk_rows(P, B, V, n_cells);
-        ld = lead_from_hit<W256>(pay, h);
+        ld = lead_from_hit<W256>(pay, P.pay_shift, h);
     } else {
         ld.found = kind != 0u;
         ld.lead_abs = (int32_t)e.y;
@@ -882,7 +882,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             ld.v_lead = 0.0f;
             V.need_lc = false;
             if (searched) {
-                ld = lead_from_hit<W256>(pay, h);
+                ld = lead_from_hit<W256>(pay, P.pay_shift, h);
                 pre_lc(P, t, V, ld);
             }
             __syncwarp();
@@ -1261,11 +1261,11 @@ __global__ void k_status_from_steps(uint32_t n_trips, const uint32_t *trip_of_id
     }
 }
 // Logical atlas of the current step for tests: occ = 0 / 1 + frac10, spd = occupant's speed
-__global__ void k_export_atlas(const u64 *B, const uint2 *pay, uint64_t n_cells, uint16_t *occ, float *spd)
+__global__ void k_export_atlas(const u64 *B, const uint2 *pay, uint32_t pay_shift, uint64_t n_cells, uint16_t *occ, float *spd)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_cells; i += (uint64_t)gridDim.x * blockDim.x) {
         const bool on = (B[i >> 6] >> (i & 63ull)) & 1ull;
-        const uint2 pc = on ? pay[i] : make_uint2(0u, 0u);
+        const uint2 pc = on ? pay[i >> pay_shift] : make_uint2(0u, 0u);
         occ[i] = on ? (uint16_t)(1u + pc.x) : (uint16_t)0u;
         spd[i] = on ? __uint_as_float(pc.y) : 0.0f;
     }

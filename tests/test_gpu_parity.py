@@ -258,8 +258,8 @@ def test_long_look_ahead_generic_walk(oracle_mod, binding, flags):
 
 
 def test_short_vehicles_plain_payload(oracle_mod, binding):
-    """veh_len = 3 m: two vehicles can share an aligned group of four cells, so payload entries are written one by
-    one instead of as whole sectors."""
+    """veh_len = 3 m: two vehicles can share an aligned group of four cells, so the payload plane keeps one entry
+    per cell (pay_shift = 0) instead of one per group."""
     net = wl.grid_network(nx=4, ny=4, lanes=2, ctrl=wl.PRIORITY)
     o_, d_ = wl.uniform_od(net, 600, 31)
     trips = wl.make_trips(net, o_, d_, wl.depart_uniform(600, 0.0, 120.0, 32), n_threads=2)
