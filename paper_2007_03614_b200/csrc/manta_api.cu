@@ -317,7 +317,11 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cuda_device);
         cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, cuda_device);
         s->l2_persist = 0;
-        if (!(p.flags & MANTA_FLAG_NO_L2_PIN) && max_persist > 0 && max_window > 0) {
+        // Only when both planes fit the carve-out and one window: a window larger than the carve-out leaves part of
+        // its lines on the evict-first miss policy, which costs far more than it saves (configs[4], 178 MB of planes:
+        // 400 us per step pinned, 142 us unpinned; profiles/r01d_*).
+        if (!(p.flags & MANTA_FLAG_NO_L2_PIN) && max_persist > 0 && max_window > 0 &&
+            s->l2_window_bytes <= (uint64_t)max_persist && s->l2_window_bytes <= (uint64_t)max_window) {
             const size_t want = (size_t)std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_persist);
             if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
                 s->l2_persist = want;
