@@ -134,11 +134,11 @@ def algorithmic_bytes(hbar, flc, lookback):
     return upd, upd + 6.0
 
 
-# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01c_inplace_state.md):
-# dram__bytes_read.sum + dram__bytes_write.sum = 76.4 MB + 9.6 MB for a launch of 383,948 vehicle-updates with the
-# L2 flushed before the launch (ncu's default cache control), i.e. 224 B per update.  bench.py reports it scaled to
-# the updates per launch of its own timed window.
-NCU_TRAFFIC_BYTES_PER_UPDATE = (76.366336e6 + 9.636352e6) / 383948.0
+# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01d_dense_payload.md):
+# dram__bytes_read.sum + dram__bytes_write.sum = 72.9 MB + 7.6 MB for a launch of 383,948 vehicle-updates with the
+# L2 flushed before the launch (ncu's default cache control), i.e. 210 B per update (live, application replay:
+# 145-170 B).  bench.py reports it scaled to the updates per launch of its own timed window.
+NCU_TRAFFIC_BYTES_PER_UPDATE = (72.912640e6 + 7.569152e6) / 383948.0
 
 
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
@@ -290,12 +290,22 @@ def main():
     sim = binding.Sim(net, params, trips, device=local, stream=stream)
     sim.set_multi_kernel(False)
     sim.step(args.start_step + W)
-    r0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+    # up to 1,200 of the K timesteps, in 12 slices spread evenly over the timed window (the active-vehicle count
+    # changes several-fold across it); the steps between the slices run untimed in the persistent kernel
     Kp = min(K, 1200)
-    ph = sim.step_timed(Kp)
-    r1 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+    n_sl = 12 if K >= 2400 else 1
+    per, gap = Kp // n_sl, (K - Kp) // n_sl
+    Kp = per * n_sl
+    ph, d = [0.0, 0.0, 0.0], None
+    for _ in range(n_sl):
+        r0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+        p_sl = sim.step_timed(per)
+        r1 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+        ph = [a + b for a, b in zip(ph, p_sl)]
+        d = {k: (d[k] if d else 0) + r1[k] - r0[k] for k in r0}
+        if gap:
+            sim.step(gap)
     sim.close()
-    d = {k: r1[k] - r0[k] for k in r0}
     hbar = d["cells_examined"] / max(1, d["vehicle_updates"])
     flc = d["lc_evals"] / max(1, d["vehicle_updates"])
     # algorithmic bytes per vehicle-update: whole step, and the update phase alone
@@ -306,7 +316,7 @@ def main():
     achieved = bytes_update * upd_per_launch / t_update / 1e9
     roofline = {"bound": "hbm", "kernel": "k_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_UPDATE * upd_per_launch,
-                "traffic_source": "ncu --set full (profiles/r01c_inplace_state.md): %.0f B per update, L2 flushed; "
+                "traffic_source": "ncu --set full (profiles/r01d_dense_payload.md): %.0f B per update, L2 flushed; "
                                   "scaled to this run's updates per launch" % NCU_TRAFFIC_BYTES_PER_UPDATE,
                 "peak_source": peak_src,
                 "bytes_per_update": bytes_update, "updates_per_launch": upd_per_launch,
