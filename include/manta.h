@@ -55,6 +55,9 @@ extern "C" {
 #define MANTA_FLAG_NO_L2_PIN 8u        /* do not pin the occupancy planes in L2 (A/B switch; the default sets the
                                           device's cudaLimitPersistingL2CacheSize to the size of the two planes)   */
 
+#define MANTA_FLAG_TINY_QUEUES 32u     /* test switch: a block keeps only 2 deferred-list entries in shared memory, so
+                                          that the overflow path through device memory runs in small cases       */
+
 typedef struct manta_sim manta_sim; /* opaque; owned by the library; one simulation on one device */
 
 /* Street network (per edge lanes, length in metres, free-flow speed).  Edges are numbered in

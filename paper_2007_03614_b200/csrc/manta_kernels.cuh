@@ -35,7 +35,7 @@ namespace manta {
 #define MANTA_BAR 1       // grid barrier: 1 = release reduction + acquire polling of the arrival counter, 0 = atomicAdd + generation word
 #endif
 #ifndef MANTA_DQ
-#define MANTA_DQ 0        // deferred-list entries a block keeps in shared memory (0: all in P.dlist)
+#define MANTA_DQ 256      // deferred-list entries (with their vehicle records) a block keeps in shared memory; the overflow goes to P.dlist (0: all there)
 #endif
 #ifndef MANTA_PF
 #define MANTA_PF 3        // state records requested ahead: 1 = next chunk into L2, 2 = into L1, 3 = 1 + the first chunks of step t + 1 before the grid barrier
@@ -807,6 +807,9 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
     const uint32_t lane_id = threadIdx.x & 31u;
+#if MANTA_DQ
+    const uint32_t dq_cap = (P.flags & MANTA_FLAG_TINY_QUEUES) ? 2u : (uint32_t)MANTA_DQ;
+#endif
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
         const uint32_t n = P.seg_cnt[seg];
         const uint32_t seg_base = seg * P.seg_cap;
@@ -897,7 +900,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
                                          : make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
                 const uint32_t k = atomicAdd(&sm.qn, 1u);
 #if MANTA_DQ
-                if (k < (uint32_t)MANTA_DQ) {
+                if (k < dq_cap) {
                     sm.dq[k][0] = s0v;
                     sm.dq[k][1] = s1v;
                     sm.dq[k][2] = e;
@@ -917,7 +920,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
         const uint32_t qn = sm.qn;
         for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) {
 #if MANTA_DQ
-            if (k < (uint32_t)MANTA_DQ) {
+            if (k < dq_cap) {
                 finish_deferred<W256>(P, t, sm, seg_base, sm.dq[k][2], sm.dq[k][0], sm.dq[k][1], n_cells);
                 continue;
             }

@@ -148,6 +148,16 @@ def test_config3_shaped_congestion_bit_exact(oracle_mod, binding, flags):
     assert s["n_done"] > 2000 and s["lane_changes"] > 1000
 
 
+@pytest.mark.parametrize("flags", [32, 34])
+def test_deferred_list_overflow_path(oracle_mod, binding, flags):
+    """MANTA_FLAG_TINY_QUEUES: only two deferred entries per block stay in shared memory, the rest take the path
+    through device memory (which full-size runs reach only when a block defers more than MANTA_DQ vehicles in one
+    step).  Congested configs[3]-shaped case with ~ 80 vehicles and several lane-change evaluations per block."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5100.0), n_threads=4)
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 1200, dense_until=0, every=40, flags=flags)
+    assert s["lc_evals"] > 100000
+
+
 def test_config4_shaped_tiled_bit_exact(oracle_mod, binding):
     """BASELINE.json configs[4] shape at 1/64 scale: 2 x 2 tiling of the Bay-Area-shaped network joined by seam
     edges, trips crossing between tiles; 10 minutes of peak demand, 2,400 steps, bit-exact against the oracle."""
