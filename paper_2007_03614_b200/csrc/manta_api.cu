@@ -450,10 +450,16 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     s->fuse_admit = !(s->prm.flags & MANTA_FLAG_NO_FUSE) && s->min_len_c >= s->P.L_c + 2u && s->P.Z_out <= 63u;
     {
         int occ = 0, coop = 0;
+        if (MANTA_REC_BYTES) {   // the two-stage pass keeps per-thread records in dynamic shared memory (opt-in above 48 KB)
+            CUDA_TRY(s, cudaFuncSetAttribute(k_persistent<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, MANTA_REC_BYTES));
+            CUDA_TRY(s, cudaFuncSetAttribute(k_persistent<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, MANTA_REC_BYTES));
+            CUDA_TRY(s, cudaFuncSetAttribute(k_update<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, MANTA_REC_BYTES));
+            CUDA_TRY(s, cudaFuncSetAttribute(k_update<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, MANTA_REC_BYTES));
+        }
         if (s->w256)
-            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<true>, MANTA_NT, 0));
+            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<true>, MANTA_NT, MANTA_REC_BYTES));
         else
-            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<false>, MANTA_NT, 0));
+            CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_persistent<false>, MANTA_NT, MANTA_REC_BYTES));
         CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
         s->grid_persist = (coop && occ > 0) ? std::min<int>(s->sm_count * occ, (int)s->n_blk_stats) : 0;
         s->grid_step = s->grid_persist ? s->grid_persist : std::min<int>(s->sm_count * 2, (int)s->n_blk_stats);
@@ -575,13 +581,20 @@ int step_attrs(const manta_sim *s, cudaLaunchAttribute *at, bool coop)
     return n;
 }
 extern "C++" template <class... KArgs, class... Args>
+cudaError_t launch_ks(const manta_sim *s, void (*kern)(KArgs...), int grid, int block, bool coop, size_t smem, Args... args);
+extern "C++" template <class... KArgs, class... Args>
 cudaError_t launch_k(const manta_sim *s, void (*kern)(KArgs...), int grid, int block, bool coop, Args... args)
+{
+    return launch_ks(s, kern, grid, block, coop, (size_t)0, args...);
+}
+extern "C++" template <class... KArgs, class... Args>
+cudaError_t launch_ks(const manta_sim *s, void (*kern)(KArgs...), int grid, int block, bool coop, size_t smem, Args... args)
 {
     cudaLaunchAttribute at[2];
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)block);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = s->stream;
     cfg.attrs = at;
     cfg.numAttrs = (unsigned)step_attrs(s, at, coop);
@@ -612,7 +625,7 @@ void launch_step_multi(manta_sim *s, uint32_t t, bool first, bool last, cudaEven
         s->launches += 1;
     }
     if (ev) cudaEventRecord(ev[1], s->stream);
-    launch_k(s, s->w256 ? k_update<true> : k_update<false>, s->grid_step, MANTA_NT, false, s->P, t);
+    launch_ks(s, s->w256 ? k_update<true> : k_update<false>, s->grid_step, MANTA_NT, false, (size_t)MANTA_REC_BYTES, s->P, t);
     if (ev) cudaEventRecord(ev[2], s->stream);
     const int admit_next = (!last && s->fuse_admit) ? 1 : 0;
     launch_k(s, k_second, s->grid_step, 256, false, s->P, t, admit_next);
@@ -641,7 +654,7 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
         for (uint32_t done = 0; done < n_steps;) {
             uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s->t;
             CUDA_TRY(s, cudaMemsetAsync(&s->P.ctr->bar_count, 0, 33 * sizeof(unsigned int), s->stream));   // bar_count .. bar_gen
-            CUDA_TRY(s, launch_k(s, s->w256 ? k_persistent<true> : k_persistent<false>, s->grid_persist, MANTA_NT, true, s->P, t0, m, s->fuse_admit ? 1 : 0));
+            CUDA_TRY(s, launch_ks(s, s->w256 ? k_persistent<true> : k_persistent<false>, s->grid_persist, MANTA_NT, true, (size_t)MANTA_REC_BYTES, s->P, t0, m, s->fuse_admit ? 1 : 0));
             s->launches += 1;
             s->t += m;
             done += m;

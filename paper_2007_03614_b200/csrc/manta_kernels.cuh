@@ -31,6 +31,10 @@ namespace manta {
 #ifndef MANTA_MINB
 #define MANTA_MINB 2      // blocks per SM the step kernels are compiled for
 #endif
+#ifndef MANTA_TWO_STAGE
+#define MANTA_TWO_STAGE 1  // update pass as two software-pipelined stages per chunk through shared memory (needs MANTA_REC_BYTES of dynamic shared memory)
+#endif
+#define MANTA_REC_BYTES (MANTA_TWO_STAGE ? 2 * 4 * 16 * MANTA_NT : 0)
 #ifndef MANTA_BAR
 #define MANTA_BAR 1       // grid barrier: 1 = release reduction + acquire polling of the arrival counter, 0 = atomicAdd + generation word
 #endif
@@ -797,19 +801,163 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     write_out(P, t, sm, seg_base, slot, V, O);
 }
 
+#if MANTA_TWO_STAGE
+// ---- the pass in two stages per chunk, software-pipelined per warp through shared memory (H <= 256 only) --------
+// Stage A of chunk k + 1 (state records, occupancy words, search; the leader's payload entry is requested with
+// cp.async straight into the thread's record) runs BEFORE stage B of chunk k (payload -> IDM -> integration ->
+// writes), so the payload gather of a chunk has a whole stage A to land and only the occupancy-word gather is
+// waited for.  A thread's record lives in its own shared-memory words (two buffers): no cross-thread traffic.
+#define REC(buf, f) rec[((buf) * 4 + (f)) * MANTA_NT + threadIdx.x]
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSmem &sm, uint4 *rec, int buf, const StBuf &S, const u64 *B,
+                                             const uint2 *pay, uint32_t seg_base, uint32_t n, uint32_t i, uint32_t dq_cap,
+                                             uint32_t &n_cells, uint32_t &n_upd)
+{
+    uint4 s0v = make_uint4(0u, 0u, 0u, CELL_NONE), s1v = s0v, s2v = s0v, s3v = s0v;
+    if (i < n) {
+        s0v = S.S0[seg_base + i];
+        s1v = S.S1[seg_base + i];
+        s2v = S.S2[seg_base + i];
+        s3v = S.S3[seg_base + i];
+    }
+    if (s0v.w == ID_GHOST) {   // the ghost of last step's arrival clears that vehicle's last mark
+        mark_toggle(P.bits[(t & 1u) ^ 1u], s0v.z);
+        S.S0[seg_base + i] = make_uint4(0u, 0u, CELL_NONE, CELL_NONE);
+    }
+    const bool live = s0v.w < ID_GHOST;
+    Veh V;
+    veh_load(V, s0v, s1v);
+    Hit h;
+    h.found = false;
+    h.cell = 0u;
+    h.dist = 0u;
+    uint32_t budget_left = 0u, dist_next = 0u;
+    int r = WIN_DONE;
+    if (live) {
+        n_upd += 1u;
+        const uint32_t start = V.c + 1u;
+        const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
+        r = leader_window(P, B, V.c, V.row0, start, own, V.len_c, P.H, s2v, s3v, h, budget_left, dist_next);
+        if (r == WIN_DONE) {
+            n_cells += h.found ? h.dist - V.c : P.H - budget_left;
+        } else if (!cannot_cross(P, V)) {   // rare: near the edge end and the window does not fit
+            h = r == WIN_MORE ? leader_continue(P, B, V, s3v.z, budget_left, dist_next, n_cells) : walk_rows(P, B, V, n_cells);
+            r = WIN_DONE;
+        }
+    }
+    const bool searched = live && r == WIN_DONE;
+    if (live && !searched) {   // look-ahead to be continued (2) or walked (3) by the deferred stage
+        const uint32_t kind = r == WIN_MORE ? 2u : 3u;
+        const uint4 e = make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
+        const uint32_t k = atomicAdd(&sm.qn, 1u);
+#if MANTA_DQ
+        if (k < dq_cap) {
+            sm.dq[k][0] = s0v;
+            sm.dq[k][1] = s1v;
+            sm.dq[k][2] = e;
+        } else
+#endif
+            P.dlist[seg_base + k] = e;
+    }
+    REC(buf, 0) = s0v;
+    REC(buf, 1) = s1v;
+    REC(buf, 2) = make_uint4(s3v.z, s3v.w, h.cell, h.dist | (searched ? 1u << 30 : 0u) | ((searched && h.found) ? 1u << 31 : 0u));
+    if (searched && h.found) cp_async8(&REC(buf, 3), &pay[h.cell >> P.pay_shift]);
+    cp_async_commit();
+}
+
+__device__ __forceinline__ void stage_finish(const DevP &P, uint32_t t, UpdateSmem &sm, uint4 *rec, int buf, uint32_t seg_base, uint32_t i,
+                                             uint32_t dq_cap)
+{
+    const uint4 m = REC(buf, 2);
+    const bool searched = (m.w >> 30) & 1u;
+    const uint4 s0v = REC(buf, 0), s1v = REC(buf, 1);
+    Veh V;
+    veh_load(V, s0v, s1v);
+    V.hopz = m.x;
+    V.claim = m.y;
+    Lead ld;
+    ld.found = (m.w >> 31) != 0u;
+    ld.lead_abs = 0;
+    ld.v_lead = 0.0f;
+    V.need_lc = false;
+    if (searched) {
+        if (ld.found) {
+            const uint2 pc = *reinterpret_cast<const uint2 *>(&REC(buf, 3));
+            ld.lead_abs = (int32_t)(((m.w & 0x3FFFFFFFu) << 10) | pc.x);
+            ld.v_lead = __uint_as_float(pc.y);
+        }
+        pre_lc(P, t, V, ld);
+    }
+    __syncwarp();
+    if (searched && !V.need_lc) {
+        const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+        write_out(P, t, sm, seg_base, i, V, O);
+    } else if (searched) {   // must look at the adjacent lane (R5): deferred, kinds 0 / 1
+        const uint4 e = make_uint4(i | ((ld.found ? 1u : 0u) << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
+        const uint32_t k = atomicAdd(&sm.qn, 1u);
+#if MANTA_DQ
+        if (k < dq_cap) {
+            sm.dq[k][0] = s0v;
+            sm.dq[k][1] = s1v;
+            sm.dq[k][2] = e;
+        } else
+#endif
+            P.dlist[seg_base + k] = e;
+    }
+    __syncwarp();
+}
+
+// the chunk loop of one segment; all warps of the block
+__device__ __forceinline__ void pass_two_stage(const DevP &P, uint32_t t, UpdateSmem &sm, uint4 *rec, const StBuf &S, const u64 *B,
+                                               const uint2 *pay, uint32_t seg_base, uint32_t n, uint32_t dq_cap, uint32_t &n_cells,
+                                               uint32_t &n_upd)
+{
+    const uint32_t lane_id = threadIdx.x & 31u;
+    uint32_t base = threadIdx.x & ~31u;
+    if (base >= n) return;
+    int buf = 0;
+    stage_search(P, t, sm, rec, buf, S, B, pay, seg_base, n, base + lane_id, dq_cap, n_cells, n_upd);
+    for (;;) {
+        uint32_t next_base = 0u;
+        if (lane_id == 0u) next_base = atomicAdd(&sm.next, 32u);
+        next_base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
+        const bool more = next_base < n;
+        if (more) {
+            stage_search(P, t, sm, rec, buf ^ 1, S, B, pay, seg_base, n, next_base + lane_id, dq_cap, n_cells, n_upd);
+            cp_async_wait<1>();   // everything but the group just committed: this chunk's payload entries are in
+        } else {
+            cp_async_wait<0>();
+        }
+        __syncwarp();
+        stage_finish(P, t, sm, rec, buf, seg_base, base + lane_id, dq_cap);
+        if (!more) break;
+        base = next_base;
+        buf ^= 1;
+    }
+}
+#undef REC
+#endif
+
 // Must be called by ALL threads of the block (contains __syncthreads).  Warps take chunks of 32 slots from a
 // shared counter, so a warp that met slow vehicles simply takes fewer chunks.
 template <bool W256>
-__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd)
+__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd, uint4 *rec = nullptr)
 {
     const int cur = (int)(t & 1u), nxt = cur ^ 1;
     const StBuf &S = P.st[sbuf_of(t)];
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
     const uint32_t lane_id = threadIdx.x & 31u;
-#if MANTA_DQ
-    const uint32_t dq_cap = (P.flags & MANTA_FLAG_TINY_QUEUES) ? 2u : (uint32_t)MANTA_DQ;
-#endif
+    const uint32_t dq_cap = MANTA_DQ ? ((P.flags & MANTA_FLAG_TINY_QUEUES) ? 2u : (uint32_t)MANTA_DQ) : 0u;
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
         const uint32_t n = P.seg_cnt[seg];
         const uint32_t seg_base = seg * P.seg_cap;
@@ -820,6 +968,11 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
         }
         DBG_STAMP(1);
         __syncthreads();
+#if MANTA_TWO_STAGE
+        if (W256) {
+            pass_two_stage(P, t, sm, rec, S, B, pay, seg_base, n, dq_cap, n_cells, n_upd);
+        } else
+#endif
         for (uint32_t base = threadIdx.x & ~31u; base < n;) {
             const uint32_t i = base + lane_id;
             uint4 s0v = make_uint4(0u, 0u, 0u, CELL_NONE), s1v = s0v, s2v = s0v, s3v = s0v;
@@ -1005,6 +1158,7 @@ __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint3
 }
 
 // ------------------------------------------------------------------------------------------------ kernels
+extern __shared__ uint4 dyn_rec[];   // MANTA_REC_BYTES: per-thread records of the two-stage pass (k_update, k_persistent)
 __global__ void __launch_bounds__(256) k_admit(const DevP P, uint32_t t)
 {
     admit_phase<false>(P, t, sbuf_of(t));
@@ -1017,7 +1171,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, u
     if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
     __syncthreads();
     uint32_t n_cells = 0u, n_upd = 0u;
-    update_phase<W256>(P, t, sm, n_cells, n_upd);
+    update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec);
     flush_stats(P, sm, n_cells, n_upd);
 }
 
@@ -1140,7 +1294,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
     if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     for (uint32_t t = t0; t < t_end; t++) {
         DBG_STAMP(0);
-        update_phase<W256>(P, t, sm, n_cells, n_upd);
+        update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(4);
         const bool more = t + 1u < t_end;
