@@ -34,7 +34,7 @@ namespace manta {
 #ifndef MANTA_TWO_STAGE
 #define MANTA_TWO_STAGE 1  // update pass as two software-pipelined stages per chunk through shared memory (needs MANTA_REC_BYTES of dynamic shared memory)
 #endif
-#define MANTA_REC_BYTES (MANTA_TWO_STAGE ? 2 * 4 * 16 * MANTA_NT : 0)
+#define MANTA_REC_BYTES (MANTA_TWO_STAGE ? 2 * 3 * 16 * MANTA_NT : 0)   // two buffers of three uint4 per thread
 #ifndef MANTA_BAR
 #define MANTA_BAR 1       // grid barrier: 1 = release reduction + acquire polling of the arrival counter, 0 = atomicAdd + generation word
 #endif
@@ -807,7 +807,7 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
 // cp.async straight into the thread's record) runs BEFORE stage B of chunk k (payload -> IDM -> integration ->
 // writes), so the payload gather of a chunk has a whole stage A to land and only the occupancy-word gather is
 // waited for.  A thread's record lives in its own shared-memory words (two buffers): no cross-thread traffic.
-#define REC(buf, f) rec[((buf) * 4 + (f)) * MANTA_NT + threadIdx.x]
+#define REC(buf, f) rec[((buf) * 3 + (f)) * MANTA_NT + threadIdx.x]   // per thread and buffer: S0 | S1 | {dist + flags, -, payload}
 __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -869,8 +869,8 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
     }
     REC(buf, 0) = s0v;
     REC(buf, 1) = s1v;
-    REC(buf, 2) = make_uint4(s3v.z, s3v.w, h.cell, h.dist | (searched ? 1u << 30 : 0u) | ((searched && h.found) ? 1u << 31 : 0u));
-    if (searched && h.found) cp_async8(&REC(buf, 3), &pay[h.cell >> P.pay_shift]);
+    REC(buf, 2).x = h.dist | (searched ? 1u << 30 : 0u) | ((searched && h.found) ? 1u << 31 : 0u);
+    if (searched && h.found) cp_async8(&REC(buf, 2).z, &pay[h.cell >> P.pay_shift]);
     cp_async_commit();
 }
 
@@ -878,28 +878,32 @@ __device__ __forceinline__ void stage_finish(const DevP &P, uint32_t t, UpdateSm
                                              uint32_t dq_cap)
 {
     const uint4 m = REC(buf, 2);
-    const bool searched = (m.w >> 30) & 1u;
+    const bool searched = (m.x >> 30) & 1u;
     const uint4 s0v = REC(buf, 0), s1v = REC(buf, 1);
     Veh V;
     veh_load(V, s0v, s1v);
-    V.hopz = m.x;
-    V.claim = m.y;
+    V.hopz = 0u;
+    V.claim = 0u;
     Lead ld;
-    ld.found = (m.w >> 31) != 0u;
+    ld.found = (m.x >> 31) != 0u;
     ld.lead_abs = 0;
     ld.v_lead = 0.0f;
     V.need_lc = false;
     if (searched) {
         if (ld.found) {
-            const uint2 pc = *reinterpret_cast<const uint2 *>(&REC(buf, 3));
-            ld.lead_abs = (int32_t)(((m.w & 0x3FFFFFFFu) << 10) | pc.x);
-            ld.v_lead = __uint_as_float(pc.y);
+            ld.lead_abs = (int32_t)(((m.x & 0x3FFFFFFFu) << 10) | m.z);
+            ld.v_lead = __uint_as_float(m.w);
         }
         pre_lc(P, t, V, ld);
     }
     __syncwarp();
     if (searched && !V.need_lc) {
         const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
+        if (O.kind == KIND_CAND) {   // edge-end candidates (~2 %) need the claim word and node id of S3 again
+            const uint4 s3v = P.st[sbuf_of(t)].S3[seg_base + i];
+            V.hopz = s3v.z;
+            V.claim = s3v.w;
+        }
         write_out(P, t, sm, seg_base, i, V, O);
     } else if (searched) {   // must look at the adjacent lane (R5): deferred, kinds 0 / 1
         const uint4 e = make_uint4(i | ((ld.found ? 1u : 0u) << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
