@@ -134,11 +134,11 @@ def algorithmic_bytes(hbar, flc, lookback):
     return upd, upd + 6.0
 
 
-# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01d_dense_payload.md):
-# dram__bytes_read.sum + dram__bytes_write.sum = 72.9 MB + 7.6 MB for a launch of 383,948 vehicle-updates with the
-# L2 flushed before the launch (ncu's default cache control), i.e. 210 B per update (live, application replay:
-# 145-170 B).  bench.py reports it scaled to the updates per launch of its own timed window.
-NCU_TRAFFIC_BYTES_PER_UPDATE = (72.912640e6 + 7.569152e6) / 383948.0
+# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01e_two_stage.md):
+# dram__bytes_read.sum + dram__bytes_write.sum = 72.7 MB + 6.7 MB for a launch of 383,948 vehicle-updates with the
+# L2 flushed before the launch (ncu's default cache control), i.e. 207 B per update (live, application replay:
+# 135-165 B).  bench.py reports it scaled to the updates per launch of its own timed window.
+NCU_TRAFFIC_BYTES_PER_UPDATE = (72.678656e6 + 6.671360e6) / 383948.0
 
 
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
@@ -316,7 +316,7 @@ def main():
     achieved = bytes_update * upd_per_launch / t_update / 1e9
     roofline = {"bound": "hbm", "kernel": "k_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_UPDATE * upd_per_launch,
-                "traffic_source": "ncu --set full (profiles/r01d_dense_payload.md): %.0f B per update, L2 flushed; "
+                "traffic_source": "ncu --set full (profiles/r01e_two_stage.md): %.0f B per update, L2 flushed; "
                                   "scaled to this run's updates per launch" % NCU_TRAFFIC_BYTES_PER_UPDATE,
                 "peak_source": peak_src,
                 "bytes_per_update": bytes_update, "updates_per_launch": upd_per_launch,

@@ -807,7 +807,7 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
 // cp.async straight into the thread's record) runs BEFORE stage B of chunk k (payload -> IDM -> integration ->
 // writes), so the payload gather of a chunk has a whole stage A to land and only the occupancy-word gather is
 // waited for.  A thread's record lives in its own shared-memory words (two buffers): no cross-thread traffic.
-#define REC(buf, f) rec[((buf) * 3 + (f)) * MANTA_NT + threadIdx.x]   // per thread and buffer: S0 | S1 | {dist + flags, -, payload}
+#define REC(buf, f) rec[((buf) * 3 + (f)) * MANTA_NT + threadIdx.x]   // per thread and buffer: S0 | S1 | {dist + flags, claim word, payload}
 __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -870,6 +870,7 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
     REC(buf, 0) = s0v;
     REC(buf, 1) = s1v;
     REC(buf, 2).x = h.dist | (searched ? 1u << 30 : 0u) | ((searched && h.found) ? 1u << 31 : 0u);
+    REC(buf, 2).y = s3v.w;   // claim word of R8
     if (searched && h.found) cp_async8(&REC(buf, 2).z, &pay[h.cell >> P.pay_shift]);
     cp_async_commit();
 }
@@ -883,7 +884,7 @@ __device__ __forceinline__ void stage_finish(const DevP &P, uint32_t t, UpdateSm
     Veh V;
     veh_load(V, s0v, s1v);
     V.hopz = 0u;
-    V.claim = 0u;
+    V.claim = m.y;
     Lead ld;
     ld.found = (m.x >> 31) != 0u;
     ld.lead_abs = 0;
@@ -899,11 +900,8 @@ __device__ __forceinline__ void stage_finish(const DevP &P, uint32_t t, UpdateSm
     __syncwarp();
     if (searched && !V.need_lc) {
         const Outcome O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
-        if (O.kind == KIND_CAND) {   // edge-end candidates (~2 %) need the claim word and node id of S3 again
-            const uint4 s3v = P.st[sbuf_of(t)].S3[seg_base + i];
-            V.hopz = s3v.z;
-            V.claim = s3v.w;
-        }
+        if (O.kind == KIND_CAND && GEOM_PRIO(V.geom))   // behind a PRIORITY node the claim word is the node: its id is in S3.z
+            V.hopz = P.st[sbuf_of(t)].S3[seg_base + i].z;
         write_out(P, t, sm, seg_base, i, V, O);
     } else if (searched) {   // must look at the adjacent lane (R5): deferred, kinds 0 / 1
         const uint4 e = make_uint4(i | ((ld.found ? 1u : 0u) << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
