@@ -1074,15 +1074,21 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
         DBG_STAMP(2);
         const uint32_t qn = sm.qn;
         for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) {
+            uint4 e, a0, a1;   // one call site: finish_deferred is ~2 k instructions
 #if MANTA_DQ
             if (k < dq_cap) {
-                finish_deferred<W256>(P, t, sm, seg_base, sm.dq[k][2], sm.dq[k][0], sm.dq[k][1], n_cells);
-                continue;
-            }
+                e = sm.dq[k][2];
+                a0 = sm.dq[k][0];
+                a1 = sm.dq[k][1];
+            } else
 #endif
-            const uint4 e = P.dlist[seg_base + k];
-            const uint32_t slot = e.x & 0x3FFFFFFFu;
-            finish_deferred<W256>(P, t, sm, seg_base, e, S.S0[seg_base + slot], S.S1[seg_base + slot], n_cells);
+            {
+                e = P.dlist[seg_base + k];
+                const uint32_t slot = e.x & 0x3FFFFFFFu;
+                a0 = S.S0[seg_base + slot];
+                a1 = S.S1[seg_base + slot];
+            }
+            finish_deferred<W256>(P, t, sm, seg_base, e, a0, a1, n_cells);
         }
         __syncthreads();
         DBG_STAMP(3);
