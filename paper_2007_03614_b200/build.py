@@ -16,7 +16,7 @@ DEPS = SOURCES + [os.path.join(CSRC, "manta_kernels.cuh"), os.path.join(CSRC, "m
                   os.path.join(_ROOT, "include", "manta.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
-              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "-Xptxas", "-v"]
 
 
 def nvcc():

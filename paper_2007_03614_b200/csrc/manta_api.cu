@@ -12,6 +12,7 @@
 #include <cstring>
 #include <numeric>
 #include <string>
+#include <thread>
 #include <vector>
 
 using namespace manta;
@@ -352,21 +353,52 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint64_t total = route_ptr[n_trips];
     if (route_ptr[0] != 0 || total >= 0xFFFFFFFFull) return fail(s, MANTA_ERR_BAD_ROUTE, "route_ptr must start at 0 and stay below 2^32 entries");
-    // ---- validation (BAD_ROUTE)
-    double max_init = 0.0;
-    for (uint32_t i = 0; i < n_trips; i++) {
-        const uint64_t b = route_ptr[i], e = route_ptr[i + 1];
-        if (e <= b || e > total) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: empty route", i);
-        for (uint64_t k = b; k < e; k++) {
-            if (route_edges[k] >= s->n_edges) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: edge id out of range", i);
-            if (k > b && s->head[route_edges[k - 1]] != s->tail[route_edges[k]])
-                return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: route not connected at position %llu", i, (unsigned long long)(k - b));
+    // ---- validation (BAD_ROUTE): every route entry is looked at once; split over host threads for large inputs, the
+    // error reported is that of the lowest trip index, as a sequential scan would report it
+    struct Bad { uint32_t trip; int kind; uint64_t pos; };   // kind 0: none
+    auto scan = [&](uint32_t i0, uint32_t i1, Bad &bad, double &max_init) {
+        for (uint32_t i = i0; i < i1; i++) {
+            const uint64_t b = route_ptr[i], e = route_ptr[i + 1];
+            if (e <= b || e > total) { bad = {i, 1, 0}; return; }
+            for (uint64_t k = b; k < e; k++) {
+                if (route_edges[k] >= s->n_edges) { bad = {i, 2, k - b}; return; }
+                if (k > b && s->head[route_edges[k - 1]] != s->tail[route_edges[k]]) { bad = {i, 3, k - b}; return; }
+            }
+            const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
+            if (!pre && !(depart_time_s[i] >= 0.0f)) { bad = {i, 4, 0}; return; }
+            if (init_speed) {
+                if (!(init_speed[i] >= 0.0f) || !std::isfinite(init_speed[i])) { bad = {i, 5, 0}; return; }
+                if (pre) max_init = std::max(max_init, (double)init_speed[i]);
+            }
         }
-        const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
-        if (!pre && !(depart_time_s[i] >= 0.0f)) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: negative departure time", i);
-        if (init_speed) {
-            if (!(init_speed[i] >= 0.0f) || !std::isfinite(init_speed[i])) return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: bad init_speed", i);
-            if (pre) max_init = std::max(max_init, (double)init_speed[i]);
+    };
+    double max_init = 0.0;
+    {
+        const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+        const unsigned nt = total < (1ull << 20) ? 1u : std::min(hw, 32u);
+        std::vector<Bad> bad(nt, Bad{0u, 0, 0});
+        std::vector<double> mx(nt, 0.0);
+        if (nt == 1u) {
+            scan(0u, n_trips, bad[0], mx[0]);
+        } else {
+            std::vector<std::thread> th;
+            for (unsigned w = 0; w < nt; w++) {
+                const uint32_t i0 = (uint32_t)((uint64_t)n_trips * w / nt), i1 = (uint32_t)((uint64_t)n_trips * (w + 1) / nt);
+                th.emplace_back([&, w, i0, i1] { scan(i0, i1, bad[w], mx[w]); });
+            }
+            for (auto &t : th) t.join();
+        }
+        for (unsigned w = 0; w < nt; w++) {   // ranges are in trip order: the first bad one is the lowest trip index
+            const Bad &b = bad[w];
+            switch (b.kind) {
+            case 0: break;
+            case 1: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: empty route", b.trip);
+            case 2: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: edge id out of range", b.trip);
+            case 3: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: route not connected at position %llu", b.trip, (unsigned long long)b.pos);
+            case 4: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: negative departure time", b.trip);
+            default: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: bad init_speed", b.trip);
+            }
+            max_init = std::max(max_init, mx[w]);
         }
     }
     const DevP saved = s->P;
@@ -385,8 +417,18 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         if (!pre && ds >= 4294967295.0) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: departure too late", i));
         dstep[i] = pre ? 0u : (uint32_t)ds;
     }
-    std::iota(trip_of_id.begin(), trip_of_id.end(), 0u);
-    std::stable_sort(trip_of_id.begin(), trip_of_id.end(), [&](uint32_t x, uint32_t y) { return dstep[x] < dstep[y]; });
+    {
+        const uint32_t max_step = *std::max_element(dstep.begin(), dstep.end());
+        if (max_step < (1u << 24)) {   // counting sort by departure step, trip order kept inside a step (stable)
+            std::vector<uint32_t> start((size_t)max_step + 2, 0u);
+            for (uint32_t i = 0; i < n_trips; i++) start[dstep[i] + 1u]++;
+            for (uint32_t v = 0; v <= max_step; v++) start[v + 1u] += start[v];
+            for (uint32_t i = 0; i < n_trips; i++) trip_of_id[start[dstep[i]]++] = i;
+        } else {
+            std::iota(trip_of_id.begin(), trip_of_id.end(), 0u);
+            std::stable_sort(trip_of_id.begin(), trip_of_id.end(), [&](uint32_t x, uint32_t y) { return dstep[x] < dstep[y]; });
+        }
+    }
     std::vector<uint32_t> depart_by_id(n_trips), route_start(n_trips);
     for (uint32_t id = 0; id < n_trips; id++) {
         depart_by_id[id] = dstep[trip_of_id[id]];

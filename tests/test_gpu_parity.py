@@ -211,6 +211,38 @@ def test_error_codes(binding):
     assert e.value.code == binding.ERR_INVALID_ARG
 
 
+def test_large_input_validation_reports_first_bad_trip(binding):
+    """manta_load_trips validates large inputs on several host threads: the error reported is still that of the
+    lowest bad trip index, and the same input without the defects loads and runs; vehicle ids (counting sort by
+    departure step, trip order inside a step) give the same admissions as a small hand-checked case."""
+    net = wl.straight_road(n_edges=4, length_m=60.0)
+    n = 400_000                                                  # 1.6 M route entries: the threaded path
+    rp = (np.arange(n + 1, dtype=np.uint64) * np.uint64(4))
+    re_ = np.tile(np.arange(4, dtype=np.uint32), n)
+    dep = (np.arange(n, dtype=np.float32) % 977) * 3.0
+    good = dict(route_ptr=rp, route_edges=re_, depart_time_s=dep, init_pos_m=None, init_speed=None)
+    bad_edges = re_.copy()
+    bad_edges[4 * 350_000 + 2] = 0                               # not connected (later trip)
+    bad_edges[4 * 120_000 + 1] = 9                               # edge id out of range (earlier trip: reported)
+    s = binding.Sim(net)
+    with pytest.raises(binding.MantaError) as e:
+        s.load_trips(dict(good, route_edges=bad_edges))
+    assert e.value.code == binding.ERR_BAD_ROUTE and "trip 120000" in str(e.value)
+    bad_dep = dep.copy()
+    bad_dep[399_999] = -1.0
+    with pytest.raises(binding.MantaError) as e:
+        s.load_trips(dict(good, depart_time_s=bad_dep))
+    assert e.value.code == binding.ERR_BAD_ROUTE and "trip 399999" in str(e.value)
+    s.load_trips(good)
+    s.step(40)
+    out = s.readback()
+    # one single-lane origin edge: one admission per step at most, in (departure step, trip index) order
+    adm = np.nonzero(out["status"] != 0)[0]
+    first = np.lexsort((np.arange(n), np.floor(dep / 0.5)))[:len(adm)]
+    assert len(adm) > 3 and np.array_equal(np.sort(adm), np.sort(first))
+    s.close()
+
+
 # ---------------------------------------------------------------------------------------------------------
 # Paths of the look-ahead that the configs above rarely take: windows that run past the four route edges cached
 # in the vehicle state (a run of short edges), windows of more than eight occupancy words, H > 256 (generic
