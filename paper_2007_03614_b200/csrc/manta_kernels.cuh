@@ -36,7 +36,7 @@ namespace manta {
 #endif
 #define MANTA_REC_BYTES (MANTA_TWO_STAGE ? 2 * 3 * 16 * MANTA_NT : 0)   // two buffers of three uint4 per thread
 #ifndef MANTA_BAR
-#define MANTA_BAR 1       // grid barrier: 1 = release reduction + acquire polling of the arrival counter, 0 = atomicAdd + generation word
+#define MANTA_BAR 3       // grid barrier: 3 = release reduction + relaxed polling of the arrival counter + one acquire load, 1 = acquire polling, 0 = atomicAdd + generation word + fences
 #endif
 #ifndef MANTA_DQ
 #define MANTA_DQ 256      // deferred-list entries (with their vehicle records) a block keeps in shared memory; the overflow goes to P.dlist (0: all there)
@@ -1215,14 +1215,21 @@ __global__ void __launch_bounds__(MANTA_NT) k_sort_scatter(const DevP P, int fro
 
 // Grid-wide barrier of the persistent kernel.  Arrival: bar.sync, then thread 0 adds 1 to the arrival counter with
 // red.release.gpu (MEMBAR.ALL.GPU + REDG: the block's writes are performed before the count moves; no round trip).
-// Departure: thread 0 polls the counter with ld.acquire.gpu until it reaches generation x grid size (each polling
-// load is LDG.STRONG.GPU + CCTL.IVALL, so the SM's L1 holds nothing stale when the other threads are let through
-// bar.sync and read the other SMs' writes with plain loads).  The counter is never reset inside a launch.  A spin
+// Departure: thread 0 polls the counter with ld.relaxed.gpu until it reaches generation x grid size, then reads it
+// once more with ld.acquire.gpu (LDG.STRONG.GPU + CCTL.IVALL: it observes a value at the end of the chain of
+// release reductions, so it synchronises with every arrival, and the SM's L1 holds nothing stale when the other
+// threads are let through bar.sync and read the other SMs' writes with plain loads).  The counter is never reset inside a launch.  A spin
 // that lasts longer than ~4 s sets the abort flag; every block then leaves the kernel and manta_step reports it.
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
 {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned *p)
+{
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_t *s_flag)
@@ -1238,7 +1245,11 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
         {
             const long long t0 = clock64();
             unsigned spins = 0u;
+#if MANTA_BAR == 3
+            while (ld_relaxed_u32(&c->bar_count) < target) {
+#else
             while (ld_acquire_u32(&c->bar_count) < target) {
+#endif
 #else
         __threadfence();
         const unsigned prev = atomicAdd(&c->bar_count, 1u);
@@ -1264,6 +1275,8 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
         }
 #if MANTA_BAR == 0
         __threadfence();
+#elif MANTA_BAR == 3
+        (void)ld_acquire_u32(&c->bar_count);   // the acquire (and the L1 invalidation) once, after the relaxed polling
 #endif
         *s_flag = ab;
     }
