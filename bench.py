@@ -6,7 +6,7 @@ Workload: BASELINE.json configs[2], the Bay-Area-shaped synthetic morning (DESIG
 the whole hot path (admission, look-ahead, IDM, lane change, integration, edge transfer, atlas write, compaction)
 over all active vehicles.  The simulation is first advanced (untimed: initialisation) to --start-step (default
 18,000 = 07:30, the start of the peak hour), then W warm-up steps, then exactly K timed steps (default 7,200 =
-07:30-08:30).  Inputs are resident in HBM when the timed region starts; the working set (1.8 GB of atlas planes,
+07:30-08:30).  Inputs are resident in HBM when the timed region starts; the working set (0.7 GB of atlas planes,
 3-6 GB of route records, 50-100 MB of vehicle state) exceeds the 126 MB L2, so no explicit L2 flush is needed.
 
   value      whole-job vehicle-updates/s (sum over ranks / max-over-ranks device time; ranks run independent
