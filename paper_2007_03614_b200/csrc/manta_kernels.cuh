@@ -857,6 +857,10 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
     if (live && !searched) {   // look-ahead to be continued (2) or walked (3) by the deferred stage
         const uint32_t kind = r == WIN_MORE ? 2u : 3u;
         const uint4 e = make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
+        // the deferred stage continues with RouteRecs cursor + 5 .. cursor + 8 (kind 2) or walks on from cursor + 1
+        // (kind 3): out of the route store into L2 now
+        prefetch_line(P.route + V.cursor + (kind == 2u ? 5u : 1u));
+        prefetch_line(P.route + V.cursor + (kind == 2u ? 8u : 4u));
         const uint32_t k = atomicAdd(&sm.qn, 1u);
 #if MANTA_DQ
         if (k < dq_cap) {
