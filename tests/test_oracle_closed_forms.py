@@ -160,8 +160,10 @@ def test_K5_config1_ring(oracle_mod):
         assert gaps.min() >= -1e-9
         v_mean.append(float(st["v"].mean()))
     assert (st["status"] == oracle_mod.ACTIVE).all()
-    # marginally string-unstable regime: space-mean speed stays in a band around v_e = 0.88887
-    assert 0.5 * G["v_e_ring600"] < np.mean(v_mean[4:]) < 1.5 * G["v_e_ring600"], v_mean
+    # marginally string-unstable regime (growth rate +5.6e-4 1/s): within two hours the waves stay small,
+    # so the space-mean speed stays within 2 % of the closed-form v_e = 0.88887 (and not above it: s_e(v) is convex,
+    # so a spread of gaps around the fixed mean gap lowers the mean speed)
+    assert all(0.98 * G["v_e_ring600"] < x < 1.002 * G["v_e_ring600"] for x in v_mean), v_mean
 
 
 def test_K12_textbook_idm_platoon(oracle_mod):
