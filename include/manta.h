@@ -55,6 +55,10 @@ extern "C" {
 #define MANTA_FLAG_NO_L2_PIN 8u        /* do not pin the occupancy planes in L2 (A/B switch; the default sets the
                                           device's cudaLimitPersistingL2CacheSize to the size of the two planes)   */
 
+#define MANTA_FLAG_FEW_SEGMENTS 64u    /* test switch: the vehicles are kept in TWO segments (two thread blocks per
+                                          phase) instead of one per resident block, so that small cases put thousands
+                                          of slots into one segment and run the multi-chunk software pipeline of the
+                                          update pass and the real overflow of the deferred queue                    */
 #define MANTA_FLAG_TINY_QUEUES 32u     /* test switch: a block keeps only 2 deferred-list entries in shared memory, so
                                           that the overflow path through device memory runs in small cases       */
 
@@ -161,6 +165,11 @@ uint64_t manta_atlas_cells(const manta_sim *sim);
 int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch);
 
 int manta_set_stream(manta_sim *sim, void *cuda_stream);   /* cudaStream_t; work already enqueued is not moved */
+/* Process-wide: the stream (cudaStream_t, NULL = legacy default stream) that simulations created AFTERWARDS use from
+ * manta_create on (its uploads and memsets included).  All work of a simulation and the frees of manta_destroy
+ * (after a synchronize) are ordered on its one stream; an allocator callback that hands out stream-ordered memory
+ * (PyTorch's caching allocator) must allocate for that stream. */
+int manta_set_default_stream(void *cuda_stream);
 /* Switches between the persistent kernel and kernel-per-phase stepping for the following manta_step calls
  * (on != 0: as if MANTA_FLAG_MULTI_KERNEL had been given).  Results are identical either way; profilers use it to
  * advance a simulation in one launch and then look at single phases. */

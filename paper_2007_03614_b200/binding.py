@@ -20,7 +20,8 @@ FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_timed",
-           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_multi_kernel",
+           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
+           "manta_set_multi_kernel",
            "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error")
 
@@ -64,6 +65,7 @@ FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.c_void_p)
 _lib = None
 _blocks = {}
 _cb = None
+_alloc_stream = None   # torch.cuda.Stream the library's allocations are made for (set by Sim(stream=...))
 
 
 def load_library():
@@ -87,6 +89,7 @@ def load_library():
     L.manta_atlas_cells.restype = C.c_uint64
     L.manta_readback_atlas.argtypes = [C.c_void_p] * 5
     L.manta_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    L.manta_set_default_stream.argtypes = [C.c_void_p]
     L.manta_set_multi_kernel.argtypes = [C.c_void_p, C.c_int]
     L.manta_launch_count.argtypes = [C.c_void_p]
     L.manta_launch_count.restype = C.c_uint64
@@ -107,8 +110,13 @@ def use_torch_allocator():
     L = load_library()
 
     def _alloc(nbytes, device, _ctx):
+        # the caching allocator hands out stream-ordered blocks: allocate for the stream the library works on
         try:
-            t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
+            if _alloc_stream is not None:
+                with torch.cuda.stream(_alloc_stream):
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
+            else:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
         except Exception:
             return None
         _blocks[t.data_ptr()] = t
@@ -143,15 +151,23 @@ class Sim:
         N = Network(int(net["n_nodes"]), int(net["n_edges"]), *[_ptr(a) for a in self._net_arrays])
         self.n_edges = int(net["n_edges"])
         self.h = C.c_void_p()
+        # one stream from manta_create on: uploads, kernels and the allocator's blocks are all ordered on it
+        self._stream = stream
+        self._use()
+        L.manta_set_default_stream(C.c_void_p(int(getattr(stream, "cuda_stream", stream or 0))))
         rc = L.manta_create(C.byref(N), C.byref(P), int(device), C.byref(self.h))
+        L.manta_set_default_stream(None)
         if rc != OK:
             self.h = None
             raise MantaError(rc, L.manta_last_error(None).decode())
         self.n_trips = 0
-        if stream is not None:
-            self.set_stream(stream)
         if trips is not None:
             self.load_trips(trips)
+
+    def _use(self):
+        """allocations made by the next library call are for this simulation's stream"""
+        global _alloc_stream
+        _alloc_stream = self._stream if hasattr(self._stream, "cuda_stream") else None
 
     def _check(self, rc):
         if rc != OK:
@@ -170,6 +186,7 @@ class Sim:
         ip, iv = trips.get("init_pos_m"), trips.get("init_speed")
         ip = None if ip is None else np.ascontiguousarray(ip, np.float32)
         iv = None if iv is None else np.ascontiguousarray(iv, np.float32)
+        self._use()
         self._check(load_library().manta_load_trips(self.h, len(dep), _ptr(rp), _ptr(re_), _ptr(dep), _ptr(ip), _ptr(iv)))
         self.n_trips = len(dep)
 
@@ -203,6 +220,7 @@ class Sim:
         ee = np.zeros(self.n_edges, np.uint32) if edge_entries else None
         tr = np.zeros((n, 2), np.uint32) if trips else None
         sm = Summary() if summary else None
+        self._use()
         self._check(load_library().manta_readback(self.h, None if S is None else C.byref(S), _ptr(ee), _ptr(tr),
                                                   None if sm is None else C.byref(sm)))
         if trips:
@@ -217,6 +235,7 @@ class Sim:
         n = int(load_library().manta_atlas_cells(self.h))
         occ, spd = np.zeros(n, np.uint16), np.zeros(n, np.float32)
         off, pitch = np.zeros(self.n_edges, np.uint32), np.zeros(self.n_edges, np.uint32)
+        self._use()
         self._check(load_library().manta_readback_atlas(self.h, _ptr(occ), _ptr(spd), _ptr(off), _ptr(pitch)))
         return dict(occ=occ, spd=spd, cell_off=off, pitch=pitch)
 

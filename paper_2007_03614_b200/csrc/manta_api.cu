@@ -22,6 +22,7 @@ namespace {
 manta_alloc_fn g_alloc = nullptr;
 manta_free_fn g_free = nullptr;
 void *g_alloc_ctx = nullptr;
+cudaStream_t g_default_stream = 0;   // manta_set_default_stream: stream of the simulations created afterwards
 thread_local std::string g_last_error;
 
 struct Alloc {
@@ -59,6 +60,7 @@ struct manta_sim {
     void *l2_window_base = nullptr;   // occupancy planes: L2 access-policy window of the step kernels
     uint64_t l2_window_bytes = 0;
     size_t l2_persist = 0;            // persisting L2 carve-out granted (0 = no pinning)
+    size_t l2_persist_before = 0;     // the device-wide limit found at create time; put back by manta_destroy
     uint32_t n_blk_stats = 0;
 };
 
@@ -169,7 +171,17 @@ void manta_destroy(manta_sim *sim)
     cudaSetDevice(sim->device);
     cudaStreamSynchronize(sim->stream);
     while (!sim->allocs.empty()) dev_free(sim, sim->allocs.back().p);
+    if (sim->l2_persist && sim->l2_persist_before < sim->l2_persist) {
+        cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, sim->l2_persist_before);
+        cudaGetLastError();
+    }
     delete sim;
+}
+
+int manta_set_default_stream(void *cuda_stream)
+{
+    g_default_stream = (cudaStream_t)cuda_stream;
+    return MANTA_OK;
 }
 
 int manta_set_stream(manta_sim *sim, void *cuda_stream)
@@ -211,6 +223,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     }
     manta_sim *s = new manta_sim();
     s->device = cuda_device;
+    s->stream = g_default_stream;
     s->prm = p;
     auto bail = [&](int rc) {
         std::string e = s->err;
@@ -226,6 +239,11 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     s->n_nodes = N;
     s->n_edges = M;
     if (net->row_ptr[0] != 0 || net->row_ptr[N] != M) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "row_ptr does not span the edges"));
+    // packing limits of the device records: a PRIORITY node id is kept in 28 bits (S3.z = node << 4), lane entries
+    // (e * 8 + lane) and claim-word indices (n_edges * 8 + node) are 32-bit
+    static_assert(MANTA_MAX_LANES <= 8, "lane entries are e * 8 + lane");
+    if (N >= (1u << 28) || (uint64_t)M * 8ull + (uint64_t)N >= 0xFFFFFFFFull)
+        return bail(fail(s, MANTA_ERR_BAD_NETWORK, "network too large for the 32-bit claim words (n_nodes < 2^28, 8 n_edges + n_nodes < 2^32)"));
     s->row_ptr.assign(net->row_ptr, net->row_ptr + N + 1);
     s->head.assign(net->head, net->head + M);
     s->tail.resize(M);
@@ -324,7 +342,10 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         if (!(p.flags & MANTA_FLAG_NO_L2_PIN) && max_persist > 0 && max_window > 0 &&
             s->l2_window_bytes <= (uint64_t)max_persist && s->l2_window_bytes <= (uint64_t)max_window) {
             const size_t want = (size_t)std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_persist);
-            if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
+            // cudaLimitPersistingL2CacheSize is a device-wide setting: it is raised here if needed and the value found
+            // is put back by manta_destroy (two simulations with pinned planes on one device share the carve-out)
+            cudaDeviceGetLimit(&s->l2_persist_before, cudaLimitPersistingL2CacheSize);
+            if (s->l2_persist_before >= want || cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
                 s->l2_persist = want;
                 s->l2_window_bytes = std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_window);
             } else {
@@ -505,6 +526,10 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
         s->grid_persist = (coop && occ > 0) ? std::min<int>(s->sm_count * occ, (int)s->n_blk_stats) : 0;
         s->grid_step = s->grid_persist ? s->grid_persist : std::min<int>(s->sm_count * 2, (int)s->n_blk_stats);
+        if (s->prm.flags & MANTA_FLAG_FEW_SEGMENTS) {   // test switch: two segments / two blocks
+            s->grid_step = std::min(s->grid_step, 2);
+            if (s->grid_persist) s->grid_persist = s->grid_step;
+        }
     }
     DevP &P = s->P;
     P.n_seg = (uint32_t)s->grid_step;
@@ -713,8 +738,16 @@ int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
     if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
     const uint32_t CH = 128;
-    std::vector<cudaEvent_t> ev(4 * CH);
-    for (auto &e : ev) CUDA_TRY(s, cudaEventCreate(&e));
+    struct Events {   // destroyed on every return path
+        std::vector<cudaEvent_t> ev;
+        ~Events() { for (auto e : ev) cudaEventDestroy(e); }
+    } E;
+    for (uint32_t k = 0; k < 4 * CH; k++) {
+        cudaEvent_t e;
+        CUDA_TRY(s, cudaEventCreate(&e));
+        E.ev.push_back(e);
+    }
+    std::vector<cudaEvent_t> &ev = E.ev;
     for (uint32_t done = 0; done < n_steps;) {
         const uint32_t m = std::min(CH, n_steps - done);
         for (uint32_t k = 0; k < m; k++, s->t++) launch_step_multi(s, s->t, done + k == 0, done + k + 1 == n_steps, &ev[4 * k]);
@@ -727,7 +760,6 @@ int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
             }
         done += m;
     }
-    for (auto &e : ev) cudaEventDestroy(e);
     return MANTA_OK;
 }
 

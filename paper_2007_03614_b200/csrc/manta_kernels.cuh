@@ -93,7 +93,7 @@ struct Outcome {
 
 // shared memory of the step kernels
 struct UpdateSmem {
-    uint32_t ev[4];               // event counters of this kernel: lane changes, lane-change evaluations, arrivals, travel steps
+    u64 ev[4];                    // event counters of this launch (up to 8,192 timesteps): lane changes, lane-change evaluations, arrivals, travel steps
     uint32_t xn, qn, flag, next;  // per segment: cross-list / deferred-list entries, next unclaimed chunk; barrier flag
     uint32_t wsum[MANTA_NW];      // re-sort: per-warp partial sums
 #if MANTA_DQ
@@ -457,8 +457,8 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
         if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
         if (O.kind == KIND_DONE) {
             P.arrive_step[V.id] = t + 1u;
-            atomicAdd(&sm.ev[EV_DONE], 1u);
-            atomicAdd(&sm.ev[EV_TRAVEL], t + 1u - P.admit_step[V.id]);
+            atomicAdd(&sm.ev[EV_DONE], 1ull);
+            atomicAdd(&sm.ev[EV_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
             S.S0[at] = make_uint4(0u, 0u, cur_abs, ID_GHOST);   // the ghost clears the time-t mark in the next step
         } else {
             // smallest id wins; the key carries ~t in the high word so claim words never need a reset
@@ -473,7 +473,7 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
     }
     if (geom_n != V.geom) S.S1[at] = make_uint4(row_n, geom_n, V.cursor, __float_as_uint(V.v0));
     if (changed) {   // executed lane change: the look-ahead continues in other rows now
-        atomicAdd(&sm.ev[EV_LC], 1u);
+        atomicAdd(&sm.ev[EV_LC], 1ull);
         const Hops hp = build_hops(P, V.cursor, V.geom, O.l_new);
         S.S2[at] = hp.s2;
         S.S3[at] = hp.s3;
@@ -793,7 +793,7 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     pre_lc(P, t, V, ld);
     Outcome O;
     if (V.need_lc) {
-        atomicAdd(&sm.ev[EV_EVAL], 1u);
+        atomicAdd(&sm.ev[EV_EVAL], 1ull);
         O = lane_change_and_finish<W256>(P, t, B, pay, V);
     } else {
         O = post_lc(P, t, V, false, 0, 0.0f, false, 0, 0.0f);
@@ -1162,10 +1162,10 @@ __device__ __forceinline__ void flush_stats(const DevP &P, UpdateSmem &sm, uint3
     }
     __syncthreads();
     if (threadIdx.x == 0u) {
-        if (sm.ev[EV_LC]) atomicAdd(&b->lane_changes, (u64)sm.ev[EV_LC]);
-        if (sm.ev[EV_EVAL]) atomicAdd(&b->lc_evals, (u64)sm.ev[EV_EVAL]);
-        if (sm.ev[EV_DONE]) atomicAdd(&b->n_done, (u64)sm.ev[EV_DONE]);
-        if (sm.ev[EV_TRAVEL]) atomicAdd(&b->sum_travel, (u64)sm.ev[EV_TRAVEL]);
+        if (sm.ev[EV_LC]) atomicAdd(&b->lane_changes, sm.ev[EV_LC]);
+        if (sm.ev[EV_EVAL]) atomicAdd(&b->lc_evals, sm.ev[EV_EVAL]);
+        if (sm.ev[EV_DONE]) atomicAdd(&b->n_done, sm.ev[EV_DONE]);
+        if (sm.ev[EV_TRAVEL]) atomicAdd(&b->sum_travel, sm.ev[EV_TRAVEL]);
     }
 }
 
@@ -1180,7 +1180,7 @@ template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, uint32_t t)
 {
     __shared__ UpdateSmem sm;
-    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
+    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0ull;
     __syncthreads();
     uint32_t n_cells = 0u, n_upd = 0u;
     update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec);
@@ -1309,7 +1309,7 @@ template <bool W256>
 __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP P, uint32_t t0, uint32_t n_steps, int fuse)
 {
     __shared__ UpdateSmem sm;
-    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0u;
+    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0ull;
     unsigned gen = 0u;
     uint32_t n_cells = 0u, n_upd = 0u;
     const uint32_t t_end = t0 + n_steps;

@@ -67,7 +67,7 @@ def states_equal(a, b, keys=("status", "route_pos", "lane", "tag", "x_fx", "v", 
         if x.dtype == np.float32:
             x, y = x.view(np.uint32), y.view(np.uint32)
         m = x != y
-        if k in ("route_pos", "lane", "tag", "x_fx", "v"):
+        if k in ("route_pos", "lane", "tag", "x_fx", "v", "acc"):
             m = m & (act | (b["status"] == ACTIVE))  # only meaningful while ACTIVE
         if m.any():
             bad.append((k, np.nonzero(m)[0][:8].tolist()))

@@ -1,6 +1,8 @@
 """GPU parity proper: the CUDA path (through the C ABI) against the oracle, bit for bit, on the same seeded
 inputs.  Integer state, occupancy, cell indices, edge transitions and counters must be identical; fp32 speeds are
 compared by bit pattern (deterministic mode: -fmad=false, same operation order)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -34,9 +36,10 @@ def describe(net, trips, o_st, g_st, idx):
     return "\n".join(lines)
 
 
-def compare(net, trips, o, g, label, atlas=False):
+def compare(net, trips, o, g, label, atlas=False, acc=False):
     o_st, g_out = o.state(), g.readback()
-    bad = states_equal(o_st, g_out)
+    keys = ("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step", "arrive_step")
+    bad = states_equal(o_st, g_out, keys + (("acc",) if acc else ()))
     if bad:
         idx = sorted({i for _, ii in bad for i in ii})
         raise AssertionError("%s: state mismatch %s\n%s" % (label, bad, describe(net, trips, o_st, g_out, idx)))
@@ -66,6 +69,7 @@ def run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=0, ev
     gp["flags"] = flags
     g = binding.Sim(net, gp, trips)
     L_fx = o.derived()["L_fx"]
+    acc = bool(flags & 4)      # MANTA_FLAG_RECORD_ACC: the acceleration applied in the last step, by bit pattern
     compare(net, trips, o, g, "t=0", atlas=True)
     t = 0
     while t < n_steps:
@@ -73,7 +77,8 @@ def run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=0, ev
         o.step(k)
         g.step(k)
         t += k
-        o_st, g_out = compare(net, trips, o, g, "t=%d" % t, atlas=bool(atlas_every) and (t % atlas_every == 0 or t < 4))
+        o_st, g_out = compare(net, trips, o, g, "t=%d" % t, atlas=bool(atlas_every) and (t % atlas_every == 0 or t < 4),
+                              acc=acc)
     check_no_overlap(net, trips, g_out, L_fx)
     check_conservation(g_out, len(trips["depart_time_s"]), g_out["summary"])
     check_entries(g_out, g_out["edge_entries"], trips)
@@ -333,3 +338,137 @@ def test_admission_fused_with_second_phase(oracle_mod, binding, ctrl, flags):
     s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1200, dense_until=0, every=3,
                     atlas_every=300, flags=flags)
     assert s["n_done"] > 300
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Parity at the load that bench.py times
+def test_acceleration_recorded_every_step(oracle_mod, binding):
+    """MANTA_FLAG_RECORD_ACC: the acceleration each vehicle applied in the last step (after lane change and before
+    the clamp of R7) equals the oracle's by bit pattern, every step, in both launch modes (north_star: speed AND
+    acceleration from identical state)."""
+    net = wl.grid_network(nx=4, ny=4, lanes=3, ctrl=wl.GREEN)
+    o_, d_ = wl.uniform_od(net, 700, 5)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(700, 0.0, 150.0, 6), n_threads=2)
+    for flags in (4, 6):
+        s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 900, dense_until=900, flags=flags)
+        assert s["lane_changes"] > 50
+
+
+@pytest.mark.parametrize("flags", [64, 66, 64 + 4])
+def test_few_segments_multi_chunk_pipeline(oracle_mod, binding, flags):
+    """MANTA_FLAG_FEW_SEGMENTS: all vehicles in two segments, so a segment holds thousands of slots: every warp runs
+    the `more` branch of the two-stage pass (search of chunk k + 1 before the finish of chunk k, second record
+    buffer, cp.async wait depth 1) many times per step, and a block defers more than MANTA_DQ = 256 vehicles per
+    step (the un-flagged overflow of the deferred queue into device memory).  Congested configs[3]-shaped case."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5100.0), n_threads=4)
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 1500, dense_until=0, every=50, atlas_every=500, flags=flags)
+    assert s["n_active"] + s["n_done"] > 10000 and s["lc_evals"] > 100000
+
+
+def compare_atlas_sparse(o, g, label):
+    """Logical atlas at any size: every cell the oracle has occupied holds the same (frac10, speed) on the GPU, and
+    the GPU has no other mark."""
+    oa, ga = o.atlas(), g.readback_atlas()
+    idx = np.nonzero(oa["occ"])[0].astype(np.int64)
+    row_off = oa["row_off"].astype(np.int64)
+    first_row = oa["first_row"].astype(np.int64)
+    row = np.searchsorted(row_off, idx, side="right") - 1
+    e = np.searchsorted(first_row, row, side="right") - 1
+    lane = row - first_row[e]
+    gi = ga["cell_off"][e].astype(np.int64) + lane * ga["pitch"][e].astype(np.int64) + (idx - row_off[row])
+    assert int(np.count_nonzero(ga["occ"])) == len(idx), label
+    assert np.array_equal(ga["occ"][gi].astype(np.int64), 1 + oa["frac"][idx].astype(np.int64)), label
+    assert np.array_equal(ga["spd"][gi].view(np.uint32), oa["spd"][idx].view(np.uint32)), label
+    return len(idx)
+
+
+def snapshot_parity(oracle_mod, binding, net, trips, params, checkpoints, flags=0, first=1, more=11, min_active=0):
+    """The library runs to each checkpoint on its own (one persistent launch per 8,192 steps, as bench.py times it);
+    its state is read back and injected into the oracle (Oracle.set_state: no arithmetic of the method), then both
+    advance `first` step(s) -- north_star's "single step from identical state" -- and `more` further steps in ONE
+    manta_step call (fused admission, software-pipelined pass), and every vehicle, the per-edge counts, the counters
+    and the logical atlas are compared bit for bit."""
+    gp = dict(params or {})
+    gp["flags"] = flags
+    g = binding.Sim(net, gp, trips)
+    o = oracle_mod.Oracle(net, params, trips)
+    L_fx = o.derived()["L_fx"]
+    t = 0
+    seen = []
+    delta_keys = ("vehicle_updates", "lane_changes", "cells_examined", "lc_evals")
+    for t_snap in checkpoints:
+        g.step(t_snap - t)
+        t = t_snap
+        snap = g.readback()
+        check_no_overlap(net, trips, snap, L_fx)
+        check_conservation(snap, len(trips["depart_time_s"]), snap["summary"])
+        check_entries(snap, snap["edge_entries"], trips)
+        n_act = int((snap["status"] == ACTIVE).sum())
+        assert n_act >= min_active, (t_snap, n_act)
+        o.set_state(t_snap, snap, snap["edge_entries"])
+        compare_atlas_sparse(o, g, "snapshot t=%d" % t)
+        g0, o0 = snap["summary"], o.summary()
+        for k in (first, more):
+            g.step(k)
+            o.step(k)
+            t += k
+            label = "t=%d (%d steps after the snapshot at %d, %d active)" % (t, t - t_snap, t_snap, n_act)
+            o_st, g_out = o.state(), g.readback()
+            bad = states_equal(o_st, g_out, ("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step",
+                                             "arrive_step") + (("acc",) if flags & 4 and k == first == 1 else ()))
+            if bad:
+                idx = sorted({i for _, ii in bad for i in ii})
+                raise AssertionError("%s: state mismatch %s\n%s" % (label, bad, describe(net, trips, o_st, g_out, idx)))
+            assert np.array_equal(o.edge_entries(), g_out["edge_entries"]), label
+            gs, os_ = g_out["summary"], o.summary()
+            for key in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps"):
+                assert gs[key] == os_[key], (label, key, gs, os_)
+            for key in delta_keys:
+                assert gs[key] - g0[key] == os_[key] - o0[key], (label, key, gs, os_)
+            compare_atlas_sparse(o, g, label)
+        seen.append((t_snap, n_act, gs["lane_changes"] - g0["lane_changes"], gs["lc_evals"] - g0["lc_evals"]))
+    g.close()
+    o.close()
+    return seen
+
+
+def test_parity_at_the_timed_load(oracle_mod, binding):
+    """BASELINE.json configs[2] at full size with ALL 3.2 M trips, the workload and launch configuration bench.py
+    times: snapshots at step 18,000 (07:30, ~229 k active: 770 slots per segment) and 25,200 (08:30, ~615 k active:
+    2,080 slots per segment, the multi-chunk pipeline and > 256 deferred vehicles per block), each followed by 12
+    steps compared against the oracle bit for bit."""
+    net, trips, params, _ = wl.config2(scale=1.0, n_threads=16)
+    assert len(trips["depart_time_s"]) == 3_200_000
+    seen = snapshot_parity(oracle_mod, binding, net, trips, params, (18000, 25200), min_active=150_000)
+    assert seen[0][1] > 200_000 and seen[1][1] > 550_000
+    assert all(lc > 500 and ev > 50_000 for _, _, lc, ev in seen)
+
+
+def test_whole_morning_small_scale(oracle_mod, binding):
+    """configs[2] at 1/64 scale, the whole morning 05:00-12:00 (50,400 steps): completions, the sum of travel steps,
+    per-edge entries and every trip's admit / arrive step equal the oracle's (compared every 2,400 steps)."""
+    net, trips, params, n_steps = wl.config2(scale=1 / 64.0, n_threads=8)
+    assert n_steps == 50400 and len(trips["depart_time_s"]) == 50000
+    s, n_launch = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=0, every=2400)
+    assert s["n_done"] == 50000 and s["n_active"] == 0 and n_launch == 21
+
+
+BIG = pytest.mark.skipif(os.environ.get("MANTA_BIG_PARITY") != "1",
+                         reason="needs ~40 GB of host memory and ~10 min: run with MANTA_BIG_PARITY=1 "
+                                "(log summarised in profiles/r02_parity_at_load.md)")
+
+
+@BIG
+def test_parity_at_load_config3_peak(oracle_mod, binding):
+    """configs[3] (lane-reduced network, 6.4 M trips in 06:00-09:00) at its peak, ~1.7 M active vehicles."""
+    net, trips, params, _ = wl.config3(scale=1.0, n_threads=16)
+    seen = snapshot_parity(oracle_mod, binding, net, trips, params, (10800,), more=5, min_active=1_000_000)
+    print("configs[3]", seen)
+
+
+@BIG
+def test_parity_at_load_config4_peak(oracle_mod, binding):
+    """configs[4] (2 x 2 tiled network, 12.8 M trips) at 08:30, ~2.2 M active vehicles."""
+    net, trips, params, _ = wl.config4(scale=1.0, n_threads=16)
+    seen = snapshot_parity(oracle_mod, binding, net, trips, params, (25200,), more=5, min_active=1_500_000)
+    print("configs[4]", seen)
