@@ -695,7 +695,7 @@ void launch_step_multi(manta_sim *s, uint32_t t, bool first, bool last, cudaEven
     launch_ks(s, s->w256 ? k_update<true> : k_update<false>, s->grid_step, MANTA_NT, false, (size_t)MANTA_REC_BYTES, s->P, t);
     if (ev) cudaEventRecord(ev[2], s->stream);
     const int admit_next = (!last && s->fuse_admit) ? 1 : 0;
-    launch_k(s, k_second, s->grid_step, 256, false, s->P, t, admit_next);
+    launch_k(s, s->w256 ? k_second<true> : k_second<false>, s->grid_step, MANTA_NT, false, s->P, t, admit_next);
     s->launches += 2;
     if (!last) {
         if (sort_due_host(t + 1u)) launch_sort(s, t + 1u);

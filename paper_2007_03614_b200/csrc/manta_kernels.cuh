@@ -739,6 +739,11 @@ __device__ __forceinline__ bool sort_due(uint32_t t) { return t != 0u && t % MAN
 // A vehicle further than Z_out cells from its edge end cannot reach it in this step (R0: Z_out > vcap dt), so it
 // can be neither an edge-end candidate nor an arrival, whatever its leader.  (R4 allows lane changes only there.)
 __device__ __forceinline__ bool cannot_cross(const DevP &P, const Veh &V) { return V.c + P.Z_out < V.len_c; }
+// A vehicle may be handed to the deferred stage -- which runs in the same phase as the claim resolution of this step and
+// the (fused) admission of the next -- only if nothing it does can matter there: it cannot reach its edge end (no
+// claim), and its time-(t+1) mark cannot fall into an entry window [0, L_c] that admission is testing (vehicles do
+// not move backwards, so c > L_c is enough; lane changes start at c >= Z_in > L_c anyway).
+__device__ __forceinline__ bool may_defer(const DevP &P, const Veh &V) { return cannot_cross(P, V) && V.c > P.L_c; }
 
 // Look-ahead past the four cached hops (rare: a run of short edges): the cache the vehicle would have four route
 // edges further on is rebuilt from the route store and searched the same way, until the budget of H cells is used
@@ -801,6 +806,30 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     write_out(P, t, sm, seg_base, slot, V, O);
 }
 
+// Puts the vehicle of slot i on the deferred list of its block.  Its time-(t-1) mark is toggled off HERE, in the pass:
+// that mark may lie in an entry window the fused admission reads while the deferred stage runs (the time-(t+1) mark
+// cannot: may_defer), so the deferred stage must only ever set marks beyond the windows.
+__device__ __forceinline__ void defer_entry(const DevP &P, uint32_t t, UpdateSmem &sm, const StBuf &S, uint32_t seg_base, uint32_t i,
+                                            uint32_t dq_cap, uint4 s0v, const uint4 &s1v, const uint4 &e)
+{
+    if (s0v.z != CELL_NONE) {
+        mark_toggle(P.bits[(t & 1u) ^ 1u], s0v.z);
+        s0v.z = CELL_NONE;
+    }
+    const uint32_t k = atomicAdd(&sm.qn, 1u);
+#if MANTA_DQ
+    if (k < dq_cap) {
+        sm.dq[k][0] = s0v;
+        sm.dq[k][1] = s1v;
+        sm.dq[k][2] = e;
+    } else
+#endif
+    {
+        P.dlist[seg_base + k] = e;
+        reinterpret_cast<uint32_t *>(&S.S0[seg_base + i])[2] = CELL_NONE;   // the stage re-reads S0 from the state array
+    }
+}
+
 #if MANTA_TWO_STAGE
 // ---- the pass in two stages per chunk, software-pipelined per warp through shared memory (H <= 256 only) --------
 // Stage A of chunk k + 1 (state records, occupancy words, search; the leader's payload entry is requested with
@@ -848,7 +877,7 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
         r = leader_window(P, B, V.c, V.row0, start, own, V.len_c, P.H, s2v, s3v, h, budget_left, dist_next);
         if (r == WIN_DONE) {
             n_cells += h.found ? h.dist - V.c : P.H - budget_left;
-        } else if (!cannot_cross(P, V)) {   // rare: near the edge end and the window does not fit
+        } else if (!may_defer(P, V)) {   // rare: near an edge end and the window does not fit
             h = r == WIN_MORE ? leader_continue(P, B, V, s3v.z, budget_left, dist_next, n_cells) : walk_rows(P, B, V, n_cells);
             r = WIN_DONE;
         }
@@ -861,15 +890,7 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
         // (kind 3): out of the route store into L2 now
         prefetch_line(P.route + V.cursor + (kind == 2u ? 5u : 1u));
         prefetch_line(P.route + V.cursor + (kind == 2u ? 8u : 4u));
-        const uint32_t k = atomicAdd(&sm.qn, 1u);
-#if MANTA_DQ
-        if (k < dq_cap) {
-            sm.dq[k][0] = s0v;
-            sm.dq[k][1] = s1v;
-            sm.dq[k][2] = e;
-        } else
-#endif
-            P.dlist[seg_base + k] = e;
+        defer_entry(P, t, sm, S, seg_base, i, dq_cap, s0v, s1v, e);
     }
     REC(buf, 0) = s0v;
     REC(buf, 1) = s1v;
@@ -909,15 +930,7 @@ __device__ __forceinline__ void stage_finish(const DevP &P, uint32_t t, UpdateSm
         write_out(P, t, sm, seg_base, i, V, O);
     } else if (searched) {   // must look at the adjacent lane (R5): deferred, kinds 0 / 1
         const uint4 e = make_uint4(i | ((ld.found ? 1u : 0u) << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u);
-        const uint32_t k = atomicAdd(&sm.qn, 1u);
-#if MANTA_DQ
-        if (k < dq_cap) {
-            sm.dq[k][0] = s0v;
-            sm.dq[k][1] = s1v;
-            sm.dq[k][2] = e;
-        } else
-#endif
-            P.dlist[seg_base + k] = e;
+        defer_entry(P, t, sm, P.st[sbuf_of(t)], seg_base, i, dq_cap, s0v, s1v, e);
     }
     __syncwarp();
 }
@@ -955,15 +968,26 @@ __device__ __forceinline__ void pass_two_stage(const DevP &P, uint32_t t, Update
 
 // Must be called by ALL threads of the block (contains __syncthreads).  Warps take chunks of 32 slots from a
 // shared counter, so a warp that met slow vehicles simply takes fewer chunks.
+// how many deferred entries of a block stay in shared memory (with their S0 / S1 records); the rest go through P.dlist.
+// Kernel-per-phase stepping keeps none: there the deferred stage runs in the next launch.
+__device__ __forceinline__ uint32_t dq_capacity(const DevP &P, bool persistent)
+{
+    if (!MANTA_DQ || !persistent) return 0u;
+    return (P.flags & MANTA_FLAG_TINY_QUEUES) ? 2u : (uint32_t)MANTA_DQ;
+}
+
+// The update pass over the block's segment.  Vehicles that must look at the adjacent lane (or continue their
+// look-ahead past the cached hops) are only QUEUED here (deferred list); they are finished by second_phase, after
+// the grid barrier, next to the claim resolution -- two dependent chains that used to run one after the other.
 template <bool W256>
-__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd, uint4 *rec = nullptr)
+__device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, uint32_t &n_upd, uint4 *rec, bool persistent)
 {
     const int cur = (int)(t & 1u), nxt = cur ^ 1;
     const StBuf &S = P.st[sbuf_of(t)];
     const u64 *B = P.bits[cur];
     const uint2 *pay = P.pay[cur];
     const uint32_t lane_id = threadIdx.x & 31u;
-    const uint32_t dq_cap = MANTA_DQ ? ((P.flags & MANTA_FLAG_TINY_QUEUES) ? 2u : (uint32_t)MANTA_DQ) : 0u;
+    const uint32_t dq_cap = dq_capacity(P, persistent);
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
         const uint32_t n = P.seg_cnt[seg];
         const uint32_t seg_base = seg * P.seg_cap;
@@ -1027,7 +1051,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
                     r = leader_window(P, B, V.c, V.row0, start, own, V.len_c, P.H, s2v, s3v, h, budget_left, dist_next);
                     if (r == WIN_DONE) {
                         n_cells += h.found ? h.dist - V.c : P.H - budget_left;
-                    } else if (!cannot_cross(P, V)) {   // rare: near the edge end and the window does not fit
+                    } else if (!may_defer(P, V)) {   // rare: near an edge end and the window does not fit
                         h = r == WIN_MORE ? leader_continue(P, B, V, s3v.z, budget_left, dist_next, n_cells) : walk_rows(P, B, V, n_cells);
                         r = WIN_DONE;
                     }
@@ -1057,15 +1081,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
                 const uint32_t kind = searched ? (ld.found ? 1u : 0u) : (r == WIN_MORE ? 2u : 3u);
                 const uint4 e = searched ? make_uint4(i | (kind << 30), (uint32_t)ld.lead_abs, __float_as_uint(ld.v_lead), 0u)
                                          : make_uint4(i | (kind << 30), budget_left, dist_next, s3v.z);
-                const uint32_t k = atomicAdd(&sm.qn, 1u);
-#if MANTA_DQ
-                if (k < dq_cap) {
-                    sm.dq[k][0] = s0v;
-                    sm.dq[k][1] = s1v;
-                    sm.dq[k][2] = e;
-                } else
-#endif
-                    P.dlist[seg_base + k] = e;
+                defer_entry(P, t, sm, S, seg_base, i, dq_cap, s0v, s1v, e);
             }
             __syncwarp();
 #if MANTA_PF
@@ -1074,45 +1090,60 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             base = __shfl_sync(0xFFFFFFFFu, next_base, 0);
 #endif
         }
-        __syncthreads();   // the deferred list of this segment is complete (and visible: same block)
+        __syncthreads();   // the cross list and the deferred list of this segment are complete
         DBG_STAMP(2);
-        const uint32_t qn = sm.qn;
-        for (uint32_t k = threadIdx.x; k < qn; k += blockDim.x) {
-            uint4 e, a0, a1;   // one call site: finish_deferred is ~2 k instructions
-#if MANTA_DQ
-            if (k < dq_cap) {
-                e = sm.dq[k][2];
-                a0 = sm.dq[k][0];
-                a1 = sm.dq[k][1];
-            } else
-#endif
-            {
-                e = P.dlist[seg_base + k];
-                const uint32_t slot = e.x & 0x3FFFFFFFu;
-                a0 = S.S0[seg_base + slot];
-                a1 = S.S1[seg_base + slot];
-            }
-            finish_deferred<W256>(P, t, sm, seg_base, e, a0, a1, n_cells);
+        if (threadIdx.x == 0u) {
+            P.seg_xn[seg] = sm.xn;
+            P.seg_qn[seg] = sm.qn;
         }
-        __syncthreads();
-        DBG_STAMP(3);
-        if (threadIdx.x == 0u) P.seg_xn[seg] = sm.xn;
     }
 }
 
 // ------------------------------------------------------------------------------------------------ X: R8
 // One thread per cross-list entry: resolve the claim; the winner moves to its next route edge and rebuilds its
 // look-ahead cache, the loser holds at the stop line; both write their time-(t+1) mark and payload.
-__device__ __forceinline__ void second_phase(const DevP &P, uint32_t t)
+// Then the deferred list of the same segment (R5-R7 for the vehicles that look at the adjacent lane, R2 for look-aheads
+// that run past the cached hops): they read atlas_t only, cannot be edge-end candidates and do not mark entry windows
+// (may_defer), so nothing they do interacts with the claims or with the fused admission.  Cross-list entries go to
+// the first MANTA_XT threads of the block, deferred entries to the others: the two chains run in different warps.
+#ifndef MANTA_XT
+#define MANTA_XT 128u   // threads of a block that take cross-list entries in the second phase; the others take deferred entries
+#endif
+template <bool W256>
+__device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, bool persistent)
 {
     const int nxt = (int)((t & 1u) ^ 1u);
     const StBuf &S = P.st[sbuf_of(t)];
     u64 *Bn = P.bits[nxt];
     uint2 *payn = P.pay[nxt];
+    const uint32_t dq_cap = dq_capacity(P, persistent);
+    const bool split = blockDim.x > MANTA_XT;
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
-        const uint32_t xn = P.seg_xn[seg];
+        const uint32_t xn = persistent ? sm.xn : P.seg_xn[seg];
+        const uint32_t qn = persistent ? sm.qn : P.seg_qn[seg];
         const uint32_t seg_base = seg * P.seg_cap;
-        for (uint32_t k = threadIdx.x; k < xn; k += blockDim.x) {
+        const uint32_t d0 = split ? MANTA_XT : 0u, dstep = blockDim.x - d0;
+        if (threadIdx.x >= d0)
+            for (uint32_t k = threadIdx.x - d0; k < qn; k += dstep) {
+                uint4 e, a0, a1;   // one call site: finish_deferred is ~2 k instructions
+#if MANTA_DQ
+                if (k < dq_cap) {
+                    e = sm.dq[k][2];
+                    a0 = sm.dq[k][0];
+                    a1 = sm.dq[k][1];
+                } else
+#endif
+                {
+                    e = P.dlist[seg_base + k];
+                    const uint32_t slot = e.x & 0x3FFFFFFFu;
+                    a0 = S.S0[seg_base + slot];
+                    a1 = S.S1[seg_base + slot];
+                }
+                finish_deferred<W256>(P, t, sm, seg_base, e, a0, a1, n_cells);
+            }
+        const uint32_t xstep = split ? MANTA_XT : blockDim.x;
+        if (threadIdx.x < xstep)
+        for (uint32_t k = threadIdx.x; k < xn; k += xstep) {
             const uint4 xl = P.xlist[seg_base + k];     // {slot, claim word, cursor, id}
             const size_t at = (size_t)seg_base + xl.x;
             uint4 s0 = S.S0[at];
@@ -1183,15 +1214,22 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_update(const DevP P, u
     if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0ull;
     __syncthreads();
     uint32_t n_cells = 0u, n_upd = 0u;
-    update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec);
+    update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec, false);
     flush_stats(P, sm, n_cells, n_upd);
 }
 
-// second phase of step t; with admit_next, the admission of step t + 1 runs in the same launch (fused, see admit_phase)
-__global__ void __launch_bounds__(256) k_second(const DevP P, uint32_t t, int admit_next)
+// second phase of step t (claim resolution + deferred list); with admit_next, the admission of step t + 1 runs in the
+// same launch (fused, see admit_phase)
+template <bool W256>
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_second(const DevP P, uint32_t t, int admit_next)
 {
+    __shared__ UpdateSmem sm;
+    if (threadIdx.x < 4u) sm.ev[threadIdx.x] = 0ull;
+    __syncthreads();
+    uint32_t n_cells = 0u;
     if (admit_next) admit_phase<true>(P, t + 1u, sbuf_of(t));
-    second_phase(P, t);
+    second_phase<W256>(P, t, sm, n_cells, false);
+    flush_stats(P, sm, n_cells, 0u);
 }
 
 // the five stages of the re-sort as kernels (multi-kernel mode); n_live / per_seg travel through sort_part[n_seg..]
@@ -1319,12 +1357,16 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
     if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     for (uint32_t t = t0; t < t_end; t++) {
         DBG_STAMP(0);
-        update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec);
+        update_phase<W256>(P, t, sm, n_cells, n_upd, dyn_rec, true);
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(4);
         const bool more = t + 1u < t_end;
         if (more && fuse) admit_phase<true>(P, t + 1u, sbuf_of(t));   // the longer dependent chain first
-        second_phase(P, t);
+        DBG_STAMP(3);
+        second_phase<W256>(P, t, sm, n_cells, true);
+#ifdef MANTA_DBG
+        if (threadIdx.x == MANTA_XT && (t & 31u) == 7u) P.dbg_buf[blockIdx.x * 8u + 7u] = gtimer();
+#endif
 #if MANTA_PF >= 3
         if (more) {   // the state records of this block's first chunks of step t + 1: on their way while the barrier completes
             const StBuf &Sn = P.st[sbuf_of(t + 1u)];
