@@ -13,7 +13,8 @@ over all active vehicles.  The simulation is first advanced (untimed: initialisa
              replicas -- "replicas only")
   e2e        same metric through the C ABI with HOST buffers: manta_load_trips (H2D of routes and departures) +
              manta_step from 05:00 to the end of the timed window + manta_readback (D2H), wall clock
-  roofline   update-phase kernel: algorithmic bytes per launch / its CUDA-event duration, vs measured HBM peak
+  roofline   update-pass kernel (k_update): SURVEY 8(d) useful bytes per launch / its CUDA-event duration, vs the
+             measured HBM peak (frac); the layout's own byte model and the committed ncu traffic beside it
   cpu_baseline  the oracle (oracle/manta_oracle.c, single thread) on a bounded sample of the same workload
 
 --impl reference times the oracle itself (there is no other reference implementation: the paper ships no code).
@@ -122,23 +123,71 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def algorithmic_bytes(hbar, flc, lookback):
-    """Algorithmic bytes per vehicle-update, 1-bit occupancy plane + 8-byte payload plane +
-    64-byte in-place vehicle state.  Update phase: state read 64 (position / speed, edge geometry, cached rows and
-    lengths of the next four route edges) + rewritten position word 16, own-lane occupancy bits hbar / 8, leader
-    payload 8, new mark (8-byte word) 8 + own payload 8, toggling the old mark off 8; a deferred adjacent-lane
-    evaluation adds its list entry (16 written + 16 read), the target row's bits ahead and behind and two payloads.
-    The whole step adds the cross-list entry and claim of the ~2 % of vehicles at an edge end and the amortised
-    re-sort (128 B per vehicle every MANTA_SORT_EVERY = 64 steps), folded in as 6 B."""
-    upd = 64.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0 + flc * (32.0 + (hbar + lookback) / 8.0 + 16.0)
-    return upd, upd + 6.0
+def contract_bytes(hbar, flc):
+    """SURVEY.md section 8(d), "Algorithmic bytes per vehicle-update", useful-byte column, evaluated at the measured
+    mean look-ahead hbar (cells) and lane-change evaluation fraction flc: active index 4, hot state read + write
+    16 + 16, route entries 16, edge attributes 16, forward occupancy scan 2 hbar (the contract counts the paper's
+    2-byte cells), leader speed 4, lane-change rows flc (2 hbar + 128 + 8), new occupancy + speed + old clear 8.
+    Returns (bytes of the update pass = everything but the lane-change rows, bytes of the whole step).  The pass
+    kernel (k_update) does not touch the lane-change rows: those vehicles are finished in the second phase."""
+    base = 4.0 + 32.0 + 16.0 + 16.0 + 2.0 * hbar + 4.0 + 8.0
+    return base, base + flc * (2.0 * hbar + 136.0)
 
 
-# DRAM bytes k_update actually moved, from the committed ncu --set full capture (profiles/r01e_two_stage.md):
-# dram__bytes_read.sum + dram__bytes_write.sum = 72.7 MB + 6.7 MB for a launch of 383,948 vehicle-updates with the
-# L2 flushed before the launch (ncu's default cache control), i.e. 207 B per update (live, application replay:
-# 135-165 B).  bench.py reports it scaled to the updates per launch of its own timed window.
-NCU_TRAFFIC_BYTES_PER_UPDATE = (72.678656e6 + 6.671360e6) / 383948.0
+def layout_bytes(hbar, flc, lookback):
+    """Bytes the method must move with THIS layout: 1-bit occupancy plane, 8-byte payload entry
+    per four cells, 64-byte in-place vehicle state.  Pass: state read 64 + rewritten position word 16, own-lane
+    occupancy bits hbar / 8, leader payload 8, new mark (8-byte word) 8 + own payload 8, old mark off 8.  Whole step:
+    + the deferred adjacent-lane evaluations (list entry 32, target row bits ahead and behind, two payloads) and 6 B
+    for the cross list, claims and the amortised re-sort."""
+    upd = 64.0 + 16.0 + hbar / 8.0 + 8.0 + 8.0 + 8.0 + 8.0
+    return upd, upd + flc * (32.0 + (hbar + lookback) / 8.0 + 16.0) + 6.0
+
+
+def source_hash():
+    """sha256 over the CUDA sources the library is built from: keys the ncu traffic captures under profiles/."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_2007_03614_b200", "csrc")
+    for name in ("manta_api.cu", "manta_kernels.cuh", "manta_device.cuh"):
+        with open(os.path.join(base, name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config, start_step):
+    """DRAM bytes k_update moved per vehicle-update (dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` capture, L2 flushed before the launch), from profiles/k_update_traffic.csv -- only a line
+    captured on THIS build of the sources (source_hash) and this workload window counts; None if there is none."""
+    path = os.path.join(ROOT, "profiles", "k_update_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    sh = source_hash()
+    best = None
+    with open(path) as f:
+        for line in f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7 or c[0].startswith("#") or c[0] == "source_hash":
+                continue
+            if c[0] == sh and int(c[1]) == config and int(c[2]) == start_step:
+                best = {"bytes_per_update": (float(c[4]) + float(c[5])) / float(c[3]), "capture": c[6], "source_hash": sh}
+    return best
+
+
+def host_cpu():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return model, os.cpu_count() or 1
+
+
+ORACLE_SAMPLE_TRIPS, ORACLE_SAMPLE_STEPS = 12000, 1800
 
 
 def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.5):
@@ -168,29 +217,32 @@ def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.
 
 
 def run_reference(args):
-    """--impl reference: the oracle as it stands on the host cores, same config / metric / unit."""
+    """--impl reference: the oracle as it stands on the host cores, same config / metric / unit.  Its timed sample is
+    the one the cpu_baseline leg of the default run uses (ORACLE_SAMPLE_TRIPS trips departing from the start of the
+    timed window, ORACLE_SAMPLE_STEPS timesteps), so the two oracle figures agree; it does not depend on --steps:
+    20 timesteps of a 12,000-trip sample would be a nearly empty network."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     net, trips, params, _ = make_workload(args.scale, config=args.config)
     K, W = args.steps, args.warmup
-    # sample sized so that W + K oracle steps end within ~2 minutes (about 1.5 us per update on one core)
-    n_sample = int(min(200000, max(2000, 100.0 / ((K + W) * 1.5e-6))))
     from oracle import manta_oracle
     manta_oracle.build()
-    upd_w, wall_w, n_tr, _ = oracle_sample(net, trips, params, args.start_step, n_sample, W + K)
-    # time K steps = total minus a separately timed W-step warm-up run of the same sample
-    upd_0, wall_0, _, _ = oracle_sample(net, trips, params, args.start_step, n_sample, W) if W else (0, 0.0, 0, 0)
-    upd, wall = upd_w - upd_0, max(wall_w - wall_0, 1e-9)
+    if W:   # warm-up: page the library and the workload in
+        oracle_sample(net, trips, params, args.start_step, 2000, min(200, 10 * W))
+    upd, wall, n_tr, _ = oracle_sample(net, trips, params, args.start_step, ORACLE_SAMPLE_TRIPS, ORACLE_SAMPLE_STEPS)
     val = upd / wall
-    sample = ("first %d trips departing from step %d of configs[%d] (scale %g), run %d timesteps from their first "
-              "departure" % (n_tr, args.start_step, args.config, args.scale, K))
+    model, cores = host_cpu()
+    sample = ("first %d trips departing from step %d of configs[%d] (scale %g), %d timesteps from their first "
+              "departure (%.2e updates in %.1f s); the sample does not scale with --steps"
+              % (n_tr, args.start_step, args.config, args.scale, ORACLE_SAMPLE_STEPS, upd, wall))
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
-           "warmup": W, "ms_per_step": wall / K * 1e3, "higher_is_better": True, "scaling": "weak",
+           "warmup": W, "ms_per_step": wall / ORACLE_SAMPLE_STEPS * 1e3, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": "%s, scale %g" % (CONFIGS[args.config][0], args.scale),
                       "sample": sample, "l2": "n/a (CPU)"},
-           "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                            "cpu_model": model, "host_cores": cores},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out), flush=True)
@@ -297,6 +349,7 @@ def main():
     per, gap = Kp // n_sl, (K - Kp) // n_sl
     Kp = per * n_sl
     ph, d = [0.0, 0.0, 0.0], None
+    sim.step_timed(3)                                     # the kernel-per-phase variants load on first use: not timed
     for _ in range(n_sl):
         r0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
         p_sl = sim.step_timed(per)
@@ -308,22 +361,34 @@ def main():
     sim.close()
     hbar = d["cells_examined"] / max(1, d["vehicle_updates"])
     flc = d["lc_evals"] / max(1, d["vehicle_updates"])
-    # algorithmic bytes per vehicle-update: whole step, and the update phase alone
-    bytes_update, bytes_step = algorithmic_bytes(hbar, flc, params.get("lookback_cells", 64))
+    # Algorithmic bytes per vehicle-update.  Contract figure: SURVEY.md section 8(d)'s useful-byte table at the
+    # measured hbar / f_lc (roofline.frac).  Beside it the bytes this layout must move (frac_layout), and the DRAM
+    # bytes ncu saw k_update move on this build, if a capture of this build is committed (frac_traffic).
+    c_update, c_step = contract_bytes(hbar, flc)
+    l_update, l_step = layout_bytes(hbar, flc, params.get("lookback_cells", 64))
     peak, peak_src = measured_peak()
     upd_per_launch = d["vehicle_updates"] / Kp
     t_update = ph[1] / Kp * 1e-3
-    achieved = bytes_update * upd_per_launch / t_update / 1e9
+    achieved = c_update * upd_per_launch / t_update / 1e9
+    tr = ncu_traffic(args.config, args.start_step)
     roofline = {"bound": "hbm", "kernel": "k_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_UPDATE * upd_per_launch,
-                "traffic_source": "ncu --set full (profiles/r01e_two_stage.md): %.0f B per update, L2 flushed; "
-                                  "scaled to this run's updates per launch" % NCU_TRAFFIC_BYTES_PER_UPDATE,
-                "peak_source": peak_src,
-                "bytes_per_update": bytes_update, "updates_per_launch": upd_per_launch,
-                "avg_launch_us": t_update * 1e6, "hbar_cells": hbar, "f_lc": flc,
-                "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp},
-                "step_bytes_per_update": bytes_step,
-                "step_frac": bytes_step * value / world / 1e9 / peak}
+                "frac": achieved / peak,
+                "bytes_model": "SURVEY.md 8(d) useful bytes at the measured hbar, f_lc; k_update = all rows but the "
+                               "lane-change rows (those vehicles are finished by k_second)",
+                "bytes_per_update": c_update, "step_bytes_per_update": c_step,
+                "step_frac": c_step * value / world / 1e9 / peak,
+                "frac_layout": l_update * upd_per_launch / t_update / 1e9 / peak,
+                "bytes_per_update_layout": l_update, "step_bytes_per_update_layout": l_step,
+                "step_frac_layout": l_step * value / world / 1e9 / peak,
+                "traffic": tr["bytes_per_update"] * upd_per_launch if tr else None,
+                "frac_traffic": tr["bytes_per_update"] * upd_per_launch / t_update / 1e9 / peak if tr else None,
+                "traffic_source": ("profiles/k_update_traffic.csv, capture %s on this build (sources %s): %.0f B per "
+                                   "update, L2 flushed before the launch; scaled to this run's updates per launch"
+                                   % (tr["capture"], tr["source_hash"], tr["bytes_per_update"])) if tr else
+                                  "no ncu capture of this build (sources %s) at this window is committed" % source_hash(),
+                "target_frac": 0.5, "peak_source": peak_src,
+                "updates_per_launch": upd_per_launch, "avg_launch_us": t_update * 1e6, "hbar_cells": hbar, "f_lc": flc,
+                "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp}}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -365,9 +430,11 @@ def main():
     if not args.no_cpu and rank == 0 and world == 1:
         from oracle import manta_oracle
         manta_oracle.build()
-        n_s, k_s = 12000, 1800
+        n_s, k_s = ORACLE_SAMPLE_TRIPS, ORACLE_SAMPLE_STEPS
         c_upd, c_wall, n_tr, _ = oracle_sample(net, trips, params, args.start_step, n_s, k_s)
+        model, cores = host_cpu()
         out["cpu_baseline"] = {"value": c_upd / c_wall, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "cpu_model": model, "host_cores": cores,
                                "sample": "first %d trips departing from step %d of the same workload, %d timesteps "
                                          "(%.2e updates in %.1f s)" % (n_tr, args.start_step, k_s, c_upd, c_wall)}
     if rank == 0:

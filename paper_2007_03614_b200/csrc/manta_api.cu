@@ -5,6 +5,7 @@
 #include "manta_kernels.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -12,6 +13,7 @@
 #include <cstring>
 #include <numeric>
 #include <string>
+#include <chrono>
 #include <thread>
 #include <vector>
 
@@ -146,6 +148,67 @@ void derive_constants(manta_sim *s, double max_init_speed)
     s->P.Z_in = s->P.L_c + s->P.Z_out;
 }
 uint32_t len_min(const manta_sim *s) { return std::max(s->P.Z_out + 1u, s->P.L_c + 1u); }
+
+// Stable counting sort on several host threads: out[r] = i for the r-th element in (key[i], i) order; elements with
+// key == MANTA_NONE are left out.  start[k] (size n_keys + 1) receives the offset of key k's run.  Every thread
+// counts its own contiguous range of i, the offsets are interleaved (key-major, thread-minor), every thread scatters
+// its range: ranges are in index order, so the order inside a key's run is the index order.
+void counting_sort_stable(const uint32_t *key, uint32_t n, uint32_t n_keys, std::vector<uint32_t> &start, std::vector<uint32_t> &out)
+{
+    const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+    unsigned nt = n < (1u << 18) ? 1u : std::min(hw, 8u);
+    while (nt > 1u && (uint64_t)nt * n_keys > (48ull << 20)) nt /= 2u;   // bound the per-thread histograms
+    std::vector<uint32_t> hist((size_t)nt * n_keys, 0u);
+    auto range = [&](unsigned w, uint64_t &i0, uint64_t &i1) { i0 = (uint64_t)n * w / nt; i1 = (uint64_t)n * (w + 1) / nt; };
+    auto run = [&](auto fn) {
+        if (nt == 1u) { fn(0u); return; }
+        std::vector<std::thread> th;
+        for (unsigned w = 0; w < nt; w++) th.emplace_back([=, &fn] { fn(w); });
+        for (auto &t : th) t.join();
+    };
+    run([&](unsigned w) {
+        uint64_t i0, i1;
+        range(w, i0, i1);
+        uint32_t *h = hist.data() + (size_t)w * n_keys;
+        for (uint64_t i = i0; i < i1; i++)
+            if (key[i] != MANTA_NONE) h[key[i]]++;
+    });
+    start.assign((size_t)n_keys + 1, 0u);
+    uint32_t acc = 0u;
+    for (uint32_t k = 0; k < n_keys; k++) {
+        start[k] = acc;
+        for (unsigned w = 0; w < nt; w++) {
+            uint32_t &h = hist[(size_t)w * n_keys + k];
+            const uint32_t c = h;
+            h = acc;
+            acc += c;
+        }
+    }
+    start[n_keys] = acc;
+    out.resize(acc);
+    run([&](unsigned w) {
+        uint64_t i0, i1;
+        range(w, i0, i1);
+        uint32_t *h = hist.data() + (size_t)w * n_keys;
+        for (uint64_t i = i0; i < i1; i++)
+            if (key[i] != MANTA_NONE) out[h[key[i]]++] = (uint32_t)i;
+    });
+}
+
+// fn(i0, i1) over [0, n) in contiguous ranges on up to 16 host threads (small n: the calling thread alone)
+template <class F>
+void parallel_ranges(uint64_t n, F fn)
+{
+    const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+    const unsigned nt = n < (1ull << 18) ? 1u : std::min(hw, 16u);
+    if (nt == 1u) {
+        fn((uint64_t)0, n);
+        return;
+    }
+    std::vector<std::thread> th;
+    for (unsigned w = 0; w < nt; w++) th.emplace_back([=, &fn] { fn(n * w / nt, n * (w + 1) / nt); });
+    for (auto &t : th) t.join();
+}
 
 }  // namespace
 
@@ -372,15 +435,52 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0 || n_trips >= 0x7FFFFFFFu)
         return fail(s, MANTA_ERR_INVALID_ARG, "null / empty / too many trips");
     CUDA_TRY(s, cudaSetDevice(s->device));
+    // MANTA_LOAD_TIMING=1: wall time of each stage of this call on stderr (initialisation is outside the timed path,
+    // but it is most of the end-to-end time of a short run)
+    const bool timing = getenv("MANTA_LOAD_TIMING") != nullptr;
+    auto t_prev = std::chrono::steady_clock::now();
+    auto lap = [&](const char *what) {
+        if (!timing) return;
+        const auto now = std::chrono::steady_clock::now();
+        fprintf(stderr, "[manta_load_trips] %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(now - t_prev).count());
+        t_prev = now;
+    };
     const uint64_t total = route_ptr[n_trips];
     if (route_ptr[0] != 0 || total >= 0xFFFFFFFFull) return fail(s, MANTA_ERR_BAD_ROUTE, "route_ptr must start at 0 and stay below 2^32 entries");
     // ---- validation (BAD_ROUTE): every route entry is looked at once; split over host threads for large inputs, the
     // error reported is that of the lowest trip index, as a sequential scan would report it
+    // The route entries (by far the largest input: 0.8 GB at configs[2]) start their way to the device NOW, on a helper
+    // thread, while this thread and its workers validate them and build ids and queues on the host: a copy from
+    // pageable memory is staged by the driver and costs as much wall time as the validation.  If the validation
+    // fails the copy is awaited and the buffer released.
+    uint32_t *d_re = (uint32_t *)dev_alloc(s, total * sizeof(uint32_t));
+    if (!d_re) return fail(s, MANTA_ERR_OOM, "device allocation of %llu bytes failed", (unsigned long long)(total * sizeof(uint32_t)));
+    struct Uploader {
+        std::thread th;
+        cudaError_t err = cudaSuccess;
+        void join() { if (th.joinable()) th.join(); }
+        ~Uploader() { join(); }
+    } up;
+    up.th = std::thread([&up, s, d_re, route_edges, total] {
+        cudaError_t e = cudaSetDevice(s->device);
+        const uint64_t slice = 16ull << 20;   // entries per copy
+        for (uint64_t off = 0; off < total && e == cudaSuccess; off += slice)
+            e = cudaMemcpyAsync(d_re + off, route_edges + off, std::min(slice, total - off) * sizeof(uint32_t), cudaMemcpyHostToDevice, s->stream);
+        up.err = e;
+    });
+    auto drop_upload = [&](int rc) {
+        up.join();
+        cudaStreamSynchronize(s->stream);
+        dev_free(s, d_re);
+        return rc;
+    };
+    std::vector<uint32_t> first_edge(n_trips);   // filled by the validation pass (route_ptr is walked in trip order there)
     struct Bad { uint32_t trip; int kind; uint64_t pos; };   // kind 0: none
     auto scan = [&](uint32_t i0, uint32_t i1, Bad &bad, double &max_init) {
         for (uint32_t i = i0; i < i1; i++) {
             const uint64_t b = route_ptr[i], e = route_ptr[i + 1];
             if (e <= b || e > total) { bad = {i, 1, 0}; return; }
+            first_edge[i] = route_edges[b];
             for (uint64_t k = b; k < e; k++) {
                 if (route_edges[k] >= s->n_edges) { bad = {i, 2, k - b}; return; }
                 if (k > b && s->head[route_edges[k - 1]] != s->tail[route_edges[k]]) { bad = {i, 3, k - b}; return; }
@@ -394,67 +494,85 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         }
     };
     double max_init = 0.0;
-    {
-        const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
-        const unsigned nt = total < (1ull << 20) ? 1u : std::min(hw, 32u);
-        std::vector<Bad> bad(nt, Bad{0u, 0, 0});
-        std::vector<double> mx(nt, 0.0);
-        if (nt == 1u) {
-            scan(0u, n_trips, bad[0], mx[0]);
-        } else {
-            std::vector<std::thread> th;
-            for (unsigned w = 0; w < nt; w++) {
-                const uint32_t i0 = (uint32_t)((uint64_t)n_trips * w / nt), i1 = (uint32_t)((uint64_t)n_trips * (w + 1) / nt);
-                th.emplace_back([&, w, i0, i1] { scan(i0, i1, bad[w], mx[w]); });
-            }
-            for (auto &t : th) t.join();
-        }
-        for (unsigned w = 0; w < nt; w++) {   // ranges are in trip order: the first bad one is the lowest trip index
-            const Bad &b = bad[w];
-            switch (b.kind) {
-            case 0: break;
-            case 1: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: empty route", b.trip);
-            case 2: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: edge id out of range", b.trip);
-            case 3: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: route not connected at position %llu", b.trip, (unsigned long long)b.pos);
-            case 4: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: negative departure time", b.trip);
-            default: return fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: bad init_speed", b.trip);
-            }
-            max_init = std::max(max_init, mx[w]);
+    const unsigned hw_val = std::max(1u, std::thread::hardware_concurrency());
+    const unsigned nt_val = total < (1ull << 20) ? 1u : std::min(hw_val, 32u);
+    std::vector<Bad> bad(nt_val, Bad{0u, 0, 0});
+    std::vector<double> mx(nt_val, 0.0);
+    std::vector<std::thread> val_threads;   // large inputs: the workers run while this thread builds the vehicle ids
+    if (nt_val == 1u) {
+        scan(0u, n_trips, bad[0], mx[0]);
+    } else {
+        for (unsigned w = 0; w < nt_val; w++) {
+            const uint32_t a = (uint32_t)((uint64_t)n_trips * w / nt_val), b = (uint32_t)((uint64_t)n_trips * (w + 1) / nt_val);
+            val_threads.emplace_back([&, w, a, b] { scan(a, b, bad[w], mx[w]); });
         }
     }
+    // ---- vehicle ids: rank in the stable (depart_step, trip index) order (needs only the departure times)
+    std::vector<uint32_t> dstep(n_trips), trip_of_id;
+    std::atomic<uint32_t> too_late(MANTA_NONE);   // lowest trip index whose departure step does not fit 32 bits
+    parallel_ranges(n_trips, [&](uint64_t a, uint64_t b) {
+        for (uint64_t i = a; i < b; i++) {
+            const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
+            const double ds = std::floor((double)depart_time_s[i] / (double)s->prm.dt);
+            if (!pre && !(ds < 4294967295.0)) {   // (also NaN / negative garbage: reported by the validation)
+                if (ds >= 4294967295.0) {
+                    uint32_t cur = too_late.load();
+                    while ((uint32_t)i < cur && !too_late.compare_exchange_weak(cur, (uint32_t)i)) {}
+                }
+                dstep[i] = 0u;
+                continue;
+            }
+            dstep[i] = (pre || ds < 0.0) ? 0u : (uint32_t)ds;
+        }
+    });
+    {
+        const uint32_t max_step = *std::max_element(dstep.begin(), dstep.end());
+        if (max_step < (1u << 24)) {   // counting sort by departure step, trip order kept inside a step (stable)
+            std::vector<uint32_t> start;
+            counting_sort_stable(dstep.data(), n_trips, max_step + 1u, start, trip_of_id);
+        } else {
+            trip_of_id.resize(n_trips);
+            std::iota(trip_of_id.begin(), trip_of_id.end(), 0u);
+            std::stable_sort(trip_of_id.begin(), trip_of_id.end(), [&](uint32_t x, uint32_t y) { return dstep[x] < dstep[y]; });
+        }
+    }
+    for (auto &t : val_threads) t.join();
+    for (unsigned w = 0; w < nt_val; w++) {   // ranges are in trip order: the first bad one is the lowest trip index
+        const Bad &b = bad[w];
+        switch (b.kind) {
+        case 0: break;
+        case 1: return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: empty route", b.trip));
+        case 2: return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: edge id out of range", b.trip));
+        case 3: return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: route not connected at position %llu", b.trip, (unsigned long long)b.pos));
+        case 4: return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: negative departure time", b.trip));
+        default: return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: bad init_speed", b.trip));
+        }
+        max_init = std::max(max_init, mx[w]);
+    }
+    if (too_late.load() != MANTA_NONE) return drop_upload(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: departure too late", too_late.load()));
+    lap("validate routes | vehicle ids");
     const DevP saved = s->P;
     derive_constants(s, max_init);
-    auto rollback = [&](int rc) { s->P = saved; return rc; };
+    bool upload_joined = false;
+    auto rollback = [&](int rc) {
+        s->P = saved;
+        if (!upload_joined) drop_upload(rc);
+        return rc;
+    };
     for (uint32_t e = 0; e < s->n_edges; e++)
         if (s->len_c[e] < len_min(s)) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "edge %u shorter than LEN_MIN for the pre-placed speeds", e));
     if (s->prm.lookback_cells < s->P.L_c + s->P.Z_out)
         return rollback(fail(s, MANTA_ERR_INVALID_ARG, "lookback_cells %u < L_c + Z_out = %u (R5)", s->prm.lookback_cells, s->P.L_c + s->P.Z_out));
 
-    // ---- vehicle ids: rank in the stable (depart_step, trip index) order
-    std::vector<uint32_t> dstep(n_trips), trip_of_id(n_trips);
-    for (uint32_t i = 0; i < n_trips; i++) {
-        const bool pre = init_pos_m && init_pos_m[i] >= 0.0f;
-        const double ds = std::floor((double)depart_time_s[i] / (double)s->prm.dt);
-        if (!pre && ds >= 4294967295.0) return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "trip %u: departure too late", i));
-        dstep[i] = pre ? 0u : (uint32_t)ds;
-    }
-    {
-        const uint32_t max_step = *std::max_element(dstep.begin(), dstep.end());
-        if (max_step < (1u << 24)) {   // counting sort by departure step, trip order kept inside a step (stable)
-            std::vector<uint32_t> start((size_t)max_step + 2, 0u);
-            for (uint32_t i = 0; i < n_trips; i++) start[dstep[i] + 1u]++;
-            for (uint32_t v = 0; v <= max_step; v++) start[v + 1u] += start[v];
-            for (uint32_t i = 0; i < n_trips; i++) trip_of_id[start[dstep[i]]++] = i;
-        } else {
-            std::iota(trip_of_id.begin(), trip_of_id.end(), 0u);
-            std::stable_sort(trip_of_id.begin(), trip_of_id.end(), [&](uint32_t x, uint32_t y) { return dstep[x] < dstep[y]; });
+    std::vector<uint32_t> depart_by_id(n_trips), route_start(n_trips), first_by_id(n_trips);
+    parallel_ranges(n_trips, [&](uint64_t i0, uint64_t i1) {
+        for (uint64_t id = i0; id < i1; id++) {
+            const uint32_t tr = trip_of_id[id];
+            depart_by_id[id] = dstep[tr];
+            route_start[id] = (uint32_t)route_ptr[tr];
+            first_by_id[id] = (init_pos_m && init_pos_m[tr] >= 0.0f) ? MANTA_NONE : first_edge[tr];   // NONE: pre-placed, no queue
         }
-    }
-    std::vector<uint32_t> depart_by_id(n_trips), route_start(n_trips);
-    for (uint32_t id = 0; id < n_trips; id++) {
-        depart_by_id[id] = dstep[trip_of_id[id]];
-        route_start[id] = (uint32_t)route_ptr[trip_of_id[id]];
-    }
+    });
     // ---- pre-placed vehicles (R1, last sentence) and their spacing check
     std::vector<uint4> init_a0;
     {
@@ -477,34 +595,32 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
                 (int64_t)(keyx[k].first & 0xFFFFFFFFull) - (int64_t)(keyx[k - 1].first & 0xFFFFFFFFull) < (int64_t)s->P.L_fx)
                 return rollback(fail(s, MANTA_ERR_BAD_ROUTE, "pre-placed vehicles closer than L on edge %llu", (unsigned long long)(keyx[k].first >> 32)));
     }
+    lap("ids -> depart / route start, pre-placed");
     // ---- admission FIFOs: waiting trips grouped by first edge, id order inside (G25)
     // q_ent = {vehicle id, depart_step, route cursor, depart_step of the next entry of the same queue or NONE}
     std::vector<uint32_t> q_edge, q_end;
     std::vector<uint4> q_ent, q_row, q_state;
     {
-        std::vector<uint32_t> cnt(s->n_edges + 1, 0);
-        for (uint32_t id = 0; id < n_trips; id++) {
-            const uint32_t tr = trip_of_id[id];
-            if (init_pos_m && init_pos_m[tr] >= 0.0f) continue;
-            cnt[route_edges[route_ptr[tr]] + 1]++;
-        }
-        for (uint32_t e = 0; e < s->n_edges; e++) cnt[e + 1] += cnt[e];
-        q_ent.assign((size_t)cnt[s->n_edges] + 1, make_uint4(MANTA_NONE, MANTA_NONE, 0u, MANTA_NONE));
-        std::vector<uint32_t> fill(cnt.begin(), cnt.end() - 1);
-        for (uint32_t id = 0; id < n_trips; id++) {
-            const uint32_t tr = trip_of_id[id];
-            if (init_pos_m && init_pos_m[tr] >= 0.0f) continue;
-            q_ent[fill[route_edges[route_ptr[tr]]]++] = make_uint4(id, depart_by_id[id], route_start[id], MANTA_NONE);
-        }
+        std::vector<uint32_t> cnt, q_ids;   // waiting vehicle ids grouped by first edge, id order inside a group
+        counting_sort_stable(first_by_id.data(), n_trips, s->n_edges, cnt, q_ids);
+        q_ent.resize(q_ids.size() + 1);
+        q_ent.back() = make_uint4(MANTA_NONE, MANTA_NONE, 0u, MANTA_NONE);
+        parallel_ranges(q_ids.size(), [&](uint64_t k0, uint64_t k1) {
+            for (uint64_t k = k0; k < k1; k++) {
+                const uint32_t id = q_ids[k];
+                const bool has_next = k + 1 < q_ids.size() && first_by_id[q_ids[k + 1]] == first_by_id[id];
+                q_ent[k] = make_uint4(id, depart_by_id[id], route_start[id], has_next ? depart_by_id[q_ids[k + 1]] : MANTA_NONE);
+            }
+        });
         for (uint32_t e = 0; e < s->n_edges; e++)
             if (cnt[e + 1] > cnt[e]) {
                 q_edge.push_back(e);
                 q_end.push_back(cnt[e + 1]);
                 const uint4 h = q_ent[cnt[e]];
                 q_state.push_back(make_uint4(h.y, cnt[e], h.x, h.z));
-                for (uint32_t k = cnt[e]; k + 1 < cnt[e + 1]; k++) q_ent[k].w = q_ent[k + 1].y;
             }
     }
+    lap("admission queues");
     // ---- launch geometry and vehicle segments.  A segment is processed by one block per phase; the persistent
     // kernel needs all of its blocks co-resident (cooperative launch), so n_seg = that grid.
     s->w256 = s->prm.lookahead_cells <= 256u && s->prm.lookback_cells <= 128u;
@@ -538,7 +654,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (cap >= 0xFFFFFFFFull) return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
     // ---- upload; expand the route store on the device
     int rc;
-    uint32_t *d_re = nullptr, *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qend;
+    uint32_t *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qend;
     uint64_t *d_rp = nullptr;
     uint4 *d_route, *d_qent, *d_qrow, *d_qstate;
     for (size_t k = 0; k < q_edge.size(); k++) {
@@ -546,7 +662,13 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         const uint32_t prio_word = s->node_prio[s->tail[e]] ? s->n_edges * 8u + s->tail[e] : MANTA_NONE;
         q_row.push_back(make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16), prio_word, e));
     }
-    if ((rc = upload(s, &d_re, route_edges, total))) return rollback(rc);
+    lap("launch geometry");
+    up.join();   // the route entries are on their way (enqueued on the simulation's stream)
+    if (up.err != cudaSuccess) {
+        s->sticky_cuda = true;
+        return rollback(fail(s, MANTA_ERR_CUDA, "route upload failed: %s", cudaGetErrorString(up.err)));
+    }
+    upload_joined = true;
     if ((rc = upload(s, &d_rp, route_ptr, (uint64_t)n_trips + 1))) return rollback(rc);
     if ((rc = upload(s, &d_rowptr, s->row_ptr.data(), s->row_ptr.size()))) return rollback(rc);
     d_route = (uint4 *)dev_alloc(s, (total + 8) * sizeof(uint4));   // + 8: the look-ahead requests four records ahead
@@ -555,6 +677,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     k_expand_routes<<<(unsigned)std::min<uint64_t>((total + 255) / 256, 65535ull * 16), 256, 0, s->stream>>>(P.edge_tab, d_rowptr, d_re, total, d_route);
     k_mark_last<<<(n_trips + 255) / 256, 256, 0, s->stream>>>(d_rp, n_trips, d_route);
     CUDA_TRY(s, cudaGetLastError());
+    lap("route upload + expand (enqueued)");
     if ((rc = upload(s, &d_rs, route_start.data(), n_trips))) return rollback(rc);
     if ((rc = upload(s, &s->d_trip_of_id, trip_of_id.data(), n_trips))) return rollback(rc);
     if ((rc = alloc_fill(s, &d_adm, n_trips, 0xFF))) return rollback(rc);
@@ -584,6 +707,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
         if ((rc = upload(s, &P.bucket_seg, bs.data(), bs.size()))) return rollback(rc);
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // bs goes out of scope
     }
+    lap("tables, state arrays, sort scratch (sync)");
     if ((rc = alloc_fill(s, &P.seg_xn, P.n_seg, 0))) return rollback(rc);
     if ((rc = alloc_fill(s, &P.dbg_buf, (uint64_t)P.n_seg * 8, 0))) return rollback(rc);
     if ((rc = alloc_fill(s, &P.seg_qn, P.n_seg, 0))) return rollback(rc);
@@ -609,6 +733,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     dev_free(s, d_re);
     dev_free(s, d_rp);
     dev_free(s, d_rowptr);
+    lap("lists, initial placement, final sync");
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
