@@ -21,12 +21,14 @@
 #include <string.h>
 
 #define NONE32 0xFFFFFFFFu
+#define NONE64 0xFFFFFFFFFFFFFFFFull
 #define BOUND_INF 0x7FFFFFFF
 
 struct mo_sim {
     /* network (lanes, length, free-flow speed per edge) */
     uint32_t n_nodes, n_edges;
     uint32_t *row_ptr, *head, *tail, *len_c;
+    uint32_t *in_idx, *indeg; /* STOP nodes (R8s): index of an edge among its head node's inbound edges; in-degree */
     uint8_t *lanes, *ctrl;
     float *limit;
     double max_limit;
@@ -50,14 +52,18 @@ struct mo_sim {
     uint32_t *route_edges; /* caller order              */
     uint32_t *trip_of_id, *id_of_trip;
     uint32_t *depart_step;
-    uint8_t *status, *lane, *tag;
+    uint8_t *status, *lane, *tag, *wait;
     uint32_t *rpos, *x_fx, *admit_step, *arrive_step;
     float *v, *acc_last;
     /* tentative next state of the step in flight */
     uint8_t *nx_kind, *nx_lane, *nx_tag;
     uint32_t *nx_x, *nx_claim;
     float *nx_v;
-    uint32_t *claim; /* [n_rows + n_nodes] min-id claim words */
+    uint64_t *claim; /* [n_rows + n_nodes] claim words: smallest key wins (key = vehicle id, or rank << 32 | id at STOP nodes) */
+    uint64_t *nx_key;
+    uint32_t W_stop; /* steps a vehicle stands at a STOP node's stop line: ceil(stop_time_s / dt) */
+    uint64_t *stat_sum; /* [stat_n_slices * n_edges] */
+    uint32_t *stat_cnt;
     /* lists */
     uint32_t *active, n_active;
     uint32_t *pending, n_pending, next_dep;
@@ -141,11 +147,35 @@ float mo_idm_acc(const mo_sim *S, float v, float v0, int has_leader, float s, fl
 
 uint32_t mo_pmlc(const mo_sim *S, uint32_t dcell) { return dcell <= 5u * S->Lam ? S->P_mlc[dcell] : 0u; }
 
+/* ---------------------------------------------------------------- R3s */
+/* Desired speed of a driver on an edge ("each driver's maximum possible speed per edge, v0, is
+ * sampled from a Gaussian distribution centered around the edge's predetermined speed limit"; reading G27):
+ * v0 = limit * clamp(1 + v0_sigma_rel * z, 1/2, 3/2), z the Irwin-Hall normal of generator words 7..9 at the
+ * counter 0xFFFFFFFF - r (r = route position), so every (vehicle, route position) has its own draw.  sigma = 0: limit. */
+static float desired_speed(const mo_sim *S, uint32_t id, uint32_t r, float limit)
+{
+    if (!(S->p.v0_sigma_rel > 0.0f)) return limit;
+    int32_t sum = 0;
+    for (uint32_t k = 7; k < 10; k++) {
+        uint32_t w = rng32(S->p.seed, id, 0xFFFFFFFFu - r, k);
+        sum += (int32_t)(w & 255u) + (int32_t)((w >> 8) & 255u) + (int32_t)((w >> 16) & 255u) + (int32_t)(w >> 24);
+    }
+    float z = (float)(sum - 1530);
+    z = z * 0.00390625f; /* 2^-8 */
+    float f = S->p.v0_sigma_rel * z;
+    f = 1.0f + f;
+    f = fmaxf(f, 0.5f);
+    f = fminf(f, 1.5f);
+    return limit * f;
+}
+
 /* ---------------------------------------------------------------- R0 */
 static void derive_constants(mo_sim *S, double max_init_speed)
 {
     const mo_params *p = &S->p;
-    double vcap = (S->max_limit > max_init_speed ? S->max_limit : max_init_speed) + (double)p->a * (double)p->dt;
+    /* the fastest possible vehicle: the largest desired speed (limit, times 3/2 at most with per-driver v0, G27) */
+    double vmax = S->max_limit * (p->v0_sigma_rel > 0.0f ? 1.5 : 1.0);
+    double vcap = (vmax > max_init_speed ? vmax : max_init_speed) + (double)p->a * (double)p->dt;
     S->L_c = (uint32_t)ceil((double)p->veh_len);
     S->L_fx = (int32_t)lround((double)p->veh_len * 1024.0);
     S->Z_out = (uint32_t)ceil(vcap * (double)p->dt) + 1u;
@@ -174,6 +204,10 @@ mo_sim *mo_create(uint32_t n_nodes, uint32_t n_edges, const uint32_t *row_ptr, c
     if (node_ctrl) memcpy(S->ctrl, node_ctrl, n_nodes);
     for (uint32_t u = 0; u < n_nodes; u++)
         for (uint32_t e = row_ptr[u]; e < row_ptr[u + 1]; e++) S->tail[e] = u;
+    S->in_idx = (uint32_t *)calloc(n_edges, sizeof(uint32_t));
+    S->indeg = (uint32_t *)calloc(n_nodes, sizeof(uint32_t));
+    for (uint32_t e = 0; e < n_edges; e++) /* inbound edges of a node in edge-id order */
+        if (head[e] < n_nodes) S->in_idx[e] = S->indeg[head[e]]++;
     S->max_limit = 0.0;
     uint32_t rows = 0;
     for (uint32_t e = 0; e < n_edges; e++) {
@@ -228,8 +262,13 @@ mo_sim *mo_create(uint32_t n_nodes, uint32_t n_edges, const uint32_t *row_ptr, c
             S->P_mlc[d] = (uint32_t)floor(4294967296.0 * exp(-(xi - 1.0) * (xi - 1.0)));
         }
     }
-    S->claim = (uint32_t *)malloc(sizeof(uint32_t) * ((size_t)rows + n_nodes));
-    for (size_t i = 0; i < (size_t)rows + n_nodes; i++) S->claim[i] = NONE32;
+    S->claim = (uint64_t *)malloc(sizeof(uint64_t) * ((size_t)rows + n_nodes));
+    for (size_t i = 0; i < (size_t)rows + n_nodes; i++) S->claim[i] = NONE64;
+    S->W_stop = (uint32_t)ceil((double)p->stop_time_s / (double)p->dt - 1e-9);
+    if (p->stat_period_steps && p->stat_n_slices) {
+        S->stat_sum = (uint64_t *)calloc((size_t)p->stat_n_slices * n_edges, sizeof(uint64_t));
+        S->stat_cnt = (uint32_t *)calloc((size_t)p->stat_n_slices * n_edges, sizeof(uint32_t));
+    }
     S->edge_entries = (uint32_t *)calloc(n_edges, sizeof(uint32_t));
     return S;
 }
@@ -238,6 +277,7 @@ void mo_destroy(mo_sim *S)
 {
     if (!S) return;
     free(S->row_ptr); free(S->head); free(S->tail); free(S->len_c); free(S->lanes); free(S->ctrl);
+    free(S->in_idx); free(S->indeg); free(S->wait); free(S->nx_key); free(S->stat_sum); free(S->stat_cnt);
     free(S->limit); free(S->first_row); free(S->row_off);
     for (int k = 0; k < 2; k++) { free(S->occ[k]); free(S->frac[k]); free(S->spd[k]); }
     free(S->P_mlc); free(S->route_ptr); free(S->route_edges); free(S->trip_of_id); free(S->id_of_trip);
@@ -322,6 +362,7 @@ int mo_load_trips(mo_sim *S, uint32_t n_trips, const uint64_t *route_ptr, const 
     S->trip_of_id = (uint32_t *)malloc(4 * n); S->id_of_trip = (uint32_t *)malloc(4 * n);
     S->depart_step = (uint32_t *)malloc(4 * n);
     S->status = (uint8_t *)calloc(n, 1); S->lane = (uint8_t *)calloc(n, 1); S->tag = (uint8_t *)calloc(n, 1);
+    S->wait = (uint8_t *)calloc(n, 1); S->nx_key = (uint64_t *)calloc(n, sizeof(uint64_t));
     S->rpos = (uint32_t *)calloc(n, 4); S->x_fx = (uint32_t *)calloc(n, 4);
     S->admit_step = (uint32_t *)malloc(4 * n); S->arrive_step = (uint32_t *)malloc(4 * n);
     S->v = (float *)calloc(n, 4); S->acc_last = (float *)calloc(n, 4);
@@ -437,18 +478,19 @@ static void admission(mo_sim *S)
             if (free_window) chosen = S->first_row[e] + l;
         }
         S->nx_claim[id] = chosen;
-        if (chosen != NONE32 && id < S->claim[chosen]) S->claim[chosen] = id; /* smallest id wins */
+        if (chosen != NONE32 && (uint64_t)id < S->claim[chosen]) S->claim[chosen] = id; /* smallest id wins */
     }
     uint32_t n_keep = 0;
     for (uint32_t k = 0; k < S->n_pending; k++) {
         uint32_t id = S->pending[k];
         uint32_t row = S->nx_claim[id];
-        if (row != NONE32 && S->claim[row] == id) {
+        if (row != NONE32 && S->claim[row] == (uint64_t)id) {
             uint32_t e = route_edge(S, id, 0);
             S->status[id] = MO_ACTIVE;
             S->x_fx[id] = 0;
             S->v[id] = 0.0f;
             S->tag[id] = 0;
+            S->wait[id] = 0;
             S->rpos[id] = 0;
             S->lane[id] = (uint8_t)(row - S->first_row[e]);
             S->admit_step[id] = S->t;
@@ -461,7 +503,7 @@ static void admission(mo_sim *S)
     }
     for (uint32_t k = 0; k < S->n_pending; k++) { /* reset the claim words used */
         uint32_t row = S->nx_claim[ordcopy[k]];
-        if (row != NONE32) S->claim[row] = NONE32;
+        if (row != NONE32) S->claim[row] = NONE64;
     }
     S->n_pending = n_keep;
     free(ordcopy);
@@ -529,7 +571,7 @@ static int lag_in_lane(mo_sim *S, int A, uint32_t e, uint32_t lt, uint32_t c, in
     return 0;
 }
 
-enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
+enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2, KIND_HOLD = 3 };
 
 /* ---------------------------------------------------------------- R2..R8 for one vehicle */
 static void update_vehicle(mo_sim *S, uint32_t id)
@@ -544,8 +586,16 @@ static void update_vehicle(mo_sim *S, uint32_t id)
     int32_t len_fx = (int32_t)(len_c << 10);
     int32_t x = (int32_t)S->x_fx[id];
     uint32_t c = (uint32_t)x >> 10;
-    float v = S->v[id], v0 = S->limit[e];
+    float v = S->v[id], v0 = desired_speed(S, id, r, S->limit[e]);
     S->n_updates++;
+    /* per-edge speed statistics (Eq. 5 inputs): instantaneous speeds of time t, every period steps */
+    if (S->stat_sum && S->t % p->stat_period_steps == 0u) {
+        uint32_t slice = S->t / p->stat_slice_steps;
+        if (slice < p->stat_n_slices) {
+            S->stat_sum[(size_t)slice * S->n_edges + e] += (uint64_t)lrintf(v * 256.0f);
+            S->stat_cnt[(size_t)slice * S->n_edges + e] += 1u;
+        }
+    }
 
     /* R2 */
     int32_t lead_abs = 0;
@@ -693,12 +743,30 @@ static void update_vehicle(mo_sim *S, uint32_t id)
         uint32_t en = route_edge(S, id, r + 1);
         uint32_t lplus = l_new;
         if (lplus > (uint32_t)S->lanes[en] - 1u) lplus = (uint32_t)S->lanes[en] - 1u;
-        uint32_t word = (S->ctrl[S->head[e]] == 0) ? S->first_row[en] + lplus /* GREEN: lane entry */
-                                                   : S->n_rows + S->head[e];  /* PRIORITY: the node */
-        S->nx_kind[id] = KIND_CAND;
+        uint32_t u = S->head[e];
+        uint32_t word = (S->ctrl[u] == 0) ? S->first_row[en] + lplus /* GREEN: lane entry */
+                                          : S->n_rows + u;           /* PRIORITY, STOP: the node */
+        uint64_t key = id;
         S->nx_x[id] = (uint32_t)(xn - len_fx);
+        if (S->ctrl[u] == 2 && S->wait[id] < S->W_stop) {
+            /* R8s ("every vehicle is designed to stop at the intersection for 2 seconds before
+             * proceeding"): it stands at the stop line for W_stop steps before it may ask for the node */
+            S->nx_kind[id] = KIND_HOLD;
+            return;
+        }
+        if (S->ctrl[u] == 2) {
+            /* R8s ("a round-robin of the nm combinations ... based on their position in their lane
+             * queue"): the n inbound x m outbound combinations take turns; at step t combination (c - t) mod nm = 0
+             * is first, then 1, ...; only the front vehicle of a lane can be here; equal combinations: smallest id */
+            uint32_t m = S->row_ptr[u + 1] - S->row_ptr[u], nm = S->indeg[u] * m;
+            uint32_t c = S->in_idx[e] * m + (en - S->row_ptr[u]);
+            uint32_t rank = (c + nm - S->t % nm) % nm;
+            key = ((uint64_t)rank << 32) | id;
+        }
+        S->nx_kind[id] = KIND_CAND;
         S->nx_claim[id] = word;
-        if (id < S->claim[word]) S->claim[word] = id;
+        S->nx_key[id] = key;
+        if (key < S->claim[word]) S->claim[word] = key;
     }
 }
 
@@ -730,7 +798,12 @@ static void commit(mo_sim *S)
             S->n_done++;
             S->sum_travel += (uint64_t)(S->arrive_step[id] - S->admit_step[id]);
             continue;
-        } else if (S->claim[S->nx_claim[id]] == id) { /* winner crosses */
+        } else if (S->nx_kind[id] == KIND_HOLD) { /* R8s: stands at the stop line, one more step done */
+            S->lane[id] = S->nx_lane[id];
+            S->x_fx[id] = (S->len_c[e] << 10) - 1u;
+            S->v[id] = 0.0f;
+            S->wait[id] += 1;
+        } else if (S->claim[S->nx_claim[id]] == S->nx_key[id]) { /* winner crosses */
             uint32_t en = route_edge(S, id, r + 1);
             uint32_t lplus = S->nx_lane[id];
             if (lplus > (uint32_t)S->lanes[en] - 1u) lplus = (uint32_t)S->lanes[en] - 1u;
@@ -739,6 +812,7 @@ static void commit(mo_sim *S)
             S->x_fx[id] = S->nx_x[id];
             S->v[id] = S->nx_v[id];
             S->tag[id] = 0;
+            S->wait[id] = 0;
             S->edge_entries[en] += 1;
         } else { /* loser holds at the stop line (G15) */
             S->lane[id] = S->nx_lane[id];
@@ -749,7 +823,7 @@ static void commit(mo_sim *S)
     }
     for (uint32_t k = 0; k < S->n_active; k++) { /* reset claim words */
         uint32_t id = S->active[k];
-        if (S->nx_kind[id] == KIND_CAND) S->claim[S->nx_claim[id]] = NONE32;
+        if (S->nx_kind[id] == KIND_CAND) S->claim[S->nx_claim[id]] = NONE64;
     }
     for (uint32_t k = 0; k < S->n_active; k++) {
         uint32_t id = S->active[k];
@@ -807,6 +881,7 @@ int mo_set_state(mo_sim *S, uint32_t t, const uint8_t *status, const uint32_t *r
         S->v[id] = v[tr];
         S->admit_step[id] = admit_step[tr];
         S->arrive_step[id] = arrive_step[tr];
+        S->wait[id] = 0;
         if (status[tr] == MO_ACTIVE) {
             uint32_t e;
             if (route_pos[tr] >= route_len(S, id)) return -3;
@@ -821,6 +896,32 @@ int mo_set_state(mo_sim *S, uint32_t t, const uint8_t *status, const uint32_t *r
     }
     if (edge_entries) memcpy(S->edge_entries, edge_entries, sizeof(uint32_t) * S->n_edges);
     return 0;
+}
+
+void mo_set_wait(mo_sim *S, const uint8_t *wait)
+{
+    for (uint32_t tr = 0; tr < S->n_trips; tr++) S->wait[S->id_of_trip[tr]] = wait[tr];
+}
+void mo_get_wait(const mo_sim *S, uint8_t *wait)
+{
+    for (uint32_t tr = 0; tr < S->n_trips; tr++) wait[tr] = S->wait[S->id_of_trip[tr]];
+}
+void mo_get_edge_speed_stats(const mo_sim *S, uint64_t *sum_q8, uint32_t *samples)
+{
+    size_t n = (size_t)S->p.stat_n_slices * S->n_edges;
+    if (!S->stat_sum) return;
+    if (sum_q8) memcpy(sum_q8, S->stat_sum, n * sizeof(uint64_t));
+    if (samples) memcpy(samples, S->stat_cnt, n * sizeof(uint32_t));
+}
+float mo_v0(const mo_sim *S, uint32_t id, uint32_t r)
+{
+    return desired_speed(S, id, r, S->limit[route_edge(S, id, r)]);
+}
+uint64_t mo_n_stopped(const mo_sim *S)
+{
+    uint64_t n = 0;
+    for (uint32_t k = 0; k < S->n_active; k++) n += (S->v[S->active[k]] == 0.0f);
+    return n;
 }
 
 /* ---------------------------------------------------------------- outputs */

@@ -35,11 +35,20 @@ typedef struct {
     float lc_gap_high;   /* g_a = g_b above 25 mph, m                         */
     float lc_eps_sigma;  /* std-dev of epsilon, m (Eq. 3, 4: 1)               */
     uint64_t seed;       /* seed of the counter-based generator (G22)         */
+    float stop_time_s;   /* STOP nodes: time every vehicle stands at the stop line, s (2) */
+    float v0_sigma_rel;  /* per-driver desired speed: v0 = limit * clamp(1 + v0_sigma_rel * z, 1/2, 3/2),
+                            z ~ N(0,1) per (vehicle, route position) (reading G27); 0 = off  */
+    uint32_t stat_period_steps; /* per-edge speed statistics (Eq. 5 inputs): every this many
+                                   steps each ACTIVE vehicle adds its speed to its edge's accumulators; 0 = off  */
+    uint32_t stat_slice_steps;  /* steps per time slice of the statistics                                     */
+    uint32_t stat_n_slices;     /* number of time slices kept                                                 */
 } mo_params;
 
 enum { MO_WAITING = 0, MO_ACTIVE = 1, MO_DONE = 2 };
 
-/* node_ctrl may be NULL (= all GREEN).  0 GREEN (case 2), 1 PRIORITY (one vehicle per node per step). */
+/* node_ctrl may be NULL (= all GREEN).  0 GREEN (case 2), 1 PRIORITY (one vehicle per node per step, smallest id),
+ * 2 STOP (case 1 in full: every vehicle stands stop_time_s at the stop line, then one vehicle per
+ * node per step in a round-robin over the (inbound edge, outbound edge) combinations; rule R8s of DESIGN.md). */
 mo_sim *mo_create(uint32_t n_nodes, uint32_t n_edges, const uint32_t *row_ptr, const uint32_t *head,
                   const float *length_m, const uint8_t *lanes, const float *speed_limit,
                   const uint8_t *node_ctrl, const mo_params *p);
@@ -53,6 +62,16 @@ int mo_step(mo_sim *S, uint32_t n_steps);
 int mo_set_state(mo_sim *S, uint32_t t, const uint8_t *status, const uint32_t *route_pos, const uint8_t *lane,
                  const uint8_t *tag, const uint32_t *x_fx, const float *v, const uint32_t *admit_step,
                  const uint32_t *arrive_step, const uint32_t *edge_entries);
+/* tests only: the stop-line counters of R8s (steps already stood at a STOP node on the current edge), caller order */
+void mo_set_wait(mo_sim *S, const uint8_t *wait);
+void mo_get_wait(const mo_sim *S, uint8_t *wait);
+/* per-edge speed statistics: sum_q8[slice * n_edges + e] = sum of rint(v * 256) over the samples, samples[...] their
+ * number; either may be NULL */
+void mo_get_edge_speed_stats(const mo_sim *S, uint64_t *sum_q8, uint32_t *samples);
+/* desired speed of vehicle `id` at route position r (R3s / G27) */
+float mo_v0(const mo_sim *S, uint32_t id, uint32_t r);
+/* ACTIVE vehicles standing still (v = 0) now: the "stuck count" of a gridlocked network */
+uint64_t mo_n_stopped(const mo_sim *S);
 void mo_destroy(mo_sim *S);
 
 /* outputs, indexed by the CALLER's trip index; any pointer may be NULL */

@@ -36,12 +36,14 @@ class _Params(C.Structure):
                 ("veh_len", C.c_float), ("lookahead_cells", C.c_uint32), ("lookback_cells", C.c_uint32),
                 ("mlc_scale_m", C.c_float), ("dlc_gain_thr", C.c_float), ("lc_alpha", C.c_float),
                 ("lc_gap_low", C.c_float), ("lc_gap_high", C.c_float), ("lc_eps_sigma", C.c_float),
-                ("seed", C.c_uint64)]
+                ("seed", C.c_uint64), ("stop_time_s", C.c_float), ("v0_sigma_rel", C.c_float),
+                ("stat_period_steps", C.c_uint32), ("stat_slice_steps", C.c_uint32), ("stat_n_slices", C.c_uint32)]
 
 
 DEFAULT_PARAMS = dict(dt=0.5, a=1.0, b=2.0, T=1.5, s0=2.0, veh_len=5.0, lookahead_cells=128, lookback_cells=64,
                       mlc_scale_m=100.0, dlc_gain_thr=0.2, lc_alpha=0.2, lc_gap_low=3.0, lc_gap_high=7.5,
-                      lc_eps_sigma=1.0, seed=20070361)
+                      lc_eps_sigma=1.0, seed=20070361, stop_time_s=2.0, v0_sigma_rel=0.0, stat_period_steps=0,
+                      stat_slice_steps=7200, stat_n_slices=0)
 
 _lib = None
 
@@ -64,6 +66,13 @@ def lib():
         L.mo_step.argtypes = [C.c_void_p, C.c_uint32]
         L.mo_set_state.restype = C.c_int
         L.mo_set_state.argtypes = [C.c_void_p, C.c_uint32] + [C.c_void_p] * 9
+        L.mo_set_wait.argtypes = [C.c_void_p, C.c_void_p]
+        L.mo_get_wait.argtypes = [C.c_void_p, C.c_void_p]
+        L.mo_get_edge_speed_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.mo_v0.restype = C.c_float
+        L.mo_v0.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32]
+        L.mo_n_stopped.restype = C.c_uint64
+        L.mo_n_stopped.argtypes = [C.c_void_p]
         L.mo_destroy.argtypes = [C.c_void_p]
         L.mo_get_state.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         L.mo_get_trip_results.argtypes = [C.c_void_p] * 3
@@ -148,6 +157,9 @@ class Oracle:
         rc = lib().mo_set_state(self.h, int(t), *[_ptr(x) for x in a])
         if rc != 0:
             raise ValueError("mo_set_state failed: %d" % rc)
+        if st.get("wait") is not None:
+            w = np.ascontiguousarray(st["wait"], np.uint8)
+            lib().mo_set_wait(self.h, _ptr(w))
 
     def state(self):
         n = self.n_trips
@@ -159,7 +171,23 @@ class Oracle:
         arr = np.zeros(n, np.uint32)
         lib().mo_get_trip_results(self.h, _ptr(adm), _ptr(arr))
         out["admit_step"], out["arrive_step"] = adm, arr
+        out["wait"] = np.zeros(n, np.uint8)
+        lib().mo_get_wait(self.h, _ptr(out["wait"]))
         return out
+
+    def edge_speed_stats(self):
+        """(sum of rint(v * 256), samples), each [stat_n_slices, n_edges]"""
+        ns = int(self.params["stat_n_slices"])
+        sm, cn = np.zeros((ns, self.n_edges), np.uint64), np.zeros((ns, self.n_edges), np.uint32)
+        if ns and self.params["stat_period_steps"]:
+            lib().mo_get_edge_speed_stats(self.h, _ptr(sm), _ptr(cn))
+        return sm, cn
+
+    def v0(self, vid, r):
+        return float(lib().mo_v0(self.h, vid, r))
+
+    def n_stopped(self):
+        return int(lib().mo_n_stopped(self.h))
 
     def edge_entries(self):
         e = np.zeros(self.n_edges, np.uint32)
@@ -171,7 +199,9 @@ class Oracle:
         lib().mo_get_summary(self.h, _ptr(s))
         keys = ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps", "vehicle_updates", "lane_changes",
                 "cells_examined", "lc_evals")
-        return {k: int(x) for k, x in zip(keys, s)}
+        out = {k: int(x) for k, x in zip(keys, s)}
+        out["n_stopped"] = self.n_stopped()
+        return out
 
     def derived(self):
         d = np.zeros(6, np.uint32)
