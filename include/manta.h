@@ -38,6 +38,11 @@ extern "C" {
 
 #define MANTA_GREEN 0    /* case 2: every vehicle passes; conflicts per (edge, lane) entry  */
 #define MANTA_PRIORITY 1 /* case 1 exclusivity: one vehicle per node per step, smallest vehicle id first */
+#define MANTA_STOP 2     /* case 1 in full: every vehicle stands stop_time_s at the stop line, then
+                            one vehicle per node per step, the (inbound, outbound) edge combinations taking turns
+                            (round-robin), equal combinations by smallest vehicle id -- rule R8s of DESIGN.md.
+                            Limits with STOP nodes: in-degree x out-degree <= 256 per STOP node, n_nodes < 2^27,
+                            n_trips <= 2^24, ceil(stop_time_s / dt) <= 7                                         */
 
 #define MANTA_WAITING 0
 #define MANTA_ACTIVE 1
@@ -92,6 +97,14 @@ typedef struct {
     float lc_eps_sigma;        /* standard deviation of epsilon, m (Eq. 3, 4)                            */
     uint64_t seed;             /* counter-based generator seed (G22)                                     */
     uint32_t flags;            /* MANTA_FLAG_*                                                           */
+    float stop_time_s;         /* MANTA_STOP nodes: standing time at the stop line, s (2)  */
+    float v0_sigma_rel;        /* per-driver desired speed (reading G27): on every edge of its route
+                                  a vehicle's v0 = limit * clamp(1 + v0_sigma_rel * z, 1/2, 3/2), z ~ N(0, 1) from the
+                                  counter-based generator; 0 = v0 is the limit                             */
+    uint32_t stat_period_steps; /* per-edge speed statistics (inputs of Eq. 5): every this many
+                                   steps each ACTIVE vehicle adds its speed to its edge's accumulators; 0 = off    */
+    uint32_t stat_slice_steps;  /* steps per time slice of the statistics (e.g. 7200 = one hour)                   */
+    uint32_t stat_n_slices;     /* time slices kept; samples of later steps are dropped                            */
 } manta_params;
 
 /* Per-trip state snapshot, indexed by the CALLER's trip index.  Any member may be NULL (skipped). */
@@ -103,6 +116,7 @@ typedef struct {
     uint32_t *x_fx;            /* position on the edge, Q22.10 metres (ACTIVE only)                      */
     float *v;                  /* speed m/s (ACTIVE only)                                                */
     float *acc;                /* acceleration applied in the last step (ACTIVE only)                    */
+    uint8_t *wait;             /* steps already stood at the stop line of a MANTA_STOP node (ACTIVE only) */
 } manta_state;
 
 typedef struct {
@@ -118,6 +132,8 @@ typedef struct {
     uint64_t lane_changes;     /* executed lane changes                                                  */
     uint64_t cells_examined;   /* atlas cells examined by the own-lane look-ahead (R2), summed           */
     uint64_t lc_evals;         /* updates that evaluated the adjacent lane (R5)                          */
+    uint64_t n_stopped;        /* ACTIVE vehicles standing still (v = 0) now: the stuck count of a gridlocked network;
+                                  n_stopped == n_active > 0 over many steps = gridlock       */
 } manta_summary;
 
 /* Optional device-memory callbacks (process-wide; install before manta_create).  alloc returns a device pointer
@@ -157,6 +173,12 @@ int manta_step_timed(manta_sim *sim, uint32_t n_steps, double phase_ms[3]);
  * ([n_edges]), per-trip admit/arrive steps ([n_trips]), and the summary counters. */
 int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,
                    manta_summary *summary);
+
+/* Per-edge speed statistics (manta_params.stat_*): sum_q8[slice * n_edges + e] = sum over the samples of
+ * rint(v * 256) (v in m/s), samples[slice * n_edges + e] = their number; mean speed = sum / (256 * samples): the
+ * per-edge average the paper's calibration compares with measured speeds (Eq. 5).  Either array
+ * may be NULL.  Error STATE if the statistics are off. */
+int manta_readback_edge_speeds(manta_sim *sim, uint64_t *sum_q8, uint32_t *samples);
 
 /* Logical atlas of the current step for tests: occ[i] = 0 (empty) or 1 + frac10 per padded cell, spd[i] the
  * occupant's speed; row (e, lane) starts at cell_off[e] + lane * pitch[e].  Sizes via manta_atlas_cells.  (On the

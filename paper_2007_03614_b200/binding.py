@@ -13,14 +13,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmanta.so")
 
 OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
-GREEN, PRIORITY = 0, 1
+GREEN, PRIORITY, STOP = 0, 1, 2
 WAITING, ACTIVE, DONE = 0, 1, 2
 NONE = 0xFFFFFFFF
 FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_timed",
-           "manta_readback", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
+           "manta_readback", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
            "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error")
@@ -43,21 +43,24 @@ class Params(C.Structure):
                 ("s0", C.c_float), ("veh_len", C.c_float), ("lookahead_cells", C.c_uint32),
                 ("lookback_cells", C.c_uint32), ("mlc_scale_m", C.c_float), ("dlc_gain_thr", C.c_float),
                 ("lc_alpha", C.c_float), ("lc_gap_low", C.c_float), ("lc_gap_high", C.c_float),
-                ("lc_eps_sigma", C.c_float), ("seed", C.c_uint64), ("flags", C.c_uint32)]
+                ("lc_eps_sigma", C.c_float), ("seed", C.c_uint64), ("flags", C.c_uint32), ("stop_time_s", C.c_float),
+                ("v0_sigma_rel", C.c_float), ("stat_period_steps", C.c_uint32), ("stat_slice_steps", C.c_uint32),
+                ("stat_n_slices", C.c_uint32)]
 
 
 class State(C.Structure):
-    _fields_ = [(k, C.c_void_p) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc")]
+    _fields_ = [(k, C.c_void_p) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc", "wait")]
 
 
 class Summary(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps",
-                                          "vehicle_updates", "lane_changes", "cells_examined", "lc_evals")]
+                                          "vehicle_updates", "lane_changes", "cells_examined", "lc_evals", "n_stopped")]
 
 
 DEFAULT_PARAMS = dict(dt=0.5, a=1.0, b=2.0, T=1.5, s0=2.0, veh_len=5.0, lookahead_cells=128, lookback_cells=64,
                       mlc_scale_m=100.0, dlc_gain_thr=0.2, lc_alpha=0.2, lc_gap_low=3.0, lc_gap_high=7.5,
-                      lc_eps_sigma=1.0, seed=20070361, flags=0)
+                      lc_eps_sigma=1.0, seed=20070361, flags=0, stop_time_s=2.0, v0_sigma_rel=0.0, stat_period_steps=0,
+                      stat_slice_steps=7200, stat_n_slices=0)
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_int, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.c_void_p)
@@ -85,6 +88,7 @@ def load_library():
     L.manta_sync.argtypes = [C.c_void_p]
     L.manta_step_timed.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(C.c_double * 3)]
     L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
+    L.manta_readback_edge_speeds.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.manta_atlas_cells.argtypes = [C.c_void_p]
     L.manta_atlas_cells.restype = C.c_uint64
     L.manta_readback_atlas.argtypes = [C.c_void_p] * 5
@@ -215,8 +219,8 @@ class Sim:
         if state:
             out.update(status=np.zeros(n, np.uint8), route_pos=np.zeros(n, np.uint32), lane=np.zeros(n, np.uint8),
                        tag=np.zeros(n, np.uint8), x_fx=np.zeros(n, np.uint32), v=np.zeros(n, np.float32),
-                       acc=np.zeros(n, np.float32))
-            S = State(*[_ptr(out[k]) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc")])
+                       acc=np.zeros(n, np.float32), wait=np.zeros(n, np.uint8))
+            S = State(*[_ptr(out[k]) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc", "wait")])
         ee = np.zeros(self.n_edges, np.uint32) if edge_entries else None
         tr = np.zeros((n, 2), np.uint32) if trips else None
         sm = Summary() if summary else None
@@ -230,6 +234,13 @@ class Sim:
         if summary:
             out["summary"] = {k: int(getattr(sm, k)) for k, _ in Summary._fields_}
         return out
+
+    def readback_edge_speeds(self):
+        """(sum of rint(v * 256), samples), each [stat_n_slices, n_edges] (manta_readback_edge_speeds)"""
+        ns = int(self.params["stat_n_slices"])
+        sm, cn = np.zeros((ns, self.n_edges), np.uint64), np.zeros((ns, self.n_edges), np.uint32)
+        self._check(load_library().manta_readback_edge_speeds(self.h, _ptr(sm), _ptr(cn)))
+        return sm, cn
 
     def readback_atlas(self):
         n = int(load_library().manta_atlas_cells(self.h))

@@ -46,7 +46,8 @@ struct manta_sim {
     // host copies of the network
     uint32_t n_nodes = 0, n_edges = 0;
     std::vector<uint32_t> row_ptr, head, tail, len_c, cell_off;
-    std::vector<uint8_t> lanes, node_prio;
+    std::vector<uint8_t> lanes, node_prio;   // node_prio: the node is PRIORITY or STOP (one vehicle per step: the claim word is the node)
+    bool has_stop = false;
     uint32_t min_len_c = 0;
     bool fuse_admit = false;      // admission of step t + 1 runs inside the second phase of step t (two barriers per step)
     double max_limit = 0.0;
@@ -141,7 +142,9 @@ int alloc_fill(manta_sim *s, T **dst, uint64_t n, int byte)
 void derive_constants(manta_sim *s, double max_init_speed)
 {
     const manta_params &p = s->prm;
-    const double vcap = std::max(s->max_limit, max_init_speed) + (double)p.a * (double)p.dt;
+    // the fastest possible vehicle: the largest desired speed (3/2 of the largest limit with per-driver v0, R3s)
+    const double vmax = s->max_limit * (p.v0_sigma_rel > 0.f ? 1.5 : 1.0);
+    const double vcap = std::max(vmax, max_init_speed) + (double)p.a * (double)p.dt;
     s->P.L_c = (uint32_t)std::ceil((double)p.veh_len);
     s->P.L_fx = (int32_t)std::lround((double)p.veh_len * 1024.0);
     s->P.Z_out = (uint32_t)std::ceil(vcap * (double)p.dt) + 1u;
@@ -277,7 +280,10 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         !(p.veh_len <= 62.f) ||   // the entry window [0, L_c] of R1 is tested in one 64-cell word
         p.lookahead_cells < 1 || p.lookahead_cells > 8192 || p.lookback_cells < 1 || p.lookback_cells > 8192 ||
         !(p.mlc_scale_m >= 1.f) || !(p.mlc_scale_m <= 10000.f) || !(p.lc_alpha >= 0.f) || !(p.lc_eps_sigma >= 0.f) ||
-        !std::isfinite(p.dlc_gain_thr) || !std::isfinite(p.lc_gap_low) || !std::isfinite(p.lc_gap_high))
+        !std::isfinite(p.dlc_gain_thr) || !std::isfinite(p.lc_gap_low) || !std::isfinite(p.lc_gap_high) ||
+        !(p.stop_time_s >= 0.f) || !(std::ceil((double)p.stop_time_s / (double)p.dt - 1e-9) <= 7.0) ||   // 3-bit stop-line counter
+        !(p.v0_sigma_rel >= 0.f) || !std::isfinite(p.v0_sigma_rel) ||
+        (p.stat_period_steps != 0u && (p.stat_slice_steps == 0u || p.stat_n_slices == 0u || p.stat_n_slices > 4096u)))
         return fail(nullptr, MANTA_ERR_INVALID_ARG, "parameter out of range");
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device < 0 || cuda_device >= n_dev) {
@@ -356,17 +362,39 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
 
     s->node_prio.assign(N, 0);
     if (net->node_ctrl)
-        for (uint32_t u = 0; u < N; u++) s->node_prio[u] = net->node_ctrl[u] == MANTA_PRIORITY ? 1 : 0;
+        for (uint32_t u = 0; u < N; u++) {
+            if (net->node_ctrl[u] > MANTA_STOP) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "node_ctrl value > 2 at node %u", u));
+            s->node_prio[u] = net->node_ctrl[u] != MANTA_GREEN ? 1 : 0;
+            s->has_stop = s->has_stop || net->node_ctrl[u] == MANTA_STOP;
+        }
+    if (s->has_stop && N >= (1u << 27)) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "STOP nodes need n_nodes < 2^27"));
+    P.W_stop = (uint32_t)std::ceil((double)p.stop_time_s / (double)p.dt - 1e-9);
+    P.id_mask = s->has_stop ? 0x00FFFFFFu : 0xFFFFFFFFu;
+    P.v0_sigma_rel = p.v0_sigma_rel;
+    P.stat_period = p.stat_period_steps; P.stat_slice = p.stat_slice_steps; P.stat_n_slices = p.stat_period_steps ? p.stat_n_slices : 0u;
     s->min_len_c = *std::min_element(s->len_c.begin(), s->len_c.end());
     // ---- device tables
     std::vector<uint4> et(M);
+    std::vector<uint4> es(s->has_stop ? M : 1u, make_uint4(0u, 0u, 0u, 0u));   // STOP nodes (R8s): {n_in * n_out, in_idx * n_out, first out-edge, 0}
+    std::vector<uint32_t> indeg(N, 0u);
     for (uint32_t e = 0; e < M; e++) {
-        const uint32_t prio = (net->node_ctrl && net->node_ctrl[s->head[e]] == MANTA_PRIORITY) ? 1u : 0u;
-        if (net->node_ctrl && net->node_ctrl[s->head[e]] > 1) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "node_ctrl value > 1"));
+        const uint32_t u = s->head[e];
+        const uint32_t prio = s->node_prio[u];
+        const bool stop = net->node_ctrl && net->node_ctrl[u] == MANTA_STOP;
         uint32_t vb;
         memcpy(&vb, &net->speed_limit[e], 4);
-        et[e] = make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16) | (prio << 27), s->head[e], vb);
+        et[e] = make_uint4(s->cell_off[e], s->len_c[e] | ((uint32_t)s->lanes[e] << 16) | (prio << 27), u | (stop ? 1u << 27 : 0u), vb);
+        if (stop) es[e].y = indeg[u];   // index among the node's inbound edges, in edge-id order (times n_out below)
+        indeg[u]++;
     }
+    if (s->has_stop)
+        for (uint32_t e = 0; e < M; e++) {
+            const uint32_t u = s->head[e];
+            if (!(net->node_ctrl[u] == MANTA_STOP)) continue;
+            const uint32_t m = s->row_ptr[u + 1] - s->row_ptr[u];
+            if ((uint64_t)indeg[u] * m > 256u) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "STOP node %u: in-degree x out-degree > 256", u));
+            es[e] = make_uint4(indeg[u] * m, es[e].y * m, s->row_ptr[u], 0u);
+        }
     std::vector<uint32_t> pm(5 * P.Lam + 1);
     for (uint32_t d = 0; d <= 5 * P.Lam; d++) {  // Eq. (2), distances in units of Lambda (G6)
         if (d <= P.Lam)
@@ -379,6 +407,15 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     int rc;
     uint4 *d_et; uint32_t *d_pm, *d_ee; u64 *d_claim; Counters *d_ctr; BlockStats *d_blk;
     if ((rc = upload(s, &d_et, et.data(), M))) return bail(rc);
+    {
+        uint4 *d_es;
+        if ((rc = upload(s, &d_es, es.data(), es.size()))) return bail(rc);
+        P.edge_stop = d_es;
+    }
+    if (P.stat_n_slices) {
+        if ((rc = alloc_fill(s, &P.stat_sum, (uint64_t)P.stat_n_slices * M, 0))) return bail(rc);
+        if ((rc = alloc_fill(s, &P.stat_cnt, (uint64_t)P.stat_n_slices * M, 0))) return bail(rc);
+    }
     if ((rc = upload(s, &d_pm, pm.data(), pm.size()))) return bail(rc);
     if ((rc = alloc_fill(s, &d_ee, M, 0))) return bail(rc);
     if ((rc = alloc_fill(s, &d_claim, (uint64_t)M * 8 + N, 0xFF))) return bail(rc);
@@ -434,6 +471,8 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (s->loaded) return fail(s, MANTA_ERR_STATE, "trips already loaded");
     if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0 || n_trips >= 0x7FFFFFFFu)
         return fail(s, MANTA_ERR_INVALID_ARG, "null / empty / too many trips");
+    if (s->has_stop && n_trips > (1u << 24))
+        return fail(s, MANTA_ERR_INVALID_ARG, "networks with STOP nodes take at most 2^24 trips (the claim key keeps the turn rank above a 24-bit vehicle id)");
     CUDA_TRY(s, cudaSetDevice(s->device));
     // MANTA_LOAD_TIMING=1: wall time of each stage of this call on stderr (initialisation is outside the timed path,
     // but it is most of the end-to-end time of a short run)
@@ -932,18 +971,20 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
     if (edge_entries)
         CUDA_TRY(s, cudaMemcpyAsync(edge_entries, s->P.edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyDeviceToHost, s->stream));
     if (st || trips || sum) {
-        // scratch: status u8 | lane u8 | tag u8 | route_pos u32 | x u32 | v f32 | acc f32 | results uint2
+        // scratch: results uint2 | route_pos u32 | x u32 | v f32 | acc f32 | status u8 | lane u8 | tag u8 | wait u8 | stopped u64
         const uint64_t nn = ((uint64_t)n + 15) & ~15ull;
-        uint8_t *buf = (uint8_t *)dev_alloc(s, nn * (3 + 16 + 8));
+        const uint64_t scratch = nn * (4 + 16 + 8) + 16;
+        uint8_t *buf = (uint8_t *)dev_alloc(s, scratch);
         if (!buf) return fail(s, MANTA_ERR_OOM, "readback scratch allocation failed");
         uint2 *d_res = (uint2 *)buf;
         uint32_t *d_rpos = (uint32_t *)(buf + nn * 8), *d_x = d_rpos + nn;
         float *d_v = (float *)(d_x + nn), *d_acc = d_v + nn;
-        uint8_t *d_status = (uint8_t *)(d_acc + nn), *d_lane = d_status + nn, *d_tag = d_lane + nn;
-        CUDA_TRY(s, cudaMemsetAsync(buf, 0, nn * (3 + 16 + 8), s->stream));
+        uint8_t *d_status = (uint8_t *)(d_acc + nn), *d_lane = d_status + nn, *d_tag = d_lane + nn, *d_wait = d_tag + nn;
+        unsigned long long *d_stopped = (unsigned long long *)(d_wait + nn);
+        CUDA_TRY(s, cudaMemsetAsync(buf, 0, scratch, s->stream));
         const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
         k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
-        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->t == 0 ? 0 : (int)(((s->t - 1u) / MANTA_SORT_EVERY) & 1u), s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc);
+        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->t == 0 ? 0 : (int)(((s->t - 1u) / MANTA_SORT_EVERY) & 1u), s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc, d_wait, d_stopped);
         CUDA_TRY(s, cudaGetLastError());
         std::vector<uint8_t> h_status(n);
         CUDA_TRY(s, cudaMemcpyAsync(h_status.data(), d_status, n, cudaMemcpyDeviceToHost, s->stream));
@@ -954,7 +995,10 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
             if (st->x_fx) CUDA_TRY(s, cudaMemcpyAsync(st->x_fx, d_x, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
             if (st->v) CUDA_TRY(s, cudaMemcpyAsync(st->v, d_v, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
             if (st->acc) CUDA_TRY(s, cudaMemcpyAsync(st->acc, d_acc, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->wait) CUDA_TRY(s, cudaMemcpyAsync(st->wait, d_wait, n, cudaMemcpyDeviceToHost, s->stream));
         }
+        unsigned long long h_stopped = 0;
+        CUDA_TRY(s, cudaMemcpyAsync(&h_stopped, d_stopped, sizeof h_stopped, cudaMemcpyDeviceToHost, s->stream));
         if (trips) CUDA_TRY(s, cudaMemcpyAsync(trips, d_res, (uint64_t)n * 8, cudaMemcpyDeviceToHost, s->stream));
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
         dev_free(s, buf);
@@ -968,6 +1012,7 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
                 sum->n_active += h_status[i] == MANTA_ACTIVE;
             }
             sum->t = s->t;
+            sum->n_stopped = h_stopped;
             for (const BlockStats &b : bs) {
                 sum->lane_changes += b.lane_changes;
                 sum->cells_examined += b.cells_examined;
@@ -978,6 +1023,19 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
             }
         }
     }
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return MANTA_OK;
+}
+
+int manta_readback_edge_speeds(manta_sim *s, uint64_t *sum_q8, uint32_t *samples)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->P.stat_n_slices) return fail(s, MANTA_ERR_STATE, "per-edge speed statistics are off (manta_params.stat_period_steps = 0)");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const uint64_t n = (uint64_t)s->P.stat_n_slices * s->n_edges;
+    if (sum_q8) CUDA_TRY(s, cudaMemcpyAsync(sum_q8, s->P.stat_sum, n * sizeof(uint64_t), cudaMemcpyDeviceToHost, s->stream));
+    if (samples) CUDA_TRY(s, cudaMemcpyAsync(samples, s->P.stat_cnt, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return MANTA_OK;
 }

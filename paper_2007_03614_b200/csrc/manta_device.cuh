@@ -44,14 +44,14 @@ typedef unsigned long long u64;
 // can hold, and DRAM sees runs of neighbouring sectors instead of single random ones.  Dead slots (arrived
 // vehicles, id = NONE) are dropped by the same pass.  Between two sorts a vehicle keeps its slot; admission
 // appends to the segment that currently covers the origin edge's stretch.
-//   S0 = { x_fx, v bits, absolute cell of the time-(t-1) mark or NONE, vehicle id or NONE (dead slot) }
+//   S0 = { x_fx | stop-line counter << 28 (R8s), v bits, absolute cell of the time-(t-1) mark or NONE, vehicle id or NONE (dead slot) }
 //   S1 = { row0 = absolute cell at which the row of the vehicle's own lane starts, geom (+ lane, tag),
 //          route cursor (absolute RouteRec index), v0 bits }
 //   S2 = { word index (cell >> 6) of the row the look-ahead continues in on route edges +1, +2, +3, +4
 //          (lane clamped hop by hop, R2) }
 //   S3 = { len_c of edges +1 | +2 << 16, len_c of edges +3 | +4 << 16 (0 = the route ended before),
 //          bit 0: the route goes on past edge +4, bits 1-3: the (clamped) lane the look-ahead is in on edge +4,
-//          bits 4-31: head node of this edge if it is a PRIORITY node (its claim word of R8),
+//          bits 4-30: head node of this edge if it is a PRIORITY or STOP node (its claim word of R8), bit 31: STOP node,
 //          lane entry (e+ * 8 + lanes(e+) - 1) the vehicle heads for at this edge's end }
 // A stayer rewrites S0 only (S1 when its tag or lane changed, S2/S3 when its lane changed).  A vehicle that
 // arrives leaves a GHOST in its slot for one step, which toggles the vehicle's last mark off (that mark is in the
@@ -71,6 +71,9 @@ typedef unsigned long long u64;
 #define GEOM_LANE(g) (((g) >> 28) & 7u)
 #define GEOM_TAG(g) ((g) >> 31)
 #define GEOM_STATIC_MASK 0x0FFFFFFFu
+#define X_MASK 0x0FFFFFFFu     // S0.x: bits 0-27 position (Q22.10, edges have at most 65,535 cells), bits 28-30 stop-line counter of R8s
+#define WAIT_SHIFT 28
+#define NODE_MASK 0x07FFFFFFu  // head-node field of edge_tab / S3.z >> 4: bits 0-26 node id, bit 27 the node is a STOP node
 #define CELL_NONE 0xFFFFFFFFu
 #define ID_GHOST 0xFFFFFFFEu   // slot of a vehicle that arrived in the previous step: clears its last mark, then dies
 #ifndef MANTA_SORT_EVERY
@@ -108,8 +111,16 @@ struct DevP {
     uint32_t seed_lo, seed_hi;
     uint32_t n_edges, n_queues, flags;
     uint32_t n_seg, seg_cap;     // active-vehicle segments
+    // STOP control (R8s), per-driver desired speed (R3s), per-edge speed statistics (R9s)
+    uint32_t W_stop;             // steps a vehicle stands at the stop line of a STOP node
+    uint32_t id_mask;            // low bits of a claim key that hold the vehicle id: 2^24 - 1 if the network has STOP nodes (the turn rank sits above), else all ones
+    float v0_sigma_rel;
+    uint32_t stat_period, stat_slice, stat_n_slices;
+    u64 *stat_sum;               // [stat_n_slices * n_edges]
+    uint32_t *stat_cnt;
+    const uint4 *edge_stop;      // per edge whose head is a STOP node: {n_in * n_out of the node, in_idx * n_out, first out-edge of the node, 0}
     // network
-    const uint4 *edge_tab;       // per edge: {cell_off, geom (len | lanes | PRIORITY bit), head node, v0 bits}
+    const uint4 *edge_tab;       // per edge: {cell_off, geom (len | lanes | PRIORITY bit), head node | STOP << 27, v0 bits}
     // atlas
     u64 *bits[2];
     uint2 *pay[2];
@@ -180,6 +191,28 @@ __device__ __forceinline__ float eps_draw(const DevP &P, uint32_t id, uint32_t t
     e = e * 0.00390625f;
     e = P.eps_sigma * e;
     return e;
+}
+
+// ------------------------------------------------------------------------------------------- R3s: per-driver v0
+// every driver's desired speed on an edge is drawn around the edge's limit (reading G27):
+// v0 = limit * clamp(1 + sigma z, 1/2, 3/2), z the Irwin-Hall normal of generator words 7..9 at counter 0xFFFFFFFF - r.
+// Evaluated when a vehicle enters an edge (admission, claim winner, pre-placement) and kept in S1.w.
+__device__ __forceinline__ uint32_t desired_speed_bits(const DevP &P, uint32_t id, uint32_t r, uint32_t limit_bits)
+{
+    if (!(P.v0_sigma_rel > 0.0f)) return limit_bits;
+    int sum = 0;
+#pragma unroll
+    for (uint32_t k = 7u; k < 10u; k++) {
+        uint32_t w = rng32(P, id, 0xFFFFFFFFu - r, k);
+        sum += (int)(w & 255u) + (int)((w >> 8) & 255u) + (int)((w >> 16) & 255u) + (int)(w >> 24);
+    }
+    float z = (float)(sum - 1530);
+    z = z * 0.00390625f;
+    float f = P.v0_sigma_rel * z;
+    f = 1.0f + f;
+    f = fmaxf(f, 0.5f);
+    f = fminf(f, 1.5f);
+    return __float_as_uint(__uint_as_float(limit_bits) * f);
 }
 
 // ------------------------------------------------------------------------------------------- R3: IDM, Eq. (1)
@@ -415,7 +448,7 @@ __device__ __forceinline__ Hops build_hops(const DevP &P, uint32_t cursor, uint3
 {
     const HopRecs R = load_hop_recs(P, cursor);
     uint32_t node = 0u;
-    if (!GEOM_LAST(geom_cur) && GEOM_PRIO(geom_cur)) node = P.edge_tab[P.route[cursor].z].z;
+    if (!GEOM_LAST(geom_cur) && GEOM_PRIO(geom_cur)) node = P.edge_tab[P.route[cursor].z].z;   // (with its STOP bit)
     return make_hops(R, geom_cur, l, node);
 }
 

@@ -75,7 +75,7 @@ struct Veh {
     int32_t x;
     float v, v0;
     uint32_t id, cursor, row0, geom, prev;
-    uint32_t len_c, n, l, c, pitch;
+    uint32_t len_c, n, l, c, pitch, wait;
     bool last;
     uint32_t claim;     // S3.w
     uint32_t hopz;      // S3.z
@@ -104,7 +104,8 @@ enum { EV_LC = 0, EV_EVAL = 1, EV_DONE = 2, EV_TRAVEL = 3 };
 
 __device__ __forceinline__ void veh_load(Veh &V, const uint4 &s0v, const uint4 &s1v)
 {
-    V.x = (int32_t)s0v.x;
+    V.x = (int32_t)(s0v.x & X_MASK);
+    V.wait = s0v.x >> WAIT_SHIFT;
     V.v = __uint_as_float(s0v.y);
     V.prev = s0v.z;
     V.id = s0v.w;
@@ -452,23 +453,41 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
         else
             mark_toggle(Bn, cell);
         pay_store(P, P.pay[nxt], cell, O.nx & 1023u, __float_as_uint(O.vn));
-        S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);
+        S.S0[at] = make_uint4(O.nx | (V.wait << WAIT_SHIFT), __float_as_uint(O.vn), cur_abs, V.id);
     } else {
         if (V.prev != CELL_NONE) mark_toggle(Bn, V.prev);
+        const bool stop = GEOM_PRIO(V.geom) && (V.hopz >> 31) != 0u;   // the head node is a STOP node (R8s)
         if (O.kind == KIND_DONE) {
             P.arrive_step[V.id] = t + 1u;
             atomicAdd(&sm.ev[EV_DONE], 1ull);
             atomicAdd(&sm.ev[EV_TRAVEL], (u64)(t + 1u - P.admit_step[V.id]));
             S.S0[at] = make_uint4(0u, 0u, cur_abs, ID_GHOST);   // the ghost clears the time-t mark in the next step
+        } else if (stop && V.wait < P.W_stop) {
+            // R8s: it stands at the stop line (the place claim losers hold at, G15) one more step;
+            // no claim, nothing for the second phase
+            const uint32_t x_line = (V.len_c << 10) - 1u;
+            const uint32_t cell = V.row0 + V.len_c - 1u;       // (no lane change this close to the edge end)
+            mark_toggle(Bn, cell);
+            pay_store(P, P.pay[nxt], cell, x_line & 1023u, 0u);
+            S.S0[at] = make_uint4(x_line | ((V.wait + 1u) << WAIT_SHIFT), 0u, cur_abs, V.id);
         } else {
-            // smallest id wins; the key carries ~t in the high word so claim words never need a reset
+            // smallest key wins; the key carries ~t in the high word so claim words never need a reset
             const uint32_t target = (V.claim & ~7u) + min(O.l_new, V.claim & 7u);   // lane entry (e+, l+)
-            const uint32_t word = GEOM_PRIO(V.geom) ? P.n_edges * 8u + (V.hopz >> 4) : target;
+            const uint32_t word = GEOM_PRIO(V.geom) ? P.n_edges * 8u + ((V.hopz >> 4) & NODE_MASK) : target;
+            uint32_t key_lo = V.id;
+            if (stop) {
+                // R8s: the n x m (inbound, outbound) combinations of the node take turns; at step t
+                // combination c has rank (c - t) mod nm, the smallest rank enters, equal ranks by smallest id
+                const uint4 es = P.edge_stop[P.route[V.cursor].z];   // {nm, in_idx * m, first out-edge of the node, 0}
+                const uint32_t c = es.y + ((V.claim >> 3) - es.z);
+                const uint32_t rank = (c + es.x - t % es.x) % es.x;
+                key_lo = (rank << 24) | V.id;
+            }
             P.cand_info[V.id] = make_uint2(target, O.nx >> 10);
-            const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)V.id;
+            const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)key_lo;
             atomicMin(&P.claim[word], key);
-            P.xlist[seg_base + atomicAdd(&sm.xn, 1u)] = make_uint4(slot, word, V.cursor, V.id);
-            S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state; the second phase decides
+            P.xlist[seg_base + atomicAdd(&sm.xn, 1u)] = make_uint4(slot | (V.wait << WAIT_SHIFT), word, V.cursor, key_lo);
+            S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state (counter 0); the second phase decides
         }
     }
     if (geom_n != V.geom) S.S1[at] = make_uint4(row_n, geom_n, V.cursor, __float_as_uint(V.v0));
@@ -564,7 +583,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb)
 #pragma unroll
             for (uint32_t l = 0; l < MANTA_MAX_LANES_DEV; l++)
                 if ((uint32_t)(key[l] >> 32) == stamp && (uint32_t)key[l] != CELL_NONE) {   // (never-claimed words are all ones)
-                    const uint2 ci = P.cand_info[(uint32_t)key[l]];   // {lane entry it heads for, landing cell}
+                    const uint2 ci = P.cand_info[(uint32_t)key[l] & P.id_mask];   // {lane entry it heads for, landing cell}
 #pragma unroll
                     for (uint32_t m = 0; m < MANTA_MAX_LANES_DEV; m++)
                         if (ci.x == er.w * 8u + m) w[m] |= 1ull << (ci.y & 63u);
@@ -587,7 +606,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb)
         const uint32_t row = er.x + l_sel * pitch;
         const size_t at = (size_t)seg * P.seg_cap + slot;
         S.S0[at] = make_uint4(0u, 0u, CELL_NONE, id);
-        S.S1[at] = make_uint4(row, geom, cursor, rr.w);
+        S.S1[at] = make_uint4(row, geom, cursor, desired_speed_bits(P, id, 0u, rr.w));
         S.S2[at] = hp.s2;
         S.S3[at] = hp.s3;
         if (S.acc) S.acc[at] = 0.0f;
@@ -607,7 +626,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb)
 // Results do not depend on slot order (every rule reads time-t state only), so any order inside a bucket will do.
 __device__ __forceinline__ uint32_t sort_key(const uint4 &s0v, uint32_t row0)
 {
-    const uint32_t cell = s0v.w == ID_GHOST ? s0v.z : row0 + (s0v.x >> 10);   // a ghost sorts by the mark it has to clear
+    const uint32_t cell = s0v.w == ID_GHOST ? s0v.z : row0 + ((s0v.x & X_MASK) >> 10);   // a ghost sorts by the mark it has to clear
     return cell >> MANTA_BUCKET_SHIFT;
 }
 __device__ __forceinline__ void sort_zero(const DevP &P)
@@ -806,6 +825,20 @@ __device__ __forceinline__ void finish_deferred(const DevP &P, uint32_t t, Updat
     write_out(P, t, sm, seg_base, slot, V, O);
 }
 
+// R9s: per-edge speed statistics (inputs of Eq. 5).  In a sampling step every live vehicle adds
+// rint(v * 256) of its time-t speed to the accumulators of (time slice, its edge).  The edge id is not part of the
+// vehicle state: one gather from the route store, in sampling steps only.
+__device__ __forceinline__ void sample_speed(const DevP &P, uint32_t t, const Veh &V)
+{
+    const uint32_t slice = t / P.stat_slice;
+    if (slice >= P.stat_n_slices) return;
+    const uint32_t e = P.route[V.cursor].z;
+    const size_t k = (size_t)slice * P.n_edges + e;
+    atomicAdd(&P.stat_sum[k], (u64)__float2int_rn(V.v * 256.0f));
+    atomicAdd(&P.stat_cnt[k], 1u);
+}
+__device__ __forceinline__ bool sampling_step(const DevP &P, uint32_t t) { return P.stat_period != 0u && t % P.stat_period == 0u; }
+
 // Puts the vehicle of slot i on the deferred list of its block.  Its time-(t-1) mark is toggled off HERE, in the pass:
 // that mark may lie in an entry window the fused admission reads while the deferred stage runs (the time-(t+1) mark
 // cannot: may_defer), so the deferred stage must only ever set marks beyond the windows.
@@ -872,6 +905,7 @@ __device__ __forceinline__ void stage_search(const DevP &P, uint32_t t, UpdateSm
     int r = WIN_DONE;
     if (live) {
         n_upd += 1u;
+        if (sampling_step(P, t)) sample_speed(P, t, V);
         const uint32_t start = V.c + 1u;
         const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
         r = leader_window(P, B, V.c, V.row0, start, own, V.len_c, P.H, s2v, s3v, h, budget_left, dist_next);
@@ -1045,6 +1079,7 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
             // ---- stage 1: look-ahead (R2)
             if (live) {
                 n_upd += 1u;
+                if (sampling_step(P, t)) sample_speed(P, t, V);
                 if (W256) {
                     const uint32_t start = V.c + 1u;
                     const uint32_t own = start < V.len_c ? min(V.len_c - start, P.H) : 0u;
@@ -1144,8 +1179,8 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
         const uint32_t xstep = split ? MANTA_XT : blockDim.x;
         if (threadIdx.x < xstep)
         for (uint32_t k = threadIdx.x; k < xn; k += xstep) {
-            const uint4 xl = P.xlist[seg_base + k];     // {slot, claim word, cursor, id}
-            const size_t at = (size_t)seg_base + xl.x;
+            const uint4 xl = P.xlist[seg_base + k];     // {slot | stop-line counter << 28, claim word, cursor, low word of the claim key}
+            const size_t at = (size_t)seg_base + (xl.x & X_MASK);
             uint4 s0 = S.S0[at];
             const uint4 s1 = S.S1[at];
             const u64 won = P.claim[xl.y];
@@ -1160,16 +1195,22 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
                 uint32_t node = 0u;
                 if (!GEOM_LAST(geom) && GEOM_PRIO(geom)) node = P.edge_tab[rn.z].z;
                 const Hops hp = make_hops(hr, geom, lplus, node);
-                S.S1[at] = make_uint4(row, geom, xl.z + 1u, rn.w);
+                uint32_t v0b = rn.w;
+                if (P.v0_sigma_rel > 0.0f) {   // R3s: this driver's desired speed on the edge it enters
+                    const uint32_t id = xl.w & P.id_mask;
+                    v0b = desired_speed_bits(P, id, xl.z + 1u - P.route_start[id], rn.w);
+                }
+                S.S1[at] = make_uint4(row, geom, xl.z + 1u, v0b);
                 S.S2[at] = hp.s2;
                 S.S3[at] = hp.s3;
                 atomicAdd(&P.edge_entries[rn.z], 1u);
                 cell = row + (s0.x >> 10);
             } else {                      // loser holds at the stop line (G15)
-                s0.x = (GEOM_LEN(s1.y) << 10) - 1u;
+                const uint32_t x_line = (GEOM_LEN(s1.y) << 10) - 1u;
+                s0.x = x_line | (xl.x & ~X_MASK);      // keeps its stop-line counter (R8s)
                 s0.y = 0u;
                 S.S0[at] = s0;
-                cell = s1.x + (s0.x >> 10);
+                cell = s1.x + (x_line >> 10);
             }
             mark_toggle(Bn, cell);
             pay_store(P, payn, cell, s0.x & 1023u, s0.y);
@@ -1405,7 +1446,8 @@ __global__ void k_expand_routes(const uint4 *edge_tab, const uint32_t *row_ptr, 
         const uint32_t e = re[k];
         const uint4 er = edge_tab[e];                       // {cell_off, static geom, head node, v0}
         const uint32_t n = GEOM_LANES(er.y);
-        const uint32_t out_base = row_ptr[er.z], d = row_ptr[er.z + 1u] - out_base;
+        const uint32_t head = er.z & NODE_MASK;
+        const uint32_t out_base = row_ptr[head], d = row_ptr[head + 1u] - out_base;
         uint32_t lo = 0u, hi = n - 1u;
         if (k + 1u < total) {
             const uint32_t j = re[k + 1u] - out_base;
@@ -1441,7 +1483,7 @@ __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init
         const uint32_t geom = rr.y & GEOM_STATIC_MASK;      // lane 0, tag 0
         const Hops hp = build_hops(P, iv.w, geom, 0u);
         S.S0[at] = make_uint4(iv.x, iv.y, CELL_NONE, iv.z);   // no earlier mark
-        S.S1[at] = make_uint4(rr.x, geom, iv.w, rr.w);
+        S.S1[at] = make_uint4(rr.x, geom, iv.w, desired_speed_bits(P, iv.z, 0u, rr.w));
         S.S2[at] = hp.s2;
         S.S3[at] = hp.s3;
         const uint32_t cell = rr.x + (iv.x >> 10);
@@ -1453,7 +1495,8 @@ __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init
 }
 // Readback: scatter the live slots of the segments into per-trip arrays (caller order).
 __global__ void k_gather_state(const DevP P, int sb, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
-                               uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc)
+                               uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc, uint8_t *wait,
+                               unsigned long long *n_stopped)
 {
     const StBuf &S = P.st[sb];
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
@@ -1468,7 +1511,9 @@ __global__ void k_gather_state(const DevP P, int sb, const uint32_t *trip_of_id,
             route_pos[tr] = s1v.z - P.route_start[s0v.w];
             lane[tr] = (uint8_t)GEOM_LANE(s1v.y);
             tag[tr] = (uint8_t)GEOM_TAG(s1v.y);
-            x_fx[tr] = s0v.x;
+            x_fx[tr] = s0v.x & X_MASK;
+            wait[tr] = (uint8_t)(s0v.x >> WAIT_SHIFT);
+            if (__uint_as_float(s0v.y) == 0.0f) atomicAdd(n_stopped, 1ull);
             v[tr] = __uint_as_float(s0v.y);
             acc[tr] = S.acc ? S.acc[seg_base + i] : 0.0f;
         }

@@ -58,7 +58,7 @@ def check_monotone(prev, cur):
     assert ((prev["status"] == DONE) <= (cur["status"] == DONE)).all()
 
 
-def states_equal(a, b, keys=("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step", "arrive_step")):
+def states_equal(a, b, keys=("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step", "arrive_step", "wait")):
     """bit-exact comparison (v compared by bit pattern); returns list of (key, first bad indices)."""
     bad = []
     act = (a["status"] == ACTIVE)
@@ -67,7 +67,7 @@ def states_equal(a, b, keys=("status", "route_pos", "lane", "tag", "x_fx", "v", 
         if x.dtype == np.float32:
             x, y = x.view(np.uint32), y.view(np.uint32)
         m = x != y
-        if k in ("route_pos", "lane", "tag", "x_fx", "v", "acc"):
+        if k in ("route_pos", "lane", "tag", "x_fx", "v", "acc", "wait"):
             m = m & (act | (b["status"] == ACTIVE))  # only meaningful while ACTIVE
         if m.any():
             bad.append((k, np.nonzero(m)[0][:8].tolist()))

@@ -12,7 +12,7 @@ from tests.helpers import ACTIVE, check_conservation, check_entries, check_no_ov
 pytestmark = pytest.mark.gpu
 
 SUMMARY_KEYS = ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps", "vehicle_updates", "lane_changes",
-                "cells_examined", "lc_evals")
+                "cells_examined", "lc_evals", "n_stopped")
 
 
 @pytest.fixture(scope="module")
@@ -38,7 +38,7 @@ def describe(net, trips, o_st, g_st, idx):
 
 def compare(net, trips, o, g, label, atlas=False, acc=False):
     o_st, g_out = o.state(), g.readback()
-    keys = ("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step", "arrive_step")
+    keys = ("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step", "arrive_step", "wait")
     bad = states_equal(o_st, g_out, keys + (("acc",) if acc else ()))
     if bad:
         idx = sorted({i for _, ii in bad for i in ii})
@@ -415,13 +415,13 @@ def snapshot_parity(oracle_mod, binding, net, trips, params, checkpoints, flags=
             label = "t=%d (%d steps after the snapshot at %d, %d active)" % (t, t - t_snap, t_snap, n_act)
             o_st, g_out = o.state(), g.readback()
             bad = states_equal(o_st, g_out, ("status", "route_pos", "lane", "tag", "x_fx", "v", "admit_step",
-                                             "arrive_step") + (("acc",) if flags & 4 and k == first == 1 else ()))
+                                             "arrive_step", "wait") + (("acc",) if flags & 4 and k == first == 1 else ()))
             if bad:
                 idx = sorted({i for _, ii in bad for i in ii})
                 raise AssertionError("%s: state mismatch %s\n%s" % (label, bad, describe(net, trips, o_st, g_out, idx)))
             assert np.array_equal(o.edge_entries(), g_out["edge_entries"]), label
             gs, os_ = g_out["summary"], o.summary()
-            for key in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps"):
+            for key in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps", "n_stopped"):
                 assert gs[key] == os_[key], (label, key, gs, os_)
             for key in delta_keys:
                 assert gs[key] - g0[key] == os_[key] - o0[key], (label, key, gs, os_)
@@ -472,3 +472,82 @@ def test_parity_at_load_config4_peak(oracle_mod, binding):
     net, trips, params, _ = wl.config4(scale=1.0, n_threads=16)
     seen = snapshot_parity(oracle_mod, binding, net, trips, params, (25200,), more=5, min_active=1_500_000)
     print("configs[4]", seen)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# STOP control, N2: per-driver desired speed and per-edge speed statistics
+@pytest.mark.parametrize("flags", [0, 2, 16, 64])
+def test_stop_control_grid_every_step(oracle_mod, binding, flags):
+    """All nodes STOP: four steps at the stop line, then the round-robin over the (inbound,
+    outbound) combinations; every vehicle, its stop-line counter and the atlas equal the oracle's every step, with
+    the fused and the separate admission, in both launch modes and with two segments."""
+    net = wl.grid_network(nx=4, ny=4, edge_len=120.0, lanes=2, ctrl=2)
+    o_, d_ = wl.uniform_od(net, 700, 51)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(700, 0.0, 200.0, 52), n_threads=2)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128), 1800, dense_until=1800, atlas_every=150,
+                    flags=flags)
+    assert s["n_done"] > 150
+
+
+@pytest.mark.parametrize("stop_s", [0.0, 1.0, 3.5])
+def test_stop_control_mixed_nodes(oracle_mod, binding, stop_s):
+    """GREEN, PRIORITY and STOP nodes in one network, other standing times (0 s: only the round-robin remains)."""
+    net = wl.grid_network(nx=5, ny=4, edge_len=90.0, lanes=3, ctrl=0)
+    net["node_ctrl"] = (np.arange(20) % 3).astype(np.uint8)
+    o_, d_ = wl.uniform_od(net, 900, 61)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(900, 0.0, 240.0, 62), n_threads=2)
+    s, _ = run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128, stop_time_s=stop_s), 1500, dense_until=300,
+                    every=7, atlas_every=300)
+    assert s["n_done"] > 200 and s["lane_changes"] > 50
+
+
+def test_stop_control_limits(binding):
+    net = wl.grid_network(nx=3, ny=3, lanes=1, ctrl=2)
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(net, dict(stop_time_s=4.0))            # 8 steps: the counter has three bits
+    assert e.value.code == binding.ERR_INVALID_ARG
+    bad = dict(net)
+    bad["node_ctrl"] = np.full(9, 3, np.uint8)
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(bad)
+    assert e.value.code == binding.ERR_BAD_NETWORK
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+def test_per_driver_desired_speed(oracle_mod, binding, flags):
+    """v0_sigma_rel = 0.1: every vehicle draws its own desired speed on every edge it enters (admission, claim winner):
+    configs[2]-shaped network, bit-exact against the oracle."""
+    net, trips, params, _ = wl.config2(scale=1 / 64.0, window=(2 * 3600.0, 2 * 3600.0 + 900.0), n_threads=4)
+    params = dict(params, v0_sigma_rel=0.1)
+    # desired speeds of up to 3/2 of the limit raise Z_out (R0), and with it the shortest admissible edge, to 25 cells
+    net = dict(net, length_m=np.maximum(net["length_m"], np.float32(26.0)))
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 2400, dense_until=60, every=30, atlas_every=1200, flags=flags)
+    assert s["n_done"] > 300
+    # and it does change the run: the same demand with v0 = limit completes a different number of trips by then
+    o = oracle_mod.Oracle(net, dict(params, v0_sigma_rel=0.0), trips)
+    o.step(2400)
+    assert o.summary()["sum_travel_steps"] != s["sum_travel_steps"]
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+def test_edge_speed_statistics(oracle_mod, binding, flags):
+    """Per-edge, per-slice sums and counts of the sampled speeds (inputs of Eq. 5) equal the oracle's integers."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 4800.0), n_threads=4)
+    params = dict(params, stat_period_steps=7, stat_slice_steps=400, stat_n_slices=3)
+    o = oracle_mod.Oracle(net, params, trips)
+    g = binding.Sim(net, dict(params, flags=flags), trips)
+    for k in range(3):
+        o.step(450)
+        g.step(450)
+        so, co = o.edge_speed_stats()
+        sg, cg = g.readback_edge_speeds()
+        assert np.array_equal(co, cg) and np.array_equal(so, sg), k
+    assert co.sum() > 100000 and (co[2] > 0).any()
+    assert states_equal(o.state(), g.readback()) == []
+    g.close()
+    # statistics off: the call says so
+    g = binding.Sim(net, dict(lookahead_cells=256), trips)
+    with pytest.raises(binding.MantaError) as e:
+        g.readback_edge_speeds()
+    assert e.value.code == binding.ERR_STATE
+    g.close()
