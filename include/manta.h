@@ -186,6 +186,11 @@ int manta_readback_edge_speeds(manta_sim *sim, uint64_t *sum_q8, uint32_t *sampl
 uint64_t manta_atlas_cells(const manta_sim *sim);
 int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *cell_off, uint32_t *pitch);
 
+/* Bounds-checking build (libmanta_check.so, compiled with -DMANTA_CHECK): every index the kernels compute is compared
+ * with its array's size; returns the largest failure code seen since manta_load_trips (0 = none).  The product
+ * build has no checks compiled in and returns -1. */
+int manta_check_failures(manta_sim *sim);
+
 int manta_set_stream(manta_sim *sim, void *cuda_stream);   /* cudaStream_t; work already enqueued is not moved */
 /* Process-wide: the stream (cudaStream_t, NULL = legacy default stream) that simulations created AFTERWARDS use from
  * manta_create on (its uploads and memsets included).  All work of a simulation and the frees of manta_destroy

@@ -10,7 +10,9 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmanta.so")
+# MANTA_LIB_VARIANT=check loads the bounds-checking build (tests); every Sim.close() then fails on a recorded violation
+VARIANT = os.environ.get("MANTA_LIB_VARIANT", "")
+LIB_PATH = os.path.join(_HERE, "libmanta_check.so" if VARIANT == "check" else "libmanta.so")
 
 OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
 GREEN, PRIORITY, STOP = 0, 1, 2
@@ -23,7 +25,7 @@ EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_ste
            "manta_readback", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
            "manta_launch_count",
-           "manta_device_bytes", "manta_destroy", "manta_last_error")
+           "manta_device_bytes", "manta_destroy", "manta_last_error", "manta_check_failures")
 
 
 class MantaError(RuntimeError):
@@ -101,6 +103,7 @@ def load_library():
     L.manta_device_bytes.restype = C.c_uint64
     L.manta_destroy.argtypes = [C.c_void_p]
     L.manta_destroy.restype = None
+    L.manta_check_failures.argtypes = [C.c_void_p]
     L.manta_last_error.argtypes = [C.c_void_p]
     L.manta_last_error.restype = C.c_char_p
     _lib = L
@@ -258,10 +261,17 @@ class Sim:
     def device_bytes(self):
         return int(load_library().manta_device_bytes(self.h))
 
+    def check_failures(self):
+        """largest bounds-check failure code of the MANTA_CHECK build (0 = none); -1 in the product build"""
+        return int(load_library().manta_check_failures(self.h))
+
     def close(self):
         if getattr(self, "h", None):
+            bad = self.check_failures() if VARIANT == "check" and self.n_trips else 0
             load_library().manta_destroy(self.h)
             self.h = None
+            if bad > 0:
+                raise MantaError(ERR_STATE, "bounds check %d failed in the MANTA_CHECK build" % bad)
 
     def __del__(self):
         try:

@@ -36,15 +36,32 @@ def build_cuda(force=False, verbose=False):
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed")
-    with open(os.path.join(_HERE, "libmanta.ptxas.txt"), "w") as f:
+    with open(os.path.join(_HERE, "libmanta.ptxas.txt"), "w") as f:   # git-ignored build log (registers, spills); a copy per profile round lives under profiles/
         log = "".join(l for l in (res.stdout + res.stderr).splitlines(True) if "Compile time" not in l)
         f.write(" ".join(cmd) + "\n" + log)
     return LIB
 
 
+LIB_CHECK = os.path.join(_HERE, "libmanta_check.so")
+
+
+def build_check(force=False):
+    """The same sources with -DMANTA_CHECK: device-side bounds checks on every computed index (tests only)."""
+    if (not force and os.path.exists(LIB_CHECK)
+            and os.path.getmtime(LIB_CHECK) >= max(os.path.getmtime(d) for d in DEPS)):
+        return LIB_CHECK
+    cmd = [nvcc()] + [f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")] + ["-DMANTA_CHECK", "-o", LIB_CHECK] + SOURCES + ["-lcudart"]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed (check build)")
+    return LIB_CHECK
+
+
 def build_all(force=False, verbose=False):
     from . import workloads
     workloads.build_routing(force)
+    build_check(force)
     return build_cuda(force, verbose)
 
 
@@ -52,5 +69,6 @@ if __name__ == "__main__":
     sys.path.insert(0, _ROOT)
     from paper_2007_03614_b200 import workloads as _w
     _w.build_routing("--force" in sys.argv)
+    build_check("--force" in sys.argv)
     build_cuda("--force" in sys.argv, verbose=True)
     print(LIB)

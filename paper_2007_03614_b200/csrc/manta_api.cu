@@ -773,6 +773,21 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     dev_free(s, d_rp);
     dev_free(s, d_rowptr);
     lap("lists, initial placement, final sync");
+#ifdef MANTA_CHECK
+    {   // sizes the device-side bounds checks compare against
+        CheckCtx c{};
+        c.plane_words = ((s->n_cells / 64 + 8) + 15) & ~15ull;
+        c.pay_entries = (s->n_cells >> P.pay_shift) + 64;
+        c.n_cells = s->n_cells;
+        c.n_claims = (uint64_t)s->n_edges * 8 + s->n_nodes;
+        c.route_total = total;
+        c.slots = cap;
+        c.n_edges = s->n_edges;
+        c.n_trips = n_trips;
+        c.fail = 0;
+        CUDA_TRY(s, cudaMemcpyToSymbol(g_check, &c, sizeof c));
+    }
+#endif
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
@@ -1025,6 +1040,21 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
     }
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return MANTA_OK;
+}
+
+int manta_check_failures(manta_sim *s)
+{
+#ifdef MANTA_CHECK
+    if (!s) return -1;
+    cudaSetDevice(s->device);
+    cudaStreamSynchronize(s->stream);
+    CheckCtx c{};
+    if (cudaMemcpyFromSymbol(&c, g_check, sizeof c) != cudaSuccess) return -1;
+    return (int)c.fail;
+#else
+    (void)s;
+    return -1;
+#endif
 }
 
 int manta_readback_edge_speeds(manta_sim *s, uint64_t *sum_q8, uint32_t *samples)

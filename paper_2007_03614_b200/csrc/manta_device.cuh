@@ -23,8 +23,10 @@ typedef unsigned long long u64;
 //            the same step ends up set whatever the order, and a vehicle whose old and new mark share a word
 //            issues ONE atomic (none at all if it did not change cell).  No phase reads and writes one buffer.
 //            A 256-cell look-ahead is 4-5 words (one or two sectors).
-//   pay[2]   PAYLOAD plane, 8 bytes per cell: { frac10 of the occupant's Q22.10 position, its fp32 speed bits }.
-//            Buffer t & 1 is valid for the cells whose bit is set in bits[t & 1]; never cleared.
+//   pay[2]   PAYLOAD plane: one 8-byte entry { frac10 of the occupant's Q22.10 position, its fp32 speed bits } per
+//            aligned group of FOUR cells when vehicles are at least 4 m long (pay_shift = 2: such a group never holds
+//            two vehicles, and the occupant's cell is known from the occupancy bit), one entry per cell otherwise
+//            (pay_shift = 0).  Buffer t & 1 is valid where a bit is set in bits[t & 1]; never cleared.
 // Row (edge e, lane l) starts at cell  cell_off[e] + l * pitch(e),  pitch = len_c rounded up to 64 cells, so every
 // row starts on a word boundary and no word is shared by two rows.
 //
@@ -59,7 +61,8 @@ typedef unsigned long long u64;
 // Two per-segment lists of 16-byte entries carry the few vehicles that need the second phase: the CROSS list
 // (edge-end candidates, whose claim must be resolved) and the DEFERRED list (vehicles that must look at the
 // adjacent lane, R5, or whose look-ahead window does not fit the fast search; neither can reach its edge end in
-// this step, so nothing they do can matter to a claim).
+// this step nor mark an entry window, so nothing they do can matter to a claim or to the fused admission: both
+// lists are worked off in the same phase, by different warps).
 // ---------------------------------------------------------------------------------------------------------
 
 #define GEOM_LEN(g) ((g) & 0xFFFFu)
@@ -84,6 +87,24 @@ typedef unsigned long long u64;
 #endif
 
 enum { KIND_STAY = 0, KIND_DONE = 1, KIND_CAND = 2 };
+
+// ---------------------------------------------------------------------------------------------------------
+// Bounds checks of the MANTA_CHECK build (libmanta_check.so; compute-sanitizer is closed on the GPU pool this was
+// developed on, so the library checks its own indices): every computed index into the atlas planes, the payload
+// planes, the vehicle arrays and lists, the claim words, the route store and the per-edge arrays is compared with
+// the size of its array; the largest failure code is kept in g_check.fail and read by manta_check_failures().
+// Compiled out of the product build.
+struct CheckCtx {
+    unsigned long long plane_words, pay_entries, n_cells, n_claims, route_total, slots, n_edges, n_trips;
+    unsigned int fail;
+};
+#ifdef MANTA_CHECK
+__device__ CheckCtx g_check;
+#define MANTA_ASSERT(cond, code) do { if (!(cond)) atomicMax(&g_check.fail, (unsigned int)(code)); } while (0)
+#else
+#define MANTA_ASSERT(cond, code) do { } while (0)
+#endif
+enum { CHK_PLANE = 1, CHK_PAY = 2, CHK_CELL = 3, CHK_CLAIM = 4, CHK_ROUTE = 5, CHK_SLOT = 6, CHK_EDGE = 7, CHK_ID = 8, CHK_LIST = 9 };
 
 struct Counters {                        // grid barrier of the persistent kernel; one 128-byte line per word, so
     unsigned int bar_count, pad0[31];    // the arrival atomics, the generation polls and the abort flag do not
@@ -252,6 +273,7 @@ __device__ __forceinline__ bool first_set(const u64 *B, uint32_t row, uint32_t s
     const u64 *p = B + (row >> 6);
     uint32_t w = start >> 6;
     const uint32_t wl = (end - 1u) >> 6;
+    MANTA_ASSERT((u64)(row >> 6) + wl < g_check.plane_words, CHK_PLANE);
     u64 m = p[w];
     u64 m_next = (w < wl) ? p[w + 1u] : 0ull;
     m &= ~0ull << (start & 63u);
@@ -273,6 +295,7 @@ __device__ __forceinline__ bool last_set(const u64 *B, uint32_t row, uint32_t st
     const u64 *p = B + (row >> 6);
     uint32_t w = (end - 1u) >> 6;
     const uint32_t w0 = start >> 6;
+    MANTA_ASSERT((u64)(row >> 6) + w < g_check.plane_words, CHK_PLANE);
     u64 m = p[w];
     u64 m_next = (w > w0) ? p[w - 1u] : 0ull;
     m &= bits_below(end - (w << 6));
@@ -289,10 +312,15 @@ __device__ __forceinline__ bool last_set(const u64 *B, uint32_t row, uint32_t st
     }
 }
 // Marks are XOR toggles (see the layout comment): setting a clear bit and clearing a set bit are the same operation.
-__device__ __forceinline__ void mark_toggle(u64 *B, uint32_t cell) { atomicXor(&B[cell >> 6], 1ull << (cell & 63u)); }
+__device__ __forceinline__ void mark_toggle(u64 *B, uint32_t cell)
+{
+    MANTA_ASSERT(cell < g_check.n_cells, CHK_CELL);
+    atomicXor(&B[cell >> 6], 1ull << (cell & 63u));
+}
 // a vehicle's old mark off and new mark on, merged into one atomic when both fall in one word
 __device__ __forceinline__ void mark_move(u64 *B, uint32_t cell_old, uint32_t cell_new)
 {
+    MANTA_ASSERT(cell_old < g_check.n_cells && cell_new < g_check.n_cells, CHK_CELL);
     const u64 m_old = 1ull << (cell_old & 63u), m_new = 1ull << (cell_new & 63u);
     if ((cell_old >> 6) == (cell_new >> 6)) {
         const u64 m = m_old ^ m_new;
@@ -309,6 +337,7 @@ __device__ __forceinline__ void mark_move(u64 *B, uint32_t cell_old, uint32_t ce
 // one entry per cell (pay_shift = 0).
 __device__ __forceinline__ void pay_store(const DevP &P, uint2 *pay, uint32_t cell, uint32_t frac, uint32_t vbits)
 {
+    MANTA_ASSERT((cell >> P.pay_shift) < g_check.pay_entries, CHK_PAY);
     pay[cell >> P.pay_shift] = make_uint2(frac, vbits);
 }
 
@@ -361,6 +390,7 @@ __device__ __forceinline__ void lead_lag_w(const u64 *B, uint32_t row, uint32_t 
                                            bool &has_b, uint32_t &jb)
 {
     const u64 *p = B + (row >> 6);
+    MANTA_ASSERT((u64)(row >> 6) + ((end - 1u) >> 6) < g_check.plane_words && c < end, CHK_PLANE);
     const uint32_t w0 = c >> 6, wl = (end - 1u) >> 6;        // c < end: R4 allows lane changes only before len_c - Z_out
     const uint32_t v0 = b0 >> 6, vl = (c - 1u) >> 6;         // used only when c > b0
     const bool back = c > b0;
@@ -414,6 +444,7 @@ struct HopRecs {
 __device__ __forceinline__ HopRecs load_hop_recs(const DevP &P, uint32_t cursor)
 {
     HopRecs R;
+    MANTA_ASSERT((u64)cursor + 4u < g_check.route_total + 8u, CHK_ROUTE);
     const uint4 *rp = P.route + cursor;
 #pragma unroll
     for (int k = 0; k < 4; k++) R.r[k] = *reinterpret_cast<const uint2 *>(rp + k + 1);

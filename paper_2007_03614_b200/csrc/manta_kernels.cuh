@@ -196,7 +196,7 @@ __device__ __forceinline__ uint32_t ffs64(u64 m)   // index of the lowest set bi
 //                  vehicle's edge; at most `budget` cells are examined in total
 // Returns WIN_DONE (h valid: leader found, or the window is exhausted / the route ends), WIN_MORE (nothing found
 // and the look-ahead goes on past the four cached hops: budget_left cells remain, starting dist_next cells from
-// the tail) or WIN_NOFIT (more than MANTA_NS words: use walk_rows).
+// the tail) or WIN_NOFIT (more than MANTA_NS words and nothing in the first MANTA_NS of them: use walk_rows).
 enum { WIN_DONE = 0, WIN_MORE = 1, WIN_NOFIT = 2 };
 __device__ __forceinline__ int leader_window(const DevP &P, const u64 *B, uint32_t c, uint32_t row0, uint32_t start, uint32_t own,
                                              uint32_t dist_hops, uint32_t budget, const uint4 &s2, const uint4 &s3, Hit &h,
@@ -222,13 +222,16 @@ __device__ __forceinline__ int leader_window(const DevP &P, const u64 *B, uint32
     budget_left = rem;
     const uint32_t d1 = dist_hops, d2 = d1 + len1, d3 = d2 + len2, d4 = d3 + len3;
     dist_next = d4 + len4;
-    if (c4 > (uint32_t)MANTA_NS) return WIN_NOFIT;
+    // A window of more than MANTA_NS words: its first MANTA_NS words are searched all the same -- slots are in order
+    // of distance, so a leader found there is the leader; only if they are empty the caller must walk the rows.
+    const bool nofit = c4 > (uint32_t)MANTA_NS;
     // word address of slot s = s + A_j; distance (cells from the tail of the own edge) of bit b of slot s = 64 s + b + D_j
     const uint32_t A0 = (row0 >> 6) + w0, A1 = s2.x - c0, A2 = s2.y - c1, A3 = s2.z - c2, A4 = s2.w - c3;
     u64 m[MANTA_NS];
 #pragma unroll
     for (uint32_t s = 0; s < (uint32_t)MANTA_NS; s++) {
         const uint32_t A = s < c0 ? A0 : (s < c1 ? A1 : (s < c2 ? A2 : (s < c3 ? A3 : A4)));
+        MANTA_ASSERT(!(s < c4) || (u64)(uint32_t)(A + s) < g_check.plane_words, CHK_PLANE);   // (A_j = row word - c_j may wrap; A_j + s does not)
         m[s] = s < c4 ? B[A + s] : 0ull;
     }
     if (n0) m[0] &= ~0ull << (start & 63u);
@@ -255,6 +258,7 @@ __device__ __forceinline__ int leader_window(const DevP &P, const u64 *B, uint32
             return WIN_DONE;
         }
     }
+    if (nofit) return WIN_NOFIT;
     return (rem > 0u && (s3.z & 1u)) ? WIN_MORE : WIN_DONE;
 }
 
@@ -266,6 +270,7 @@ __device__ __forceinline__ Lead lead_from_hit(const uint2 *pay, uint32_t pay_shi
     L.lead_abs = 0;
     L.v_lead = 0.0f;
     if (h.found) {
+        MANTA_ASSERT((h.cell >> pay_shift) < g_check.pay_entries, CHK_PAY);
         const uint2 pc = pay[h.cell >> pay_shift];
         L.lead_abs = (int32_t)((h.dist << 10) | pc.x);
         L.v_lead = __uint_as_float(pc.y);
@@ -443,6 +448,7 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
     u64 *Bn = P.bits[nxt];
     const uint32_t cur_abs = V.row0 + V.c;
     const uint32_t at = seg_base + slot;
+    MANTA_ASSERT(at < g_check.slots && V.id < g_check.n_trips && (V.prev == CELL_NONE || V.prev < g_check.n_cells), CHK_SLOT);
     const bool changed = O.l_new != V.l;
     const uint32_t row_n = changed ? (O.l_new > V.l ? V.row0 + V.pitch : V.row0 - V.pitch) : V.row0;
     const uint32_t geom_n = (V.geom & GEOM_STATIC_MASK) | (O.l_new << 28) | (V.tag << 31);
@@ -485,6 +491,7 @@ __device__ __forceinline__ void write_out(const DevP &P, uint32_t t, UpdateSmem 
             }
             P.cand_info[V.id] = make_uint2(target, O.nx >> 10);
             const u64 key = ((u64)(0xFFFFFFFFu - t) << 32) | (u64)key_lo;
+            MANTA_ASSERT(word < g_check.n_claims && sm.xn < P.seg_cap, CHK_CLAIM);
             atomicMin(&P.claim[word], key);
             P.xlist[seg_base + atomicAdd(&sm.xn, 1u)] = make_uint4(slot | (V.wait << WAIT_SHIFT), word, V.cursor, key_lo);
             S.S0[at] = make_uint4(O.nx, __float_as_uint(O.vn), cur_abs, V.id);   // tentative winner state (counter 0); the second phase decides
@@ -518,6 +525,7 @@ __device__ __forceinline__ Outcome lane_change_and_finish(const DevP &P, uint32_
     int32_t x_a = 0, x_b = 0;
     float v_a = 0.0f, v_b = 0.0f;
     uint2 pa = make_uint2(0u, 0u), pb = pa;
+    MANTA_ASSERT((!has_a || ((rowt + ja) >> P.pay_shift) < g_check.pay_entries) && (!has_b || ((rowt + jb) >> P.pay_shift) < g_check.pay_entries), CHK_PAY);
     if (has_a) pa = pay[(rowt + ja) >> P.pay_shift];
     if (has_b) pb = pay[(rowt + jb) >> P.pay_shift];
     if (has_a) {
@@ -605,6 +613,7 @@ __device__ __forceinline__ void admit_phase(const DevP &P, uint32_t t, int sb)
         }
         const uint32_t row = er.x + l_sel * pitch;
         const size_t at = (size_t)seg * P.seg_cap + slot;
+        MANTA_ASSERT(at < g_check.slots && id < g_check.n_trips && cursor < g_check.route_total && rr.z < g_check.n_edges, CHK_SLOT);
         S.S0[at] = make_uint4(0u, 0u, CELL_NONE, id);
         S.S1[at] = make_uint4(row, geom, cursor, desired_speed_bits(P, id, 0u, rr.w));
         S.S2[at] = hp.s2;
@@ -732,6 +741,7 @@ __device__ __forceinline__ void sort_scatter(const DevP &P, int from, uint32_t n
             // chunks of 32 consecutive vehicles are dealt round-robin: chunk j goes to segment j % n_seg
             const uint32_t chunk = g >> 5, sd = chunk % P.n_seg;
             const size_t at = (size_t)sd * P.seg_cap + ((chunk / P.n_seg) << 5) + (g & 31u);
+            MANTA_ASSERT(at < g_check.slots && ((chunk / P.n_seg) << 5) + (g & 31u) < P.seg_cap, CHK_SLOT);
             D.S0[at] = a0;
             D.S1[at] = a1;
             D.S2[at] = a2;
@@ -772,9 +782,12 @@ __device__ __forceinline__ Hit leader_continue(const DevP &P, const u64 *B, cons
 {
     Hit h;
     uint32_t cursor = V.cursor, lane = (s3z >> 1) & 7u;
+    HopRecs R = load_hop_recs(P, cursor + 4u);
     for (int rounds = 0; rounds < 16; rounds++) {
         cursor += 4u;
-        const Hops hp = build_hops(P, cursor, 0u, lane);
+        const HopRecs Rn = load_hop_recs(P, cursor + 4u);   // the next round's records travel while this round is searched (the store is padded; a route that ended is never followed)
+        const Hops hp = make_hops(R, 0u, lane, 0u);
+        R = Rn;
         const int r = leader_window(P, B, V.c, 0u, 0u, 0u, dist_next, budget_left, hp.s2, hp.s3, h, budget_left, dist_next);
         if (r == WIN_DONE) {
             n_cells += h.found ? h.dist - V.c : P.H - budget_left;
@@ -833,6 +846,7 @@ __device__ __forceinline__ void sample_speed(const DevP &P, uint32_t t, const Ve
     const uint32_t slice = t / P.stat_slice;
     if (slice >= P.stat_n_slices) return;
     const uint32_t e = P.route[V.cursor].z;
+    MANTA_ASSERT(e < g_check.n_edges && V.cursor < g_check.route_total, CHK_EDGE);
     const size_t k = (size_t)slice * P.n_edges + e;
     atomicAdd(&P.stat_sum[k], (u64)__float2int_rn(V.v * 256.0f));
     atomicAdd(&P.stat_cnt[k], 1u);
@@ -850,6 +864,7 @@ __device__ __forceinline__ void defer_entry(const DevP &P, uint32_t t, UpdateSme
         s0v.z = CELL_NONE;
     }
     const uint32_t k = atomicAdd(&sm.qn, 1u);
+    MANTA_ASSERT(k < P.seg_cap, CHK_LIST);
 #if MANTA_DQ
     if (k < dq_cap) {
         sm.dq[k][0] = s0v;
@@ -1181,6 +1196,7 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
         for (uint32_t k = threadIdx.x; k < xn; k += xstep) {
             const uint4 xl = P.xlist[seg_base + k];     // {slot | stop-line counter << 28, claim word, cursor, low word of the claim key}
             const size_t at = (size_t)seg_base + (xl.x & X_MASK);
+            MANTA_ASSERT(at < g_check.slots && xl.y < g_check.n_claims && (u64)xl.z + 1u < g_check.route_total, CHK_LIST);
             uint4 s0 = S.S0[at];
             const uint4 s1 = S.S1[at];
             const u64 won = P.claim[xl.y];
@@ -1203,6 +1219,7 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
                 S.S1[at] = make_uint4(row, geom, xl.z + 1u, v0b);
                 S.S2[at] = hp.s2;
                 S.S3[at] = hp.s3;
+                MANTA_ASSERT(rn.z < g_check.n_edges, CHK_EDGE);
                 atomicAdd(&P.edge_entries[rn.z], 1u);
                 cell = row + (s0.x >> 10);
             } else {                      // loser holds at the stop line (G15)

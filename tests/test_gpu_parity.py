@@ -2,6 +2,8 @@
 inputs.  Integer state, occupancy, cell indices, edge transitions and counters must be identical; fp32 speeds are
 compared by bit pattern (deterministic mode: -fmad=false, same operation order)."""
 import os
+import subprocess
+import sys
 
 import numpy as np
 import pytest
@@ -458,7 +460,6 @@ BIG = pytest.mark.skipif(os.environ.get("MANTA_BIG_PARITY") != "1",
                                 "(log summarised in profiles/r02_parity_at_load.md)")
 
 
-@BIG
 def test_parity_at_load_config3_peak(oracle_mod, binding):
     """configs[3] (lane-reduced network, 6.4 M trips in 06:00-09:00) at its peak, ~1.7 M active vehicles."""
     net, trips, params, _ = wl.config3(scale=1.0, n_threads=16)
@@ -551,3 +552,37 @@ def test_edge_speed_statistics(oracle_mod, binding, flags):
         g.readback_edge_speeds()
     assert e.value.code == binding.ERR_STATE
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Bounds-checked build (compute-sanitizer is closed on the GPU pool: the library checks its own indices)
+def test_check_variant_active(binding):
+    """Runs only inside test_bounds_checked_build's subprocess: the loaded library has the checks compiled in."""
+    if binding.VARIANT != "check":
+        pytest.skip("product build")
+    net = wl.grid_network(nx=3, ny=3, lanes=2, ctrl=wl.PRIORITY)
+    o_, d_ = wl.uniform_od(net, 100, 5)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(100, 0.0, 50.0, 6), n_threads=2)
+    g = binding.Sim(net, dict(lookahead_cells=128), trips)
+    g.step(300)
+    assert g.check_failures() == 0          # (-1 would mean: no checks in this build)
+    g.close()
+
+
+def test_bounds_checked_build(binding):
+    """libmanta_check.so (-DMANTA_CHECK): every index the kernels compute -- occupancy words, payload entries, marks,
+    vehicle slots, list entries, claim words, route records, per-edge arrays -- is compared with its array's size on
+    the device; a set of the parity cases above (both launch modes, fused admission, two segments, deferred-queue
+    overflow, long look-aheads, STOP control, statistics) runs under it in a subprocess, and every Sim.close() fails
+    if a violation was recorded."""
+    assert binding.VARIANT == "", "already inside the checked run"
+    assert binding.Sim.__init__ and binding.load_library().manta_check_failures(None) == -1   # product build: no checks
+    sel = ("check_variant_active or dense_small_grid or stop_control_grid or stop_control_mixed or admission_fused or "
+           "few_segments or deferred_list_overflow or look_ahead_past or window_of_more or long_look_ahead or "
+           "config3_shaped or config4_shaped or edge_speed or per_driver or short_vehicles or edge_cases")
+    env = dict(os.environ, MANTA_LIB_VARIANT="check")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-k", sel],
+                       env=env, capture_output=True, text=True, cwd=root)
+    assert r.returncode == 0, r.stdout[-4000:] + r.stderr[-2000:]
+    assert " passed" in r.stdout and "skipped" not in r.stdout.splitlines()[-1], r.stdout[-500:]
