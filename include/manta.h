@@ -174,6 +174,17 @@ int manta_step_timed(manta_sim *sim, uint32_t n_steps, double phase_ms[3]);
 int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,
                    manta_summary *summary);
 
+/* Checkpoint / resume (and tests): replaces the dynamic state by the caller's -- the arrays manta_readback returns
+ * (caller trip order; status, route_pos, lane, tag, x_fx, v required, wait optional, acc ignored), the per-trip
+ * admit / arrive steps, the cumulative per-edge entries (NULL: kept) and the step counter t -- and rebuilds the
+ * atlas, the vehicle slots and the admission queues from it.  Summary counters that are not functions of the state
+ * (vehicle_updates, lane_changes, cells_examined, lc_evals) and the speed statistics are left to restart / continue.
+ * Errors: INVALID_ARG (missing array; status > 2; route position, lane, position, speed or counter out of range; an
+ * admitted trip queued behind a waiting one; two vehicles in one cell -- the last is found while rebuilding and
+ * leaves the handle unusable), STATE (no trips loaded), OOM, CUDA.  Otherwise a failed call changes nothing. */
+int manta_load_state(manta_sim *sim, uint32_t t, const manta_state *state, const manta_trip_result *trips,
+                     const uint32_t *edge_entries);
+
 /* Per-edge speed statistics (manta_params.stat_*): sum_q8[slice * n_edges + e] = sum over the samples of
  * rint(v * 256) (v in m/s), samples[slice * n_edges + e] = their number; mean speed = sum / (256 * samples): the
  * per-edge average the paper's calibration compares with measured speeds (Eq. 5).  Either array

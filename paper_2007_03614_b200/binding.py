@@ -22,7 +22,7 @@ FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_timed",
-           "manta_readback", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
+           "manta_readback", "manta_load_state", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
            "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error", "manta_check_failures")
@@ -91,6 +91,7 @@ def load_library():
     L.manta_step_timed.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(C.c_double * 3)]
     L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
     L.manta_readback_edge_speeds.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.manta_load_state.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(State), C.c_void_p, C.c_void_p]
     L.manta_atlas_cells.argtypes = [C.c_void_p]
     L.manta_atlas_cells.restype = C.c_uint64
     L.manta_readback_atlas.argtypes = [C.c_void_p] * 5
@@ -237,6 +238,21 @@ class Sim:
         if summary:
             out["summary"] = {k: int(getattr(sm, k)) for k, _ in Summary._fields_}
         return out
+
+    def load_state(self, t, st, edge_entries=None):
+        """manta_load_state: st = dict with status, route_pos, lane, tag, x_fx, v, admit_step, arrive_step (as readback
+        returns them) and optionally wait."""
+        n = self.n_trips
+        a = dict(status=np.ascontiguousarray(st["status"], np.uint8), route_pos=np.ascontiguousarray(st["route_pos"], np.uint32),
+                 lane=np.ascontiguousarray(st["lane"], np.uint8), tag=np.ascontiguousarray(st["tag"], np.uint8),
+                 x_fx=np.ascontiguousarray(st["x_fx"], np.uint32), v=np.ascontiguousarray(st["v"], np.float32),
+                 acc=None, wait=None if st.get("wait") is None else np.ascontiguousarray(st["wait"], np.uint8))
+        assert all(x is None or len(x) == n for x in a.values())
+        S = State(*[_ptr(a[k]) for k in ("status", "route_pos", "lane", "tag", "x_fx", "v", "acc", "wait")])
+        tr = np.ascontiguousarray(np.stack([np.asarray(st["admit_step"], np.uint32), np.asarray(st["arrive_step"], np.uint32)], 1))
+        ee = None if edge_entries is None else np.ascontiguousarray(edge_entries, np.uint32)
+        self._use()
+        self._check(load_library().manta_load_state(self.h, int(t), C.byref(S), _ptr(tr), _ptr(ee)))
 
     def readback_edge_speeds(self):
         """(sum of rint(v * 256), samples), each [stat_n_slices, n_edges] (manta_readback_edge_speeds)"""

@@ -725,6 +725,19 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if ((rc = upload(s, &d_qent, q_ent.data(), q_ent.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qend, q_end.data(), q_end.size()))) return rollback(rc);
     if ((rc = upload(s, &d_qstate, q_state.data(), q_state.size()))) return rollback(rc);
+    {   // for manta_load_state: where each queue starts, how long each route is
+        std::vector<uint32_t> q_begin(q_state.size()), route_len(n_trips);
+        for (size_t k = 0; k < q_state.size(); k++) q_begin[k] = q_state[k].y;
+        parallel_ranges(n_trips, [&](uint64_t i0, uint64_t i1) {
+            for (uint64_t id = i0; id < i1; id++) route_len[id] = (uint32_t)(route_ptr[trip_of_id[id] + 1] - route_ptr[trip_of_id[id]]);
+        });
+        uint32_t *d_qb, *d_rl;
+        if ((rc = upload(s, &d_qb, q_begin.data(), q_begin.size()))) return rollback(rc);
+        if ((rc = upload(s, &d_rl, route_len.data(), route_len.size()))) return rollback(rc);
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // the vectors go out of scope
+        P.q_begin = d_qb;
+        P.route_len = d_rl;
+    }
     if ((rc = alloc_fill(s, &P.cand_info, n_trips, 0))) return rollback(rc);
     for (int k = 0; k < 2; k++) {
         uint4 **arr[4] = {&P.st[k].S0, &P.st[k].S1, &P.st[k].S2, &P.st[k].S3};
@@ -1040,6 +1053,69 @@ int manta_readback(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_
     }
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return MANTA_OK;
+}
+
+int manta_load_state(manta_sim *s, uint32_t t, const manta_state *st, const manta_trip_result *trips, const uint32_t *edge_entries)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    if (!st || !trips || !st->status || !st->route_pos || !st->lane || !st->tag || !st->x_fx || !st->v || t >= 0xFFFFFFF0u)
+        return fail(s, MANTA_ERR_INVALID_ARG, "manta_load_state needs status, route_pos, lane, tag, x_fx, v and the trip results");
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    const uint32_t n = s->n_trips;
+    const uint64_t nn = ((uint64_t)n + 15) & ~15ull;
+    // scratch: steps uint2 | route_pos u32 | x u32 | v f32 | status u8 | lane u8 | tag u8 | wait u8 | counter, error
+    uint8_t *buf = (uint8_t *)dev_alloc(s, nn * (8 + 12 + 4) + 16);
+    if (!buf) return fail(s, MANTA_ERR_OOM, "state scratch allocation failed");
+    uint2 *d_steps = (uint2 *)buf;
+    uint32_t *d_rpos = (uint32_t *)(buf + nn * 8), *d_x = d_rpos + nn;
+    float *d_v = (float *)(d_x + nn);
+    uint8_t *d_status = (uint8_t *)(d_v + nn), *d_lane = d_status + nn, *d_tag = d_lane + nn, *d_wait = d_tag + nn;
+    uint32_t *d_counter = (uint32_t *)(d_wait + nn), *d_err = d_counter + 1;
+    auto done = [&](int rc) { cudaStreamSynchronize(s->stream); dev_free(s, buf); return rc; };
+#define TRY_LS(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { s->sticky_cuda = true; return done(fail(s, MANTA_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_))); } } while (0)
+    TRY_LS(cudaMemsetAsync(d_counter, 0, 8, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_steps, trips, (uint64_t)n * 8, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_rpos, st->route_pos, (uint64_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_x, st->x_fx, (uint64_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_v, st->v, (uint64_t)n * 4, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_status, st->status, n, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_lane, st->lane, n, cudaMemcpyHostToDevice, s->stream));
+    TRY_LS(cudaMemcpyAsync(d_tag, st->tag, n, cudaMemcpyHostToDevice, s->stream));
+    if (st->wait) TRY_LS(cudaMemcpyAsync(d_wait, st->wait, n, cudaMemcpyHostToDevice, s->stream));
+    StateIn in{d_status, d_lane, d_tag, st->wait ? d_wait : nullptr, d_rpos, d_x, d_v, d_steps};
+    const int g = (int)std::min<uint32_t>((std::max(n, s->P.n_queues) + 255) / 256, 4096);
+    // pass 1: validation only -- a bad state leaves the simulation as it was
+    k_state_validate<<<g, 256, 0, s->stream>>>(s->P, in, s->d_trip_of_id, n, d_err);
+    uint32_t h_err = 0;
+    TRY_LS(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s->stream));
+    TRY_LS(cudaStreamSynchronize(s->stream));
+    if (h_err) {
+        static const char *what[] = {"", "status value above 2", "route position beyond the trip's route", "lane, position, speed or stop counter out of range",
+                                     "an admitted trip stands behind a waiting one of the same origin edge (admission is first in, first out)"};
+        return done(fail(s, MANTA_ERR_INVALID_ARG, "manta_load_state: %s", what[std::min<uint32_t>(h_err, 4u)]));
+    }
+    // pass 2: rebuild.  Both occupancy planes empty (no vehicle has an earlier mark), claims unclaimed, counters restarted.
+    const uint64_t plane_words = ((s->n_cells / 64 + 8) + 15) & ~15ull;
+    TRY_LS(cudaMemsetAsync(s->P.bits[0], 0, 2 * plane_words * sizeof(u64), s->stream));
+    TRY_LS(cudaMemsetAsync(s->P.claim, 0xFF, ((uint64_t)s->n_edges * 8 + s->n_nodes) * sizeof(u64), s->stream));
+    TRY_LS(cudaMemsetAsync(s->P.blk, 0, sizeof(BlockStats) * s->n_blk_stats, s->stream));
+    if (edge_entries) TRY_LS(cudaMemcpyAsync(s->P.edge_entries, edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyHostToDevice, s->stream));
+    const int sb = t == 0 ? 0 : (int)(((t - 1u) / MANTA_SORT_EVERY) & 1u);
+    k_state_load<<<g, 256, 0, s->stream>>>(s->P, in, s->d_trip_of_id, n, t, sb, d_counter, d_err);
+    k_state_counts<<<(s->P.n_seg + 255) / 256, 256, 0, s->stream>>>(s->P, d_counter);
+    s->launches += 3;
+    TRY_LS(cudaGetLastError());
+    TRY_LS(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s->stream));
+    TRY_LS(cudaStreamSynchronize(s->stream));
+#undef TRY_LS
+    s->t = t;
+    if (h_err) {   // found while rebuilding: the state is unusable now
+        s->sticky_cuda = true;
+        return done(fail(s, MANTA_ERR_INVALID_ARG, "manta_load_state: two vehicles in one atlas cell; the simulation must be destroyed"));
+    }
+    return done(MANTA_OK);
 }
 
 int manta_check_failures(manta_sim *s)

@@ -162,6 +162,8 @@ struct DevP {
     uint32_t *bucket_seg;        // [n_buckets] segment that holds the bucket's vehicles: where admission appends
     // per vehicle id
     const uint32_t *route_start;
+    const uint32_t *route_len;   // entries of the trip's route (manta_load_state validates route positions against it)
+    const uint32_t *q_begin;     // [n_queues] index in q_ent of the queue's first entry (q_state moves on; this does not)
     uint32_t *admit_step;
     uint32_t *arrive_step;
     // admission queues: one FIFO per origin edge (reading G25), entries in vehicle-id order

@@ -1510,6 +1510,93 @@ __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init
         atomicAdd(&P.edge_entries[rr.z], 1u);
     }
 }
+// manta_load_state, pass 1: nothing is written but the error word (1 bad status, 2 route position beyond the route,
+// 3 lane / position beyond the edge, 4 an admitted trip behind a waiting one in its origin queue).
+struct StateIn {
+    const uint8_t *status, *lane, *tag, *wait;   // caller (trip) order; wait may be null
+    const uint32_t *route_pos, *x_fx;
+    const float *v;
+    const uint2 *steps;                          // {admit_step, arrive_step} per trip
+};
+__global__ void k_state_validate(const DevP P, StateIn in, const uint32_t *trip_of_id, uint32_t n_trips, uint32_t *err)
+{
+    for (uint32_t id = blockIdx.x * blockDim.x + threadIdx.x; id < n_trips; id += gridDim.x * blockDim.x) {
+        const uint32_t tr = trip_of_id[id];
+        const uint32_t st = in.status[tr];
+        if (st > 2u) { atomicMax(err, 1u); continue; }
+        if (st != 1u) continue;
+        if (in.route_pos[tr] >= P.route_len[id]) { atomicMax(err, 2u); continue; }
+        const uint4 rr = P.route[P.route_start[id] + in.route_pos[tr]];
+        if (in.lane[tr] >= GEOM_LANES(rr.y) || (in.x_fx[tr] >> 10) >= GEOM_LEN(rr.y) || (in.wait && in.wait[tr] > 7u) || !(in.v[tr] >= 0.0f))
+            atomicMax(err, 3u);
+    }
+    for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < P.n_queues; k += gridDim.x * blockDim.x) {
+        bool waiting_seen = false;
+        for (uint32_t i = P.q_begin[k]; i < P.q_end[k]; i++) {
+            const bool waiting = in.status[trip_of_id[P.q_ent[i].x]] == 0u;
+            if (waiting_seen && !waiting) atomicMax(err, 4u);
+            waiting_seen = waiting_seen || waiting;
+        }
+    }
+}
+// pass 2: per-id results, vehicle slots (dealt round-robin over the segments through one counter), marks and payload of
+// atlas_t (the other plane is empty: no vehicle has an earlier mark), arrival counters, queue heads.
+__global__ void k_state_load(const DevP P, StateIn in, const uint32_t *trip_of_id, uint32_t n_trips, uint32_t t, int sb,
+                             uint32_t *slot_counter, uint32_t *err)
+{
+    const StBuf &S = P.st[sb];
+    u64 *B = P.bits[t & 1u];
+    uint2 *pay = P.pay[t & 1u];
+    unsigned long long done = 0ull, travel = 0ull;
+    for (uint32_t id = blockIdx.x * blockDim.x + threadIdx.x; id < n_trips; id += gridDim.x * blockDim.x) {
+        const uint32_t tr = trip_of_id[id];
+        const uint2 steps = in.steps[tr];
+        P.admit_step[id] = steps.x;
+        P.arrive_step[id] = steps.y;
+        const uint32_t st = in.status[tr];
+        if (st == 2u) {
+            done += 1ull;
+            travel += (unsigned long long)(steps.y - steps.x);
+        }
+        if (st != 1u) continue;
+        const uint32_t cursor = P.route_start[id] + in.route_pos[tr];
+        const uint4 rr = P.route[cursor];
+        const uint32_t l = in.lane[tr];
+        const uint32_t geom = (rr.y & GEOM_STATIC_MASK) | (l << 28) | ((uint32_t)(in.tag[tr] != 0u) << 31);
+        const uint32_t row = rr.x + l * pitch_of(GEOM_LEN(rr.y));
+        const Hops hp = build_hops(P, cursor, geom, l);
+        const uint32_t slot = atomicAdd(slot_counter, 1u);
+        const size_t at = (size_t)(slot % P.n_seg) * P.seg_cap + slot / P.n_seg;
+        const uint32_t x = in.x_fx[tr], vb = __float_as_uint(in.v[tr]);
+        S.S0[at] = make_uint4(x | ((in.wait ? (uint32_t)in.wait[tr] : 0u) << WAIT_SHIFT), vb, CELL_NONE, id);
+        S.S1[at] = make_uint4(row, geom, cursor, desired_speed_bits(P, id, in.route_pos[tr], rr.w));
+        S.S2[at] = hp.s2;
+        S.S3[at] = hp.s3;
+        if (S.acc) S.acc[at] = 0.0f;
+        const uint32_t cell = row + (x >> 10);
+        const u64 bit = 1ull << (cell & 63u);
+        if (atomicOr(&B[cell >> 6], bit) & bit) atomicMax(err, 5u);   // two vehicles in one cell
+        pay_store(P, pay, cell, x & 1023u, vb);
+    }
+    if (done) {
+        atomicAdd(&P.blk[blockIdx.x % 64u].n_done, done);
+        atomicAdd(&P.blk[blockIdx.x % 64u].sum_travel, travel);
+    }
+    for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < P.n_queues; k += gridDim.x * blockDim.x) {
+        uint32_t i = P.q_begin[k];
+        const uint32_t end = P.q_end[k];
+        while (i < end && in.status[trip_of_id[P.q_ent[i].x]] != 0u) i++;
+        const uint4 h = P.q_ent[i];   // (the padding entry after the last queue if i == total)
+        P.q_state[k] = i < end ? make_uint4(h.y, i, h.x, h.z) : make_uint4(CELL_NONE, i, CELL_NONE, 0u);
+    }
+}
+__global__ void k_state_counts(const DevP P, const uint32_t *slot_counter)
+{
+    const uint32_t total = *slot_counter;
+    for (uint32_t seg = blockIdx.x * blockDim.x + threadIdx.x; seg < P.n_seg; seg += gridDim.x * blockDim.x)
+        P.seg_cnt[seg] = total / P.n_seg + (seg < total % P.n_seg ? 1u : 0u);
+}
+
 // Readback: scatter the live slots of the segments into per-trip arrays (caller order).
 __global__ void k_gather_state(const DevP P, int sb, const uint32_t *trip_of_id, uint8_t *status, uint32_t *route_pos,
                                uint8_t *lane, uint8_t *tag, uint32_t *x_fx, float *v, float *acc, uint8_t *wait,

@@ -586,3 +586,73 @@ def test_bounds_checked_build(binding):
                        env=env, capture_output=True, text=True, cwd=root)
     assert r.returncode == 0, r.stdout[-4000:] + r.stderr[-2000:]
     assert " passed" in r.stdout and "skipped" not in r.stdout.splitlines()[-1], r.stdout[-500:]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# manta_load_state: checkpoint / resume, and the oracle's state injected into the library
+@pytest.mark.parametrize("t_snap", [1, 64, 130, 191])
+def test_load_state_from_the_oracle(oracle_mod, binding, t_snap):
+    """The oracle runs to t_snap; its state goes into a fresh simulation through manta_load_state; from there both are
+    compared every step (atlas included).  t_snap = 64 sits on a spatial re-sort, 1 / 191 are odd steps (the other
+    occupancy plane is the current one)."""
+    net = wl.grid_network(nx=5, ny=4, edge_len=90.0, lanes=3, ctrl=0)
+    net["node_ctrl"] = (np.arange(20) % 3).astype(np.uint8)          # GREEN, PRIORITY and STOP nodes
+    o_, d_ = wl.uniform_od(net, 900, 61)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(900, 0.0, 240.0, 62), n_threads=2)
+    params = dict(lookahead_cells=128)
+    o = oracle_mod.Oracle(net, params, trips)
+    o.step(t_snap)
+    g = binding.Sim(net, params, trips)
+    g.load_state(t_snap, o.state(), o.edge_entries())
+    base = o.summary()
+    for k in range(150):
+        o.step(1)
+        g.step(1)
+        o_st, g_out = o.state(), g.readback()
+        assert states_equal(o_st, g_out) == [], (t_snap, k, states_equal(o_st, g_out))
+        assert np.array_equal(o.edge_entries(), g_out["edge_entries"])
+        os_, gs = o.summary(), g_out["summary"]
+        for key in ("t", "n_waiting", "n_active", "n_done", "sum_travel_steps", "n_stopped"):
+            assert os_[key] == gs[key], (key, os_, gs)
+        assert gs["vehicle_updates"] == os_["vehicle_updates"] - base["vehicle_updates"]   # counters restart at the load
+        if k % 25 == 0:
+            compare_atlas_sparse(o, g, "t=%d" % (t_snap + k + 1))
+    g.close()
+
+
+def test_load_state_checkpoint_and_rewind(oracle_mod, binding):
+    """A snapshot read back at step 700 of a congested configs[3]-shaped run resumes in a NEW simulation and, later,
+    in the same one (rewind): all three continuations are identical, and equal to the oracle's."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5100.0), n_threads=4)
+    a = binding.Sim(net, params, trips)
+    a.step(700)
+    snap = a.readback()
+    b = binding.Sim(net, params, trips)
+    b.load_state(700, snap, snap["edge_entries"])
+    o = oracle_mod.Oracle(net, params, trips)
+    o.set_state(700, snap, snap["edge_entries"])
+    a.step(500)
+    b.step(500)
+    o.step(500)
+    ra, rb = a.readback(), b.readback()
+    assert states_equal(ra, rb) == [] and states_equal(o.state(), rb) == []
+    assert np.array_equal(ra["edge_entries"], rb["edge_entries"]) and np.array_equal(o.edge_entries(), rb["edge_entries"])
+    a.load_state(700, snap, snap["edge_entries"])                     # rewind the first one
+    a.step(500)
+    assert states_equal(a.readback(), rb) == []
+    # a bad state is refused and changes nothing
+    bad = dict(snap)
+    bad["lane"] = np.full_like(snap["lane"], 7)
+    with pytest.raises(binding.MantaError) as e:
+        b.load_state(1200, bad, None)
+    assert e.value.code == binding.ERR_INVALID_ARG
+    bad = dict(snap)
+    bad["route_pos"] = snap["route_pos"] + 10000
+    with pytest.raises(binding.MantaError) as e:
+        b.load_state(1200, bad, None)
+    assert e.value.code == binding.ERR_INVALID_ARG
+    b.step(100)
+    o.step(100)
+    assert states_equal(o.state(), b.readback()) == []
+    a.close()
+    b.close()
