@@ -10,9 +10,10 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# MANTA_LIB_VARIANT=check loads the bounds-checking build (tests); every Sim.close() then fails on a recorded violation
+# MANTA_LIB_VARIANT=check loads the bounds-checking build (tests; every Sim.close() then fails on a recorded violation),
+# MANTA_LIB_VARIANT=fast the fast-mode build (FMA contraction allowed: not bit-exact against the oracle)
 VARIANT = os.environ.get("MANTA_LIB_VARIANT", "")
-LIB_PATH = os.path.join(_HERE, "libmanta_check.so" if VARIANT == "check" else "libmanta.so")
+LIB_PATH = os.path.join(_HERE, {"check": "libmanta_check.so", "fast": "libmanta_fast.so"}.get(VARIANT, "libmanta.so"))
 
 OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
 GREEN, PRIORITY, STOP = 0, 1, 2

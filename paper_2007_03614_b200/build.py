@@ -58,10 +58,29 @@ def build_check(force=False):
     return LIB_CHECK
 
 
+LIB_FAST = os.path.join(_HERE, "libmanta_fast.so")
+
+
+def build_fast(force=False):
+    """Fast mode: the same sources with FMA contraction allowed (-fmad=true).  Not bit-exact against
+    the oracle: held to a per-step tolerance instead (tests/test_gpu_parity.py::test_fast_mode_one_step)."""
+    if (not force and os.path.exists(LIB_FAST)
+            and os.path.getmtime(LIB_FAST) >= max(os.path.getmtime(d) for d in DEPS)):
+        return LIB_FAST
+    flags = ["-fmad=true" if f == "-fmad=false" else f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")]
+    cmd = [nvcc()] + flags + ["-DMANTA_FAST", "-o", LIB_FAST] + SOURCES + ["-lcudart"]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed (fast build)")
+    return LIB_FAST
+
+
 def build_all(force=False, verbose=False):
     from . import workloads
     workloads.build_routing(force)
     build_check(force)
+    build_fast(force)
     return build_cuda(force, verbose)
 
 
@@ -70,5 +89,6 @@ if __name__ == "__main__":
     from paper_2007_03614_b200 import workloads as _w
     _w.build_routing("--force" in sys.argv)
     build_check("--force" in sys.argv)
+    build_fast("--force" in sys.argv)
     build_cuda("--force" in sys.argv, verbose=True)
     print(LIB)

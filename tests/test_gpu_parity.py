@@ -656,3 +656,61 @@ def test_load_state_checkpoint_and_rewind(oracle_mod, binding):
     assert states_equal(o.state(), b.readback()) == []
     a.close()
     b.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# fast mode (libmanta_fast.so: FMA contraction allowed), held to tolerances instead of bit-exactness
+def test_fast_variant_one_step_and_aggregates(oracle_mod, binding):
+    """Runs only inside test_fast_mode's subprocess (MANTA_LIB_VARIANT=fast).  From IDENTICAL state (the oracle's,
+    through manta_load_state) one step: speeds within 1e-5 relative (north_star), accelerations within 1e-5 of
+    max(|acc|, a) -- Eq. 1 is a difference of O(a) terms, so near equilibrium |acc| << a and an error of one ulp of
+    the terms is more than 1e-5 of acc itself (fast mode) --, positions within one fixed-point
+    unit, same lanes / edges.  Then 1,500 steps on its own: completions, mean travel time and per-edge entries within
+    0.5 % of the oracle's (north_star's bar for runs that are not bit-exact)."""
+    if binding.VARIANT != "fast":
+        pytest.skip("product build")
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5100.0), n_threads=4)
+    o = oracle_mod.Oracle(net, params, trips)
+    o.step(800)
+    g = binding.Sim(net, dict(params, flags=4), trips)
+    worst_v = worst_a = 0.0
+    for rep in range(6):
+        g.load_state(800 + rep * 40, o.state(), o.edge_entries())
+        o.step(1)
+        g.step(1)
+        a, b = o.state(), g.readback()
+        assert np.array_equal(a["status"], b["status"])
+        act = a["status"] == ACTIVE
+        assert act.sum() > 5000
+        assert np.array_equal(a["lane"][act], b["lane"][act]) and np.array_equal(a["route_pos"][act], b["route_pos"][act])
+        dx = np.abs(a["x_fx"][act].astype(np.int64) - b["x_fx"][act].astype(np.int64))
+        dv = np.abs(a["v"][act].astype(np.float64) - b["v"][act]) / np.maximum(np.abs(a["v"][act]), 1e-3)
+        da = np.abs(a["acc"][act].astype(np.float64) - b["acc"][act]) / np.maximum(np.abs(a["acc"][act]), 1.0)
+        assert dx.max() <= 1 and dv.max() <= 1e-5 and da.max() <= 1e-5, (rep, dx.max(), dv.max(), da.max())
+        worst_v, worst_a = max(worst_v, dv.max()), max(worst_a, da.max())
+        o.step(39)
+    print("fast mode, one step from identical state: max rel dv %.2e, max dacc / max(|acc|, 1) %.2e" % (worst_v, worst_a))
+    g.close()
+    g = binding.Sim(net, params, trips)
+    o = oracle_mod.Oracle(net, params, trips)
+    g.step(1500)
+    o.step(1500)
+    gs, os_ = g.readback(), o.summary()
+    assert abs(gs["summary"]["n_done"] - os_["n_done"]) <= 0.005 * os_["n_done"]
+    mt_g = gs["summary"]["sum_travel_steps"] / gs["summary"]["n_done"]
+    mt_o = os_["sum_travel_steps"] / os_["n_done"]
+    assert abs(mt_g - mt_o) <= 0.005 * mt_o
+    ee_o, ee_g = o.edge_entries().astype(np.int64), gs["edge_entries"].astype(np.int64)
+    busy = ee_o >= 100
+    assert busy.sum() > 20 and np.abs(ee_g[busy] - ee_o[busy]).sum() <= 0.005 * ee_o[busy].sum()
+    g.close()
+
+
+def test_fast_mode(binding):
+    """libmanta_fast.so (same sources, -fmad=true) against the oracle, in a subprocess (one library per process)."""
+    assert binding.VARIANT == ""
+    env = dict(os.environ, MANTA_LIB_VARIANT="fast")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-s", "-k",
+                        "fast_variant_one_step"], env=env, capture_output=True, text=True, cwd=root)
+    assert r.returncode == 0 and "1 passed" in r.stdout, r.stdout[-4000:] + r.stderr[-2000:]
