@@ -714,3 +714,65 @@ def test_fast_mode(binding):
     r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-s", "-k",
                         "fast_variant_one_step"], env=env, capture_output=True, text=True, cwd=root)
     assert r.returncode == 0 and "1 passed" in r.stdout, r.stdout[-4000:] + r.stderr[-2000:]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# The limits the library states (include/manta.h, DESIGN.md section 6 "Limits"): cases AT the limits run and match
+# the oracle; one step beyond is refused with an error code.
+def test_limits_of_the_layout(oracle_mod, binding):
+    """An edge of 65,535 cells (the 16-bit length field) with 8 lanes (the 3-bit lane fields), the shortest admissible
+    edges (LEN_MIN = 10 cells at a 13.9 m/s limit), a node of out-degree 255 (the 8-bit turn index of R0), H = 256 and
+    look-back 128 (the widest single-round scans): bit-exact against the oracle; length 65,536, 9 lanes, out-degree
+    256, a 9-cell edge are BAD_NETWORK."""
+    V0 = 50 / 3.6
+    # node 0 -> 1: the long 8-lane edge; 1 -> 2..256: 255 short out-edges (10 cells); each of those -> 257 (sink edge 12 m)
+    n_out = 255
+    tail = [0] + [1] * n_out + list(range(2, 2 + n_out))
+    head = [1] + list(range(2, 2 + n_out)) + [2 + n_out] * n_out
+    length = [65535.0] + [10.0] * n_out + [12.0] * n_out
+    lanes = [8] + [1] * n_out + [2] * n_out
+
+    def make(length, lanes, tail=tail, head=head):
+        net = wl._csr_from_edges(3 + n_out, np.array(tail, np.int64), np.array(head, np.int64),
+                                 length_m=np.array(length, np.float32), lanes=np.array(lanes, np.uint8),
+                                 speed_limit=np.full(len(tail), V0, np.float32))
+        net["node_ctrl"] = np.zeros(3 + n_out, np.uint8)
+        return net
+    net = make(length, lanes)
+    # 120 vehicles pre-placed (lane 0, R1) near the far end of the long edge, heading for random exits
+    n = 120
+    first_out = int(net["row_ptr"][1])
+    rng_ = np.random.default_rng(5)
+    outs = rng_.integers(0, n_out, n)
+    routes = np.stack([np.zeros(n, np.int64), first_out + outs, first_out + n_out + outs], 1)
+    trips = dict(route_ptr=np.arange(0, 3 * n + 1, 3, dtype=np.uint64), route_edges=routes.astype(np.uint32).ravel(),
+                 depart_time_s=np.zeros(n, np.float32), init_pos_m=(65500.0 - 12.0 * np.arange(n)).astype(np.float32),
+                 init_speed=rng_.uniform(0.0, 12.0, n).astype(np.float32))
+    params = dict(lookahead_cells=256, lookback_cells=128)
+    s, _ = run_both(oracle_mod, binding, net, trips, params, 700, dense_until=700, atlas_every=0)
+    assert s["n_done"] > 60 and s["lane_changes"] > 30
+    for bad_len, bad_lanes, code in (([65536.0] + length[1:], lanes, binding.ERR_BAD_NETWORK),
+                                     (length, [9] + lanes[1:], binding.ERR_BAD_NETWORK),
+                                     (length[:1] + [9.0] + length[2:], lanes, binding.ERR_BAD_NETWORK)):
+        with pytest.raises(binding.MantaError) as e:
+            binding.Sim(make(bad_len, bad_lanes), params)
+        assert e.value.code == code
+    t2, h2 = tail + [1], head + [2 + n_out]                       # a 256th out-edge of node 1
+    with pytest.raises(binding.MantaError) as e:
+        binding.Sim(make(length + [12.0], lanes + [1], t2, h2), params)
+    assert e.value.code == binding.ERR_BAD_NETWORK
+    for p_bad in (dict(lookahead_cells=8193), dict(veh_len=63.0), dict(lookback_cells=0)):
+        with pytest.raises(binding.MantaError) as e:
+            binding.Sim(net, p_bad)
+        assert e.value.code == binding.ERR_INVALID_ARG
+
+
+def test_idle_and_tiny_inputs(oracle_mod, binding):
+    """Nothing to do for hundreds of steps (all departures in the future), then one vehicle; a trip whose route is one
+    edge; a run that ends with everybody arrived and keeps stepping."""
+    net = wl.straight_road(n_edges=3, length_m=40.0, lanes=2)
+    trips = dict(route_ptr=np.array([0, 3, 4], np.uint64), route_edges=np.array([0, 1, 2, 1], np.uint32),
+                 depart_time_s=np.array([200.0, 201.0], np.float32), init_pos_m=None, init_speed=None)
+    for flags in (0, 2):
+        s, _ = run_both(oracle_mod, binding, net, trips, None, 700, dense_until=0, every=70, flags=flags)
+        assert s["n_done"] == 2 and s["n_active"] == 0 and s["vehicle_updates"] > 0
