@@ -164,6 +164,15 @@ int manta_step(manta_sim *sim, uint32_t n_steps);
 int manta_step_async(manta_sim *sim, uint32_t n_steps);
 int manta_sync(manta_sim *sim);
 
+/* Replica batching (the calibration runs several parameter sets per iteration): advances 2..4
+ * independent simulations -- each created and loaded on its own, typically the same network and demand with
+ * different model parameters -- by n_steps in ONE cooperative launch per 8,192 steps; every phase works through all
+ * replicas between the same two grid barriers, so the per-step synchronisation is paid once for the batch.  Results
+ * of every replica are exactly those of stepping it alone.  All simulations must be on the same device and stream, at
+ * the same step counter, with the same launch geometry (n_sims = 1: plain manta_step).  Errors: INVALID_ARG, STATE
+ * (the batch does not fit the device's shared memory), CUDA.  Returns after the steps completed. */
+int manta_step_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps);
+
 /* Same as manta_step, with CUDA events recorded on the simulation's stream around every phase; adds the device
  * time of the admission, update and second (claim resolution) phases (ms, summed over the n_steps) to phase_ms[0..2].
  * For measurement only (the events cost a little); results are identical to manta_step. */

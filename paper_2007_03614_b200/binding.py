@@ -22,6 +22,7 @@ NONE = 0xFFFFFFFF
 FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
+           "manta_step_batch",
            "manta_step_timed",
            "manta_readback", "manta_load_state", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
@@ -89,6 +90,7 @@ def load_library():
     for f in ("manta_step", "manta_step_async"):
         getattr(L, f).argtypes = [C.c_void_p, C.c_uint32]
     L.manta_sync.argtypes = [C.c_void_p]
+    L.manta_step_batch.argtypes = [C.POINTER(C.c_void_p), C.c_uint32, C.c_uint32]
     L.manta_step_timed.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(C.c_double * 3)]
     L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
     L.manta_readback_edge_speeds.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -140,6 +142,14 @@ def use_torch_allocator():
 
 def _ptr(a):
     return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def step_batch(sims, n=1):
+    """manta_step_batch: advance several simulations (same device, stream, step counter) in one launch."""
+    arr = (C.c_void_p * len(sims))(*[s.h for s in sims])
+    rc = load_library().manta_step_batch(arr, len(sims), int(n))
+    if rc != OK:
+        raise MantaError(rc, load_library().manta_last_error(sims[0].h).decode())
 
 
 class Sim:

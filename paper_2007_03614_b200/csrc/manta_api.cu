@@ -690,7 +690,8 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     P.n_seg = (uint32_t)s->grid_step;
     P.seg_cap = (n_trips + P.n_seg - 1u) / P.n_seg + 256u;
     const uint64_t cap = (uint64_t)P.n_seg * P.seg_cap;
-    if (cap >= 0xFFFFFFFFull) return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
+    if (cap >= 0xFFFFFFFFull || P.seg_cap >= (1u << 28))   // list entries keep the slot in 28 bits (cross list) / 30 bits (deferred list)
+        return rollback(fail(s, MANTA_ERR_INVALID_ARG, "too many trips for the segment layout"));
     // ---- upload; expand the route store on the device
     int rc;
     uint32_t *d_rowptr = nullptr, *d_rs, *d_adm, *d_arr, *d_qend;
@@ -921,6 +922,69 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
     }
     CUDA_TRY(s, cudaGetLastError());
     return MANTA_OK;
+}
+
+namespace {
+extern "C++" template <int NB>
+int launch_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps, bool w256, int fuse)
+{
+    manta_sim *s0 = sims[0];
+    BatchP<NB> bp{};
+    for (uint32_t r = 0; r < (uint32_t)NB; r++) bp.p[r] = sims[std::min(r, n_sims - 1u)]->P;
+    void (*kern)(BatchP<NB>, int, uint32_t, uint32_t, int) = w256 ? k_persistent_batch<true, NB> : k_persistent_batch<false, NB>;
+    const size_t smem = MANTA_BATCH_SMEM(NB);
+    CUDA_TRY(s0, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CUDA_TRY(s0, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, MANTA_NT, smem));
+    if (occ * s0->sm_count < s0->grid_persist)
+        return fail(s0, MANTA_ERR_STATE, "a batch of %u simulations does not fit the device next to each other (%d blocks per SM)", n_sims, occ);
+    for (uint32_t done = 0; done < n_steps;) {
+        const uint32_t m = std::min<uint32_t>(n_steps - done, 8192u), t0 = s0->t + done;
+        CUDA_TRY(s0, cudaMemsetAsync(&s0->P.ctr->bar_count, 0, 33 * sizeof(unsigned int), s0->stream));
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeCooperative;
+        at[0].val.cooperative = 1;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)s0->grid_persist);
+        cfg.blockDim = dim3(MANTA_NT);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = s0->stream;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;   // no L2 window: each replica has its own occupancy planes, together beyond the carve-out
+        CUDA_TRY(s0, cudaLaunchKernelEx(&cfg, kern, bp, (int)n_sims, t0, m, fuse));
+        s0->launches += 1;
+        done += m;
+    }
+    return MANTA_OK;
+}
+}  // namespace
+
+int manta_step_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps)
+{
+    if (!sims || n_sims == 0 || !sims[0]) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null batch");
+    if (n_sims == 1) return manta_step(sims[0], n_steps);
+    manta_sim *s0 = sims[0];
+    if (n_sims > 4) return fail(s0, MANTA_ERR_INVALID_ARG, "at most 4 simulations per batch");
+    bool fuse = true;
+    for (uint32_t r = 0; r < n_sims; r++) {
+        manta_sim *s = sims[r];
+        const int rc = check_ready(s, n_steps);
+        if (rc) return rc;
+        for (uint32_t q = 0; q < r; q++)
+            if (sims[q] == s) return fail(s0, MANTA_ERR_INVALID_ARG, "a simulation appears twice in the batch");
+        if (s->device != s0->device || s->stream != s0->stream || s->t != s0->t || s->grid_persist != s0->grid_persist ||
+            s->w256 != s0->w256 || s->P.n_seg != s0->P.n_seg || s->grid_persist == 0)
+            return fail(s0, MANTA_ERR_INVALID_ARG, "simulations of a batch must share device, stream, step counter and launch geometry "
+                                                   "(same look-ahead class, persistent kernel available)");
+        fuse = fuse && s->fuse_admit;
+    }
+    CUDA_TRY(s0, cudaSetDevice(s0->device));
+    int rc = n_sims == 2 ? launch_batch<2>(sims, n_sims, n_steps, s0->w256, fuse ? 1 : 0)
+                         : launch_batch<4>(sims, n_sims, n_steps, s0->w256, fuse ? 1 : 0);
+    if (rc) return rc;
+    CUDA_TRY(s0, cudaGetLastError());
+    for (uint32_t r = 0; r < n_sims; r++) sims[r]->t += n_steps;
+    return manta_sync(s0);
 }
 
 int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])

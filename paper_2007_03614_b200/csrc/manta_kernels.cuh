@@ -94,6 +94,7 @@ struct Outcome {
 // shared memory of the step kernels
 struct UpdateSmem {
     u64 ev[4];                    // event counters of this launch (up to 8,192 timesteps): lane changes, lane-change evaluations, arrivals, travel steps
+    u64 wcnt[MANTA_NT / 32][2];   // replica batching only: cells examined, vehicle-updates per warp (its lane 0 adds, no atomics; per-thread registers in the single-simulation kernels)
     uint32_t xn, qn, flag, next;  // per segment: cross-list / deferred-list entries, next unclaimed chunk; barrier flag
     uint32_t wsum[MANTA_NW];      // re-sort: per-warp partial sums
 #if MANTA_DQ
@@ -1159,8 +1160,11 @@ __device__ __forceinline__ void update_phase(const DevP &P, uint32_t t, UpdateSm
 #ifndef MANTA_XT
 #define MANTA_XT 128u   // threads of a block that take cross-list entries in the second phase; the others take deferred entries
 #endif
+// Replica batching (k_persistent_batch): replica r of n gets its own share of both thread ranges, so that the chains of
+// the replicas run side by side as well.
 template <bool W256>
-__device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, bool persistent)
+__device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSmem &sm, uint32_t &n_cells, bool persistent,
+                                             uint32_t r = 0u, uint32_t n = 1u)
 {
     const int nxt = (int)((t & 1u) ^ 1u);
     const StBuf &S = P.st[sbuf_of(t)];
@@ -1168,13 +1172,14 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
     uint2 *payn = P.pay[nxt];
     const uint32_t dq_cap = dq_capacity(P, persistent);
     const bool split = blockDim.x > MANTA_XT;
+    const uint32_t xw = split ? max(32u, (MANTA_XT / n) & ~31u) : blockDim.x, x_lo = split ? xw * r : 0u;
+    const uint32_t dw = split ? max(32u, ((blockDim.x - MANTA_XT) / n) & ~31u) : blockDim.x, d_lo = split ? MANTA_XT + dw * r : 0u;
     for (uint32_t seg = blockIdx.x; seg < P.n_seg; seg += gridDim.x) {
         const uint32_t xn = persistent ? sm.xn : P.seg_xn[seg];
         const uint32_t qn = persistent ? sm.qn : P.seg_qn[seg];
         const uint32_t seg_base = seg * P.seg_cap;
-        const uint32_t d0 = split ? MANTA_XT : 0u, dstep = blockDim.x - d0;
-        if (threadIdx.x >= d0)
-            for (uint32_t k = threadIdx.x - d0; k < qn; k += dstep) {
+        if (threadIdx.x >= d_lo && threadIdx.x < d_lo + dw)
+            for (uint32_t k = threadIdx.x - d_lo; k < qn; k += dw) {
                 uint4 e, a0, a1;   // one call site: finish_deferred is ~2 k instructions
 #if MANTA_DQ
                 if (k < dq_cap) {
@@ -1191,9 +1196,8 @@ __device__ __forceinline__ void second_phase(const DevP &P, uint32_t t, UpdateSm
                 }
                 finish_deferred<W256>(P, t, sm, seg_base, e, a0, a1, n_cells);
             }
-        const uint32_t xstep = split ? MANTA_XT : blockDim.x;
-        if (threadIdx.x < xstep)
-        for (uint32_t k = threadIdx.x; k < xn; k += xstep) {
+        if (threadIdx.x >= x_lo && threadIdx.x < x_lo + xw)
+        for (uint32_t k = threadIdx.x - x_lo; k < xn; k += xw) {
             const uint4 xl = P.xlist[seg_base + k];     // {slot | stop-line counter << 28, claim word, cursor, low word of the claim key}
             const size_t at = (size_t)seg_base + (xl.x & X_MASK);
             MANTA_ASSERT(at < g_check.slots && xl.y < g_check.n_claims && (u64)xl.z + 1u < g_check.route_total, CHK_LIST);
@@ -1384,19 +1388,19 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     return *s_flag == 0u;
 }
 
-__device__ __forceinline__ bool sort_all(const DevP &P, UpdateSmem &sm, int from, unsigned &gen)
+__device__ __forceinline__ bool sort_all(const DevP &P, UpdateSmem &sm, int from, unsigned &gen, Counters *ctr)
 {
     uint32_t n_live, per_seg;
     sort_zero(P);
-    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    if (!grid_barrier(ctr, gen, &sm.flag)) return false;
     sort_count(P, from);
-    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    if (!grid_barrier(ctr, gen, &sm.flag)) return false;
     sort_partial(P, sm);
-    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    if (!grid_barrier(ctr, gen, &sm.flag)) return false;
     sort_scan(P, sm, n_live, per_seg);
-    if (!grid_barrier(P.ctr, gen, &sm.flag)) return false;
+    if (!grid_barrier(ctr, gen, &sm.flag)) return false;
     sort_scatter(P, from, n_live, per_seg);
-    return grid_barrier(P.ctr, gen, &sm.flag);
+    return grid_barrier(ctr, gen, &sm.flag);
 }
 
 // One cooperative launch = n_steps timesteps; the host is not involved between steps.  Two grid barriers per
@@ -1410,7 +1414,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
     uint32_t n_cells = 0u, n_upd = 0u;
     const uint32_t t_end = t0 + n_steps;
     // the first step of a launch: re-sort if due, admission on its own
-    if (sort_due(t0) && !sort_all(P, sm, sbuf_of(t0 - 1u), gen)) return;
+    if (sort_due(t0) && !sort_all(P, sm, sbuf_of(t0 - 1u), gen, P.ctr)) return;
     admit_phase<false>(P, t0, sbuf_of(t0));
     if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
     for (uint32_t t = t0; t < t_end; t++) {
@@ -1443,7 +1447,7 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
         if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
         DBG_STAMP(6);
         if (more) {
-            if (sort_due(t + 1u) && !sort_all(P, sm, sbuf_of(t), gen)) return;
+            if (sort_due(t + 1u) && !sort_all(P, sm, sbuf_of(t), gen, P.ctr)) return;
             if (!fuse) {
                 admit_phase<false>(P, t + 1u, sbuf_of(t + 1u));
                 if (!grid_barrier(P.ctr, gen, &sm.flag)) return;
@@ -1451,6 +1455,117 @@ __global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent(const DevP 
         }
     }
     flush_stats(P, sm, n_cells, n_upd);
+}
+
+// ------------------------------------------------------------------------------------------------ replica batching
+// SURVEY 8(f) N4 (the calibration runs several parameter sets per iteration): up to NB independent
+// simulations -- own parameters, atlas, vehicles, results; same launch geometry and step counter -- advance in ONE
+// cooperative launch.  Every phase loops over the replicas between the same two grid barriers per timestep, so the
+// barriers, their fences and the wait for the slowest block are paid once per step instead of once per replica and
+// step, and the SMs that a single simulation leaves idle ~ 40 % of a step have the other replicas' chunks to run.
+// The barrier words are replica 0's.  Shared memory: the records of the two-stage pass (used by one replica's pass
+// at a time), then one UpdateSmem per replica (its lists must survive the barrier between pass and second phase).
+template <int NB>
+struct BatchP {
+    DevP p[NB];
+};
+#define MANTA_BATCH_SMEM(nb) (MANTA_REC_BYTES + (nb) * sizeof(UpdateSmem))
+// per-thread counters of one pass -> the replica's shared counters (one shared atomic per warp and counter)
+__device__ __forceinline__ void add_counts(UpdateSmem &sm, uint32_t n_cells, uint32_t n_upd)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_cells += __shfl_down_sync(0xFFFFFFFFu, n_cells, d);
+        n_upd += __shfl_down_sync(0xFFFFFFFFu, n_upd, d);
+    }
+    if ((threadIdx.x & 31u) == 0u) {
+        sm.wcnt[threadIdx.x >> 5][0] += (u64)n_cells;
+        sm.wcnt[threadIdx.x >> 5][1] += (u64)n_upd;
+    }
+}
+template <bool W256, int NB>
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_persistent_batch(const BatchP<NB> Bp, int n_rep, uint32_t t0, uint32_t n_steps, int fuse)
+{
+    UpdateSmem *sm = reinterpret_cast<UpdateSmem *>(reinterpret_cast<unsigned char *>(dyn_rec) + MANTA_REC_BYTES);
+    for (uint32_t k = threadIdx.x; k < (uint32_t)NB * (4u + 2u * MANTA_NW); k += blockDim.x) {
+        UpdateSmem &q = sm[k / (4u + 2u * MANTA_NW)];
+        const uint32_t j = k % (4u + 2u * MANTA_NW);
+        if (j < 4u) q.ev[j] = 0ull;
+        else q.wcnt[(j - 4u) >> 1][(j - 4u) & 1u] = 0ull;
+    }
+    Counters *ctr = Bp.p[0].ctr;
+    unsigned gen = 0u;
+    const uint32_t t_end = t0 + n_steps;
+    // the replica loops are NOT unrolled: one copy of the phase code, the replica's parameter block addressed by r
+    if (sort_due(t0)) {
+#pragma unroll 1
+        for (int r = 0; r < n_rep; r++)
+            if (!sort_all(Bp.p[r], sm[r], sbuf_of(t0 - 1u), gen, ctr)) return;
+    }
+#pragma unroll 1
+    for (int r = 0; r < n_rep; r++) admit_phase<false>(Bp.p[r], t0, sbuf_of(t0));
+    if (!grid_barrier(ctr, gen, &sm[0].flag)) return;
+    for (uint32_t t = t0; t < t_end; t++) {
+#pragma unroll 1
+        for (int r = 0; r < n_rep; r++) {
+            uint32_t n_cells = 0u, n_upd = 0u;
+            update_phase<W256>(Bp.p[r], t, sm[r], n_cells, n_upd, dyn_rec, true);
+            add_counts(sm[r], n_cells, n_upd);
+        }
+        if (!grid_barrier(ctr, gen, &sm[0].flag)) return;
+        const bool more = t + 1u < t_end;
+#pragma unroll 1
+        for (int r = 0; r < n_rep; r++) {
+            uint32_t n_cells = 0u;
+            if (more && fuse) admit_phase<true>(Bp.p[r], t + 1u, sbuf_of(t));
+            second_phase<W256>(Bp.p[r], t, sm[r], n_cells, true, (uint32_t)r, (uint32_t)n_rep);
+            add_counts(sm[r], n_cells, 0u);
+        }
+#if MANTA_PF >= 3
+        if (more) {   // the state records of this block's first chunks of step t + 1, every replica's: on their way while the barrier completes
+#pragma unroll 1
+            for (int r = 0; r < n_rep; r++) {
+                const DevP &P = Bp.p[r];
+                const StBuf &Sn = P.st[sbuf_of(t + 1u)];
+                const uint32_t at = blockIdx.x * P.seg_cap + threadIdx.x;
+                if (blockIdx.x < P.n_seg && threadIdx.x < P.seg_cnt[blockIdx.x]) {
+                    prefetch_line(&Sn.S0[at]);
+                    prefetch_line(&Sn.S1[at]);
+                    prefetch_line(&Sn.S2[at]);
+                    prefetch_line(&Sn.S3[at]);
+                }
+            }
+        }
+#endif
+        if (!grid_barrier(ctr, gen, &sm[0].flag)) return;
+        if (more) {
+            if (sort_due(t + 1u)) {
+#pragma unroll 1
+                for (int r = 0; r < n_rep; r++)
+                    if (!sort_all(Bp.p[r], sm[r], sbuf_of(t), gen, ctr)) return;
+            }
+            if (!fuse) {
+#pragma unroll 1
+                for (int r = 0; r < n_rep; r++) admit_phase<false>(Bp.p[r], t + 1u, sbuf_of(t + 1u));
+                if (!grid_barrier(ctr, gen, &sm[0].flag)) return;
+            }
+        }
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int r = 0; r < n_rep; r++) {
+        if (threadIdx.x == 0u) {
+            BlockStats *b = &Bp.p[r].blk[blockIdx.x];
+            u64 c = 0ull, u = 0ull;
+            for (uint32_t w = 0; w < (uint32_t)MANTA_NW; w++) {
+                c += sm[r].wcnt[w][0];
+                u += sm[r].wcnt[w][1];
+            }
+            if (c) atomicAdd(&b->cells_examined, c);
+            if (u) atomicAdd(&b->n_updates, u);
+        }
+        flush_stats(Bp.p[r], sm[r], 0u, 0u);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ set-up kernels

@@ -776,3 +776,36 @@ def test_idle_and_tiny_inputs(oracle_mod, binding):
     for flags in (0, 2):
         s, _ = run_both(oracle_mod, binding, net, trips, None, 700, dense_until=0, every=70, flags=flags)
         assert s["n_done"] == 2 and s["n_active"] == 0 and s["vehicle_updates"] > 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# replica batching -- several parameter sets advanced in one cooperative launch
+@pytest.mark.parametrize("n_rep", [2, 3, 4])
+def test_replica_batching_bit_exact(oracle_mod, binding, n_rep):
+    """n_rep simulations of one network and demand with different IDM parameters and seeds (a calibration sweep,
+    PAPER.md:148) advance through manta_step_batch; every replica equals its own oracle bit for bit (state, per-edge
+    entries, counters), i.e. batching changes nothing but the launch."""
+    net, trips, params, _ = wl.config3(scale=1 / 64.0, window=(4200.0, 5100.0), n_threads=4)
+    sets = [dict(a=1.0, b=2.0, T=1.5, s0=2.0, seed=11), dict(a=1.4, b=2.5, T=1.2, s0=2.5, seed=12),
+            dict(a=0.8, b=1.5, T=1.8, s0=1.5, seed=13), dict(a=2.0, b=3.0, T=1.0, s0=3.0, seed=14)][:n_rep]
+    gs = [binding.Sim(net, dict(params, **p), trips) for p in sets]
+    os_ = [oracle_mod.Oracle(net, dict(params, **p), trips) for p in sets]
+    t = 0
+    for k in (1, 63, 1, 200, 333, 402):              # crosses re-sorts at 64, 128, ...; single steps too
+        binding.step_batch(gs, k)
+        for o in os_:
+            o.step(k)
+        t += k
+        for r, (o, g) in enumerate(zip(os_, gs)):
+            compare(net, trips, o, g, "replica %d t=%d" % (r, t), atlas=(t in (1, 1000)))
+    sums = [g.readback()["summary"]["sum_travel_steps"] for g in gs]
+    assert len(set(sums)) == n_rep                    # the parameter sets do differ
+    # a replica can go on alone afterwards, and a batch needs equal step counters
+    gs[0].step(10)
+    os_[0].step(10)
+    compare(net, trips, os_[0], gs[0], "replica 0 alone")
+    with pytest.raises(binding.MantaError) as e:
+        binding.step_batch(gs, 5)
+    assert e.value.code == binding.ERR_INVALID_ARG
+    for g in gs:
+        g.close()
