@@ -57,8 +57,10 @@ extern "C" {
 #define MANTA_FLAG_RECORD_ACC 4u       /* keep each vehicle's last acceleration for manta_state.acc (tests)  */
 #define MANTA_FLAG_NO_FUSE 16u         /* admission of step t + 1 as a phase of its own (three grid barriers per step)
                                           instead of inside the second phase of step t (A/B switch)              */
-#define MANTA_FLAG_NO_L2_PIN 8u        /* do not pin the occupancy planes in L2 (A/B switch; the default sets the
-                                          device's cudaLimitPersistingL2CacheSize to the size of the two planes)   */
+#define MANTA_FLAG_NO_L2_PIN 8u        /* never pin the occupancy planes in L2 (A/B switch).  By default the planes get a
+                                          persisting L2 access-policy window while at least 400,000 vehicle slots are in
+                                          use (counted at manta_sync) and the planes fit the device's carve-out; the
+                                          device-wide cudaLimitPersistingL2CacheSize is raised for that and put back     */
 
 #define MANTA_FLAG_FEW_SEGMENTS 64u    /* test switch: the vehicles are kept in TWO segments (two thread blocks per
                                           phase) instead of one per resident block, so that small cases put thousands

@@ -62,8 +62,10 @@ struct manta_sim {
     bool w256 = true;             // look-ahead <= 256 cells and look-back <= 128: whole-window scans
     void *l2_window_base = nullptr;   // occupancy planes: L2 access-policy window of the step kernels
     uint64_t l2_window_bytes = 0;
-    size_t l2_persist = 0;            // persisting L2 carve-out granted (0 = no pinning)
-    size_t l2_persist_before = 0;     // the device-wide limit found at create time; put back by manta_destroy
+    size_t l2_want = 0;               // carve-out the two planes would need (0: they do not fit, or MANTA_FLAG_NO_L2_PIN)
+    size_t l2_persist = 0;            // persisting L2 carve-out currently granted (0 = not pinned now)
+    size_t l2_persist_before = 0;     // the device-wide limit found when pinning began; put back when it ends
+    uint64_t live_slots = 0;          // vehicle slots in use at the last manta_sync: decides whether pinning pays (pin_update)
     uint32_t n_blk_stats = 0;
 };
 
@@ -237,8 +239,9 @@ void manta_destroy(manta_sim *sim)
     cudaSetDevice(sim->device);
     cudaStreamSynchronize(sim->stream);
     while (!sim->allocs.empty()) dev_free(sim, sim->allocs.back().p);
-    if (sim->l2_persist && sim->l2_persist_before < sim->l2_persist) {
-        cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, sim->l2_persist_before);
+    if (sim->l2_persist) {
+        cudaCtxResetPersistingL2Cache();
+        if (sim->l2_persist_before < sim->l2_persist) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, sim->l2_persist_before);
         cudaGetLastError();
     }
     delete sim;
@@ -441,17 +444,9 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         // 400 us per step pinned, 142 us unpinned; profiles/r01d_*).
         if (!(p.flags & MANTA_FLAG_NO_L2_PIN) && max_persist > 0 && max_window > 0 &&
             s->l2_window_bytes <= (uint64_t)max_persist && s->l2_window_bytes <= (uint64_t)max_window) {
-            const size_t want = (size_t)std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_persist);
-            // cudaLimitPersistingL2CacheSize is a device-wide setting: it is raised here if needed and the value found
-            // is put back by manta_destroy (two simulations with pinned planes on one device share the carve-out)
-            cudaDeviceGetLimit(&s->l2_persist_before, cudaLimitPersistingL2CacheSize);
-            if (s->l2_persist_before >= want || cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
-                s->l2_persist = want;
-                s->l2_window_bytes = std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_window);
-            } else {
-                cudaGetLastError();
-            }
-        }
+            s->l2_want = (size_t)std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_persist);
+            s->l2_window_bytes = std::min<uint64_t>(s->l2_window_bytes, (uint64_t)max_window);
+        }   // whether the window is USED is decided per manta_step call, by the load (pin_update)
     }
     P.pay_shift = P.L_fx >= 4096 ? 2u : 0u;   // one payload entry per aligned group of four cells when L >= 4 m
     for (int k = 0; k < 2; k++)
@@ -820,6 +815,33 @@ int check_ready(manta_sim *s, uint32_t n_steps)
     return MANTA_OK;
 }
 
+// The persisting carve-out takes L2 away from everything else.  It pays once the touched working set of a step no
+// longer fits L2 next to the planes: measured at configs[2] / [3] (profiles/r02_final.md), pinned vs not: 26.3 vs 24.7 us
+// per step at 0.29 M vehicles, 30.6 vs 30.7 at 0.45 M, 40.0 vs 40.5 at 0.67 M, 84.2 vs 86.3 at 2.1 M.  So the window is
+// switched on for a manta_step call that starts with at least MANTA_PIN_MIN_SLOTS vehicle slots in use (as counted at
+// the last manta_sync) and off below (the decision holds for the whole call: the host is not involved between steps).
+// cudaLimitPersistingL2CacheSize is a device-wide setting: raised while pinning, put back afterwards.
+#ifndef MANTA_PIN_MIN_SLOTS
+#define MANTA_PIN_MIN_SLOTS 400000ull
+#endif
+void pin_update(manta_sim *s)
+{
+    const bool want = s->l2_want != 0 && s->live_slots >= MANTA_PIN_MIN_SLOTS;
+    if (want && !s->l2_persist) {
+        cudaDeviceGetLimit(&s->l2_persist_before, cudaLimitPersistingL2CacheSize);
+        if (s->l2_persist_before >= s->l2_want || cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, s->l2_want) == cudaSuccess)
+            s->l2_persist = s->l2_want;
+        else
+            cudaGetLastError();
+    } else if (!want && s->l2_persist) {
+        cudaStreamSynchronize(s->stream);
+        cudaCtxResetPersistingL2Cache();
+        if (s->l2_persist_before < s->l2_persist) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, s->l2_persist_before);
+        cudaGetLastError();
+        s->l2_persist = 0;
+    }
+}
+
 // Launch attributes of the step kernels: L2 access-policy window over the occupancy planes (+ cooperative).
 int step_attrs(const manta_sim *s, cudaLaunchAttribute *at, bool coop)
 {
@@ -907,6 +929,7 @@ int manta_step_async(manta_sim *s, uint32_t n_steps)
     int rc = check_ready(s, n_steps);
     if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
+    pin_update(s);
     if ((s->prm.flags & MANTA_FLAG_MULTI_KERNEL) || s->grid_persist == 0) {
         for (uint32_t k = 0; k < n_steps; k++, s->t++) launch_step_multi(s, s->t, k == 0, k + 1 == n_steps, nullptr);
     } else {
@@ -993,6 +1016,7 @@ int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
     int rc = check_ready(s, n_steps);
     if (rc) return rc;
     CUDA_TRY(s, cudaSetDevice(s->device));
+    pin_update(s);
     const uint32_t CH = 128;
     struct Events {   // destroyed on every return path
         std::vector<cudaEvent_t> ev;
@@ -1042,6 +1066,12 @@ int manta_sync(manta_sim *s)
             s->sticky_cuda = true;
             return fail(s, MANTA_ERR_CUDA, "grid barrier of the persistent step kernel timed out");
         }
+    }
+    if (s->loaded && s->l2_want) {   // slots in use now (dead ones included): what pin_update goes by
+        std::vector<uint32_t> cnt(s->P.n_seg);
+        CUDA_TRY(s, cudaMemcpyAsync(cnt.data(), s->P.seg_cnt, (uint64_t)s->P.n_seg * 4, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        s->live_slots = std::accumulate(cnt.begin(), cnt.end(), (uint64_t)0);
     }
     return MANTA_OK;
 }
