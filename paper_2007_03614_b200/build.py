@@ -77,11 +77,13 @@ def build_fast(force=False):
 
 
 def build_all(force=False, verbose=False):
+    """Everything the package needs; the three nvcc compilations run side by side."""
+    from concurrent.futures import ThreadPoolExecutor
     from . import workloads
     workloads.build_routing(force)
-    build_check(force)
-    build_fast(force)
-    return build_cuda(force, verbose)
+    with ThreadPoolExecutor(3) as ex:
+        jobs = [ex.submit(build_check, force), ex.submit(build_fast, force), ex.submit(build_cuda, force, verbose)]
+        return [j.result() for j in jobs][-1]
 
 
 if __name__ == "__main__":
