@@ -579,7 +579,8 @@ def test_bounds_checked_build(binding):
     assert binding.Sim.__init__ and binding.load_library().manta_check_failures(None) == -1   # product build: no checks
     sel = ("check_variant_active or dense_small_grid or stop_control_grid or stop_control_mixed or admission_fused or "
            "few_segments or deferred_list_overflow or look_ahead_past or window_of_more or long_look_ahead or "
-           "config3_shaped or config4_shaped or edge_speed or per_driver or short_vehicles or edge_cases")
+           "config3_shaped or config4_shaped or edge_speed or per_driver or short_vehicles or edge_cases or random_small or "
+           "limits_of or load_state or replica_batching")
     env = dict(os.environ, MANTA_LIB_VARIANT="check")
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-k", sel],
@@ -809,3 +810,56 @@ def test_replica_batching_bit_exact(oracle_mod, binding, n_rep):
     assert e.value.code == binding.ERR_INVALID_ARG
     for g in gs:
         g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Randomised differential cases: small random networks and parameter sets, every step against the oracle
+def random_case(seed):
+    """A random strongly connected network (ring through all nodes + random chords), random lengths from the shortest
+    admissible to a few hundred cells, 1-8 lanes, limits 5-30 m/s, random node controls, and random model parameters."""
+    rng_ = np.random.default_rng(seed)
+    n_nodes = int(rng_.integers(6, 30))
+    perm = rng_.permutation(n_nodes)
+    tail = list(perm)
+    head = list(np.roll(perm, -1))
+    for _ in range(int(rng_.integers(n_nodes, 3 * n_nodes))):
+        a, b = rng_.integers(0, n_nodes, 2)
+        if a != b:
+            tail.append(int(a))
+            head.append(int(b))
+    pairs = sorted(set(zip(tail, head)))
+    tail = np.array([p[0] for p in pairs], np.int64)
+    head = np.array([p[1] for p in pairs], np.int64)
+    m = len(tail)
+    limit = rng_.choice([5.0, 8.94, 13.89, 20.0, 29.06], m).astype(np.float32)
+    dt = float(rng_.choice([0.5, 0.5, 0.25, 1.0]))
+    a_ = float(rng_.uniform(0.6, 3.0))
+    v0_sig = float(rng_.choice([0.0, 0.0, 0.1, 0.25]))
+    vcap = float(limit.max()) * (1.5 if v0_sig > 0 else 1.0) + a_ * dt
+    z_out = int(np.ceil(vcap * dt)) + 1
+    veh_len = float(rng_.choice([3.0, 4.0, 5.0, 7.5]))
+    len_min = max(z_out + 1, int(np.ceil(veh_len)) + 1)
+    length = np.where(rng_.random(m) < 0.3, len_min + rng_.integers(0, 6, m), rng_.integers(len_min, 400, m)).astype(np.float32)
+    net = wl._csr_from_edges(n_nodes, tail, head, length_m=length, lanes=rng_.integers(1, 9, m).astype(np.uint8),
+                             speed_limit=limit)
+    net["node_ctrl"] = rng_.integers(0, 3, n_nodes).astype(np.uint8) if rng_.random() < 0.7 else np.zeros(n_nodes, np.uint8)
+    n_trips = int(rng_.integers(50, 400))
+    o_, d_ = wl.uniform_od(net, n_trips, seed + 1)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(n_trips, 0.0, float(rng_.uniform(5.0, 120.0)), seed + 2), n_threads=2)
+    lookback = int(np.ceil(veh_len)) + z_out + int(rng_.integers(0, 80))
+    params = dict(dt=dt, a=a_, b=float(rng_.uniform(1.0, 4.0)), T=float(rng_.uniform(0.5, 2.0)), s0=float(rng_.uniform(1.0, 4.0)),
+                  veh_len=veh_len, lookahead_cells=int(rng_.choice([40, 128, 256, 300])), lookback_cells=lookback,
+                  mlc_scale_m=float(rng_.choice([30.0, 100.0])), dlc_gain_thr=float(rng_.uniform(0.05, 0.5)),
+                  lc_alpha=float(rng_.uniform(0.05, 0.4)), lc_eps_sigma=float(rng_.choice([0.0, 1.0])),
+                  seed=int(rng_.integers(1, 2 ** 40)), stop_time_s=float(rng_.choice([2.0, 1.0, 0.0])) * (dt / 0.5),
+                  v0_sigma_rel=v0_sig)
+    return net, trips, params
+
+
+@pytest.mark.parametrize("seed", list(range(100, 160)))
+def test_random_small_cases(oracle_mod, binding, seed):
+    net, trips, params = random_case(seed)
+    flags = (0, 2, 16, 64, 6, 66)[seed % 6]
+    n_steps = int(min(900, 400 / params["dt"]))
+    s, _ = run_both(oracle_mod, binding, net, trips, params, n_steps, dense_until=n_steps, atlas_every=97, flags=flags)
+    assert s["vehicle_updates"] > 1000
