@@ -1007,7 +1007,9 @@ int manta_step_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps)
     if (rc) return rc;
     CUDA_TRY(s0, cudaGetLastError());
     for (uint32_t r = 0; r < n_sims; r++) sims[r]->t += n_steps;
-    return manta_sync(s0);
+    rc = manta_sync(s0);   // (the barrier words, and with them the abort flag, are replica 0's)
+    for (uint32_t r = 1; r < n_sims && rc == MANTA_OK; r++) rc = manta_sync(sims[r]);
+    return rc;
 }
 
 int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
