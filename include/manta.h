@@ -185,6 +185,28 @@ int manta_step_timed(manta_sim *sim, uint32_t n_steps, double phase_ms[3]);
 int manta_readback(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,
                    manta_summary *summary);
 
+/* manta_readback for callers that must not allocate device memory.  manta_readback takes a temporary staging block
+ * (28 bytes per trip) from cudaMalloc or the manta_set_allocator callback on every call and frees it again.  Two kinds
+ * of caller cannot afford that: a host program that has already given all free device memory to a pool of its own (a
+ * training framework's caching allocator, a fixed memory partition) -- there a fresh cudaMalloc simply fails -- and a
+ * loop that reads results while other streams are busy, because cudaMalloc / cudaFree may wait for the whole device
+ * and stall that work.  This variant runs the same two gather kernels with their staging arrays inside a fixed
+ * array that is part of the library image itself (static __device__, 7 MiB: MANTA_NOALLOC_MAX_TRIPS x 28 B; every
+ * device that loads libmanta.so holds it until the process exits).  It calls no cudaMalloc, cudaFree, allocator
+ * callback or other routine that allocates device memory (host side: two small std::vector temporaries for the
+ * summary).  Arguments, outputs and results are exactly those of manta_readback.
+ *   - Limit: simulations with more than MANTA_NOALLOC_MAX_TRIPS trips are refused with MANTA_ERR_INVALID_ARG and a
+ *     text that names the limit; nothing is read in that case.  Use manta_readback for those.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, once per device, with
+ *     that device current).  Make that first call before any stream capture begins.
+ *   - All calls on a device share the one array and it keeps the previous call's contents; each call clears the part
+ *     it reads before its kernels run.  Two calls that overlapped on the GPU would race on it; inside one process the
+ *     library therefore holds a lock from the first kernel until the results are on the host, so calls from several
+ *     threads (or for several simulations) simply run one after the other. */
+#define MANTA_NOALLOC_MAX_TRIPS 262144u
+int manta_readback_noalloc(manta_sim *sim, manta_state *state, uint32_t *edge_entries, manta_trip_result *trips,
+                           manta_summary *summary);
+
 /* Checkpoint / resume (and tests): replaces the dynamic state by the caller's -- the arrays manta_readback returns
  * (caller trip order; status, route_pos, lane, tag, x_fx, v required, wait optional, acc ignored), the per-trip
  * admit / arrive steps, the cumulative per-edge entries (NULL: kept) and the step counter t -- and rebuilds the

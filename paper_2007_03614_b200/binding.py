@@ -19,12 +19,13 @@ OK, ERR_INVALID_ARG, ERR_BAD_NETWORK, ERR_BAD_ROUTE, ERR_OOM, ERR_CUDA, ERR_STAT
 GREEN, PRIORITY, STOP = 0, 1, 2
 WAITING, ACTIVE, DONE = 0, 1, 2
 NONE = 0xFFFFFFFF
+NOALLOC_MAX_TRIPS = 262144   # MANTA_NOALLOC_MAX_TRIPS
 FLAG_MULTI_KERNEL, FLAG_RECORD_ACC = 2, 4
 
 EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_step", "manta_step_async", "manta_sync",
            "manta_step_batch",
            "manta_step_timed",
-           "manta_readback", "manta_load_state", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
+           "manta_readback", "manta_readback_noalloc", "manta_load_state", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
            "manta_launch_count",
            "manta_device_bytes", "manta_destroy", "manta_last_error", "manta_check_failures")
@@ -93,6 +94,7 @@ def load_library():
     L.manta_step_batch.argtypes = [C.POINTER(C.c_void_p), C.c_uint32, C.c_uint32]
     L.manta_step_timed.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(C.c_double * 3)]
     L.manta_readback.argtypes = [C.c_void_p, C.POINTER(State), C.c_void_p, C.c_void_p, C.POINTER(Summary)]
+    L.manta_readback_noalloc.argtypes = L.manta_readback.argtypes
     L.manta_readback_edge_speeds.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     L.manta_load_state.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(State), C.c_void_p, C.c_void_p]
     L.manta_atlas_cells.argtypes = [C.c_void_p]
@@ -227,7 +229,9 @@ class Sim:
     def sync(self):
         self._check(load_library().manta_sync(self.h))
 
-    def readback(self, state=True, edge_entries=True, trips=True, summary=True):
+    def readback(self, state=True, edge_entries=True, trips=True, summary=True, noalloc=False):
+        """manta_readback; noalloc=True calls manta_readback_noalloc instead (same outputs, no device allocation, at most
+        NOALLOC_MAX_TRIPS trips -- see include/manta.h for who needs that and what it costs)."""
         n = self.n_trips
         out = {}
         S = None
@@ -240,8 +244,8 @@ class Sim:
         tr = np.zeros((n, 2), np.uint32) if trips else None
         sm = Summary() if summary else None
         self._use()
-        self._check(load_library().manta_readback(self.h, None if S is None else C.byref(S), _ptr(ee), _ptr(tr),
-                                                  None if sm is None else C.byref(sm)))
+        fn = load_library().manta_readback_noalloc if noalloc else load_library().manta_readback
+        self._check(fn(self.h, None if S is None else C.byref(S), _ptr(ee), _ptr(tr), None if sm is None else C.byref(sm)))
         if trips:
             out["admit_step"], out["arrive_step"] = tr[:, 0].copy(), tr[:, 1].copy()
         if edge_entries:

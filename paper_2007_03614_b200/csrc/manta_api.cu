@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <numeric>
 #include <string>
 #include <chrono>
@@ -18,6 +19,14 @@
 #include <vector>
 
 using namespace manta;
+
+// Scratch of manta_readback_noalloc (include/manta.h): the per-trip staging arrays that manta_readback takes from the
+// allocator live here instead, in device memory that belongs to the loaded library itself.  Every device that loads
+// libmanta.so holds these 7 MiB until the process exits.  In HOST code the name below is only a handle for
+// cudaGetSymbolAddress -- it is not a device address and must never be handed to a kernel or a memset as one.
+#define MANTA_NOALLOC_BYTES_PER_TRIP 28u   /* results 8 | route_pos 4 | x 4 | v 4 | acc 4 | status, lane, tag, wait 1 each */
+#define MANTA_NOALLOC_SCRATCH_BYTES ((uint64_t)MANTA_NOALLOC_MAX_TRIPS * MANTA_NOALLOC_BYTES_PER_TRIP + 256u)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MANTA_NOALLOC_SCRATCH_BYTES];
 
 namespace {
 
@@ -1266,6 +1275,95 @@ int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell
         if (cell_off) cell_off[e] = s->cell_off[e];
         if (pitch) pitch[e] = (s->len_c[e] + 63u) & ~63u;
     }
+    return MANTA_OK;
+}
+
+
+// ---- manta_readback_noalloc: manta_readback without any device allocation ------------------------------------------
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;                              // one call at a time per process: every call uses the same array
+void *g_noalloc_ptr[kNoallocMaxDevices] = {};         // device address of g_noalloc_scratch, per device ordinal
+}  // namespace
+
+int manta_readback_noalloc(manta_sim *s, manta_state *st, uint32_t *edge_entries, manta_trip_result *trips, manta_summary *sum)
+{
+    if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
+    if (s->sticky_cuda) return fail(s, MANTA_ERR_CUDA, "earlier CUDA failure");
+    if (!s->loaded) return fail(s, MANTA_ERR_STATE, "no trips loaded");
+    const uint32_t n = s->n_trips;
+    if (n > MANTA_NOALLOC_MAX_TRIPS)
+        return fail(s, MANTA_ERR_INVALID_ARG, "manta_readback_noalloc: %u trips exceed the built-in scratch of MANTA_NOALLOC_MAX_TRIPS = %u trips; use manta_readback",
+                    n, MANTA_NOALLOC_MAX_TRIPS);
+    if (s->device < 0 || s->device >= kNoallocMaxDevices)
+        return fail(s, MANTA_ERR_INVALID_ARG, "manta_readback_noalloc: device ordinal %d beyond the %d this call keeps an address for", s->device, kNoallocMaxDevices);
+    CUDA_TRY(s, cudaSetDevice(s->device));
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);   // held until the results are on the host: the array is shared
+    if (!g_noalloc_ptr[s->device]) {
+        // set-up, once per device, with that device current: the array's address on THIS device
+        void *p = nullptr;
+        CUDA_TRY(s, cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        g_noalloc_ptr[s->device] = p;
+    }
+    uint8_t *buf = (uint8_t *)g_noalloc_ptr[s->device];
+    if (edge_entries)
+        CUDA_TRY(s, cudaMemcpyAsync(edge_entries, s->P.edge_entries, (uint64_t)s->n_edges * 4, cudaMemcpyDeviceToHost, s->stream));
+    if (st || trips || sum) {
+        // same staging layout as manta_readback, inside the static array
+        const uint64_t nn = ((uint64_t)n + 15) & ~15ull;
+        const uint64_t used = nn * MANTA_NOALLOC_BYTES_PER_TRIP + 16;
+        uint2 *d_res = (uint2 *)buf;
+        uint32_t *d_rpos = (uint32_t *)(buf + nn * 8), *d_x = d_rpos + nn;
+        float *d_v = (float *)(d_x + nn), *d_acc = d_v + nn;
+        uint8_t *d_status = (uint8_t *)(d_acc + nn), *d_lane = d_status + nn, *d_tag = d_lane + nn, *d_wait = d_tag + nn;
+        unsigned long long *d_stopped = (unsigned long long *)(d_wait + nn);
+        // the array still holds the previous call's rows and stop count: everything read below starts from zero
+        CUDA_TRY(s, cudaMemsetAsync(buf, 0, used, s->stream));
+        const int g = (int)std::min<uint32_t>((n + 255) / 256, 4096);
+        k_status_from_steps<<<g, 256, 0, s->stream>>>(n, s->d_trip_of_id, s->P.admit_step, s->P.arrive_step, d_status, d_res);
+        k_gather_state<<<(unsigned)std::min<uint32_t>(s->P.n_seg, 4096u), 256, 0, s->stream>>>(s->P, s->t == 0 ? 0 : (int)(((s->t - 1u) / MANTA_SORT_EVERY) & 1u), s->d_trip_of_id, d_status, d_rpos, d_lane, d_tag, d_x, d_v, d_acc, d_wait, d_stopped);
+        CUDA_TRY(s, cudaGetLastError());
+        std::vector<uint8_t> own_status;   // host memory only, and only when the caller gave no status array
+        uint8_t *h_status = st && st->status ? st->status : nullptr;
+        if (!h_status && sum) {
+            own_status.resize(n);
+            h_status = own_status.data();
+        }
+        if (h_status) CUDA_TRY(s, cudaMemcpyAsync(h_status, d_status, n, cudaMemcpyDeviceToHost, s->stream));
+        if (st) {
+            if (st->route_pos) CUDA_TRY(s, cudaMemcpyAsync(st->route_pos, d_rpos, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->lane) CUDA_TRY(s, cudaMemcpyAsync(st->lane, d_lane, n, cudaMemcpyDeviceToHost, s->stream));
+            if (st->tag) CUDA_TRY(s, cudaMemcpyAsync(st->tag, d_tag, n, cudaMemcpyDeviceToHost, s->stream));
+            if (st->x_fx) CUDA_TRY(s, cudaMemcpyAsync(st->x_fx, d_x, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->v) CUDA_TRY(s, cudaMemcpyAsync(st->v, d_v, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->acc) CUDA_TRY(s, cudaMemcpyAsync(st->acc, d_acc, (uint64_t)n * 4, cudaMemcpyDeviceToHost, s->stream));
+            if (st->wait) CUDA_TRY(s, cudaMemcpyAsync(st->wait, d_wait, n, cudaMemcpyDeviceToHost, s->stream));
+        }
+        unsigned long long h_stopped = 0;
+        CUDA_TRY(s, cudaMemcpyAsync(&h_stopped, d_stopped, sizeof h_stopped, cudaMemcpyDeviceToHost, s->stream));
+        if (trips) CUDA_TRY(s, cudaMemcpyAsync(trips, d_res, (uint64_t)n * 8, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        if (sum) {
+            std::vector<BlockStats> bs(s->n_blk_stats);
+            CUDA_TRY(s, cudaMemcpy(bs.data(), s->P.blk, sizeof(BlockStats) * bs.size(), cudaMemcpyDeviceToHost));
+            memset(sum, 0, sizeof *sum);
+            for (uint32_t i = 0; i < n; i++) {
+                sum->n_waiting += h_status[i] == MANTA_WAITING;
+                sum->n_active += h_status[i] == MANTA_ACTIVE;
+            }
+            sum->t = s->t;
+            sum->n_stopped = h_stopped;
+            for (const BlockStats &b : bs) {
+                sum->lane_changes += b.lane_changes;
+                sum->cells_examined += b.cells_examined;
+                sum->lc_evals += b.lc_evals;
+                sum->n_done += b.n_done;
+                sum->sum_travel_steps += b.sum_travel;
+                sum->vehicle_updates += b.n_updates;
+            }
+        }
+    }
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return MANTA_OK;
 }
 
