@@ -41,8 +41,8 @@ extern "C" {
 #define MANTA_STOP 2     /* case 1 in full: every vehicle stands stop_time_s at the stop line, then
                             one vehicle per node per step, the (inbound, outbound) edge combinations taking turns
                             (round-robin), equal combinations by smallest vehicle id -- rule R8s of DESIGN.md.
-                            Limits with STOP nodes: in-degree x out-degree <= 256 per STOP node, n_nodes < 2^27,
-                            n_trips <= 2^24, ceil(stop_time_s / dt) <= 7                                         */
+                            Limits that apply only to networks with STOP nodes: in-degree x out-degree <= 256 per
+                            STOP node, n_trips < 2^24, ceil(stop_time_s / dt) <= 7 (else stop_time_s is unused) */
 
 #define MANTA_WAITING 0
 #define MANTA_ACTIVE 1
@@ -80,7 +80,7 @@ typedef struct {
     const float *length_m;       /* [n_edges]  > 0; rounded to whole 1 m cells; >= LEN_MIN (R0) */
     const uint8_t *lanes;        /* [n_edges]  1..8                                                     */
     const float *speed_limit;    /* [n_edges]  m/s, > 0; used as IDM v0                   */
-    const uint8_t *node_ctrl;    /* [n_nodes] MANTA_GREEN / MANTA_PRIORITY, or NULL = all GREEN         */
+    const uint8_t *node_ctrl;    /* [n_nodes] MANTA_GREEN / MANTA_PRIORITY / MANTA_STOP, or NULL = all GREEN */
 } manta_network;
 
 /* Model parameters; one set shared by all vehicles.  delta of Eq. 1 is fixed at 4. */
@@ -147,7 +147,7 @@ int manta_set_allocator(manta_alloc_fn alloc, manta_free_fn free_, void *ctx);
 /* Builds the atlas (one row of 1 m cells per (edge, lane)) and the static tables of R0 on
  * `cuda_device`.  Errors: INVALID_ARG (NULL, params->size mismatch, non-positive dt/a/b/...), BAD_NETWORK (lanes
  * outside 1..8, length < LEN_MIN or > 65535 cells, non-finite values, head out of range, out-degree > 255,
- * more than 2^32 - 1 atlas cells), OOM, CUDA. */
+ * more than 2^32 - 1 atlas cells, n_nodes >= 2^27, 8 n_edges + n_nodes >= 2^32), OOM, CUDA. */
 int manta_create(const manta_network *net, const manta_params *params, int cuda_device, manta_sim **out);
 
 /* Loads the demand: trip i follows route_edges[route_ptr[i] .. route_ptr[i+1]-1] ("routes are
@@ -212,9 +212,12 @@ int manta_readback_noalloc(manta_sim *sim, manta_state *state, uint32_t *edge_en
  * admit / arrive steps, the cumulative per-edge entries (NULL: kept) and the step counter t -- and rebuilds the
  * atlas, the vehicle slots and the admission queues from it.  Summary counters that are not functions of the state
  * (vehicle_updates, lane_changes, cells_examined, lc_evals) and the speed statistics are left to restart / continue.
- * Errors: INVALID_ARG (missing array; status > 2; route position, lane, position, speed or counter out of range; an
- * admitted trip queued behind a waiting one; two vehicles in one cell -- the last is found while rebuilding and
- * leaves the handle unusable), STATE (no trips loaded), OOM, CUDA.  Otherwise a failed call changes nothing. */
+ * Errors: INVALID_ARG (missing array; status > 2; route position, lane, position or counter out of range; a speed
+ * that is negative, not finite or above the fastest possible one = max(largest desired speed, largest init_speed)
+ * + a dt; admit / arrive steps that contradict the status or lie after t; an admitted trip queued behind a waiting
+ * one; two vehicles in one cell -- the last is found while rebuilding and leaves the handle unusable), STATE (no
+ * trips loaded), OOM, CUDA.  Otherwise a failed call changes nothing.  NOT checked: that vehicles of one lane are at
+ * least veh_len apart (a state that a run of this library or of the rules R1-R8 produced always is). */
 int manta_load_state(manta_sim *sim, uint32_t t, const manta_state *state, const manta_trip_result *trips,
                      const uint32_t *edge_entries);
 

@@ -73,8 +73,8 @@ struct manta_sim {
     uint64_t l2_window_bytes = 0;
     size_t l2_want = 0;               // carve-out the two planes would need (0: they do not fit, or MANTA_FLAG_NO_L2_PIN)
     size_t l2_persist = 0;            // persisting L2 carve-out currently granted (0 = not pinned now)
-    size_t l2_persist_before = 0;     // the device-wide limit found when pinning began; put back when it ends
-    uint64_t live_slots = 0;          // vehicle slots in use at the last manta_sync: decides whether pinning pays (pin_update)
+    uint64_t live_slots = 0;          // vehicle slots in use at the last manta_sync / manta_load_trips / manta_load_state: decides whether pinning pays (pin_update)
+    std::vector<uint32_t> seg_cnt_host;   // manta_sync's copy of the segment counts
     uint32_t n_blk_stats = 0;
 };
 
@@ -160,6 +160,9 @@ void derive_constants(manta_sim *s, double max_init_speed)
     s->P.L_fx = (int32_t)std::lround((double)p.veh_len * 1024.0);
     s->P.Z_out = (uint32_t)std::ceil(vcap * (double)p.dt) + 1u;
     s->P.Z_in = s->P.L_c + s->P.Z_out;
+    float vc = (float)vcap;
+    if ((double)vc < vcap) vc = std::nextafterf(vc, INFINITY);   // rounded up: the bound manta_load_state holds speeds to
+    s->P.vcap = vc;
 }
 uint32_t len_min(const manta_sim *s) { return std::max(s->P.Z_out + 1u, s->P.L_c + 1u); }
 
@@ -242,17 +245,14 @@ uint64_t manta_launch_count(const manta_sim *sim) { return sim ? sim->launches :
 uint64_t manta_device_bytes(const manta_sim *sim) { return sim ? sim->dev_bytes : 0; }
 uint64_t manta_atlas_cells(const manta_sim *sim) { return sim ? sim->n_cells : 0; }
 
+namespace { void pin_release(manta_sim *s); }
 void manta_destroy(manta_sim *sim)
 {
     if (!sim) return;
     cudaSetDevice(sim->device);
     cudaStreamSynchronize(sim->stream);
     while (!sim->allocs.empty()) dev_free(sim, sim->allocs.back().p);
-    if (sim->l2_persist) {
-        cudaCtxResetPersistingL2Cache();
-        if (sim->l2_persist_before < sim->l2_persist) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, sim->l2_persist_before);
-        cudaGetLastError();
-    }
+    if (sim->l2_persist) pin_release(sim);
     delete sim;
 }
 
@@ -293,7 +293,7 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
         p.lookahead_cells < 1 || p.lookahead_cells > 8192 || p.lookback_cells < 1 || p.lookback_cells > 8192 ||
         !(p.mlc_scale_m >= 1.f) || !(p.mlc_scale_m <= 10000.f) || !(p.lc_alpha >= 0.f) || !(p.lc_eps_sigma >= 0.f) ||
         !std::isfinite(p.dlc_gain_thr) || !std::isfinite(p.lc_gap_low) || !std::isfinite(p.lc_gap_high) ||
-        !(p.stop_time_s >= 0.f) || !(std::ceil((double)p.stop_time_s / (double)p.dt - 1e-9) <= 7.0) ||   // 3-bit stop-line counter
+        !(p.stop_time_s >= 0.f) || !std::isfinite(p.stop_time_s) ||   // (its length in steps is limited only where STOP nodes exist: below)
         !(p.v0_sigma_rel >= 0.f) || !std::isfinite(p.v0_sigma_rel) ||
         (p.stat_period_steps != 0u && (p.stat_slice_steps == 0u || p.stat_n_slices == 0u || p.stat_n_slices > 4096u)))
         return fail(nullptr, MANTA_ERR_INVALID_ARG, "parameter out of range");
@@ -320,11 +320,12 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
     s->n_nodes = N;
     s->n_edges = M;
     if (net->row_ptr[0] != 0 || net->row_ptr[N] != M) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "row_ptr does not span the edges"));
-    // packing limits of the device records: a PRIORITY node id is kept in 28 bits (S3.z = node << 4), lane entries
+    // packing limits of the device records: a node id is kept in 27 bits (NODE_MASK), lane entries
     // (e * 8 + lane) and claim-word indices (n_edges * 8 + node) are 32-bit
     static_assert(MANTA_MAX_LANES <= 8, "lane entries are e * 8 + lane");
-    if (N >= (1u << 28) || (uint64_t)M * 8ull + (uint64_t)N >= 0xFFFFFFFFull)
-        return bail(fail(s, MANTA_ERR_BAD_NETWORK, "network too large for the 32-bit claim words (n_nodes < 2^28, 8 n_edges + n_nodes < 2^32)"));
+    // (bit 27 of the node word in edge_tab.z / S3.z is the STOP flag in every network, so node ids stay below 2^27)
+    if (N >= (1u << 27) || (uint64_t)M * 8ull + (uint64_t)N >= 0xFFFFFFFFull)
+        return bail(fail(s, MANTA_ERR_BAD_NETWORK, "network too large for the device records (n_nodes < 2^27, 8 n_edges + n_nodes < 2^32)"));
     s->row_ptr.assign(net->row_ptr, net->row_ptr + N + 1);
     s->head.assign(net->head, net->head + M);
     s->tail.resize(M);
@@ -379,8 +380,11 @@ int manta_create(const manta_network *net, const manta_params *prm, int cuda_dev
             s->node_prio[u] = net->node_ctrl[u] != MANTA_GREEN ? 1 : 0;
             s->has_stop = s->has_stop || net->node_ctrl[u] == MANTA_STOP;
         }
-    if (s->has_stop && N >= (1u << 27)) return bail(fail(s, MANTA_ERR_BAD_NETWORK, "STOP nodes need n_nodes < 2^27"));
-    P.W_stop = (uint32_t)std::ceil((double)p.stop_time_s / (double)p.dt - 1e-9);
+    const double w_stop = std::ceil((double)p.stop_time_s / (double)p.dt - 1e-9);
+    if (s->has_stop && !(w_stop <= 7.0))   // only networks with STOP nodes use the 3-bit stop-line counter of S0.x
+        return bail(fail(s, MANTA_ERR_INVALID_ARG, "stop_time_s = %g s is %.0f steps of dt = %g s; MANTA_STOP nodes allow at most 7 steps (3-bit stop-line counter)",
+                         (double)p.stop_time_s, w_stop, (double)p.dt));
+    P.W_stop = s->has_stop ? (uint32_t)w_stop : 0u;
     P.id_mask = s->has_stop ? 0x00FFFFFFu : 0xFFFFFFFFu;
     P.v0_sigma_rel = p.v0_sigma_rel;
     P.stat_period = p.stat_period_steps; P.stat_slice = p.stat_slice_steps; P.stat_n_slices = p.stat_period_steps ? p.stat_n_slices : 0u;
@@ -475,8 +479,8 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     if (s->loaded) return fail(s, MANTA_ERR_STATE, "trips already loaded");
     if (!route_ptr || !route_edges || !depart_time_s || n_trips == 0 || n_trips >= 0x7FFFFFFFu)
         return fail(s, MANTA_ERR_INVALID_ARG, "null / empty / too many trips");
-    if (s->has_stop && n_trips > (1u << 24))
-        return fail(s, MANTA_ERR_INVALID_ARG, "networks with STOP nodes take at most 2^24 trips (the claim key keeps the turn rank above a 24-bit vehicle id)");
+    if (s->has_stop && n_trips >= (1u << 24))   // strictly: id 2^24 - 1 under turn rank 255 would give the key of an unclaimed word
+        return fail(s, MANTA_ERR_INVALID_ARG, "networks with STOP nodes take fewer than 2^24 trips (the claim key keeps the turn rank above a 24-bit vehicle id)");
     CUDA_TRY(s, cudaSetDevice(s->device));
     // MANTA_LOAD_TIMING=1: wall time of each stage of this call on stderr (initialisation is outside the timed path,
     // but it is most of the end-to-end time of a short run)
@@ -809,6 +813,7 @@ int manta_load_trips(manta_sim *s, uint32_t n_trips, const uint64_t *route_ptr, 
     s->n_trips = n_trips;
     s->loaded = true;
     s->t = 0;
+    s->live_slots = n_init;   // slots in use before the first step: the pre-placed vehicles
     s->grid_admit = (int)std::max<uint32_t>(1u, std::min<uint32_t>((P.n_queues + 255u) / 256u, (uint32_t)s->sm_count * 8u));   // k_admit alone
     return MANTA_OK;
 }
@@ -833,20 +838,50 @@ int check_ready(manta_sim *s, uint32_t n_steps)
 #ifndef MANTA_PIN_MIN_SLOTS
 #define MANTA_PIN_MIN_SLOTS 400000ull
 #endif
+// Several simulations may pin on one device (replica runs, batches): the limit found before the FIRST of them pinned is
+// kept per device and put back, and the persisting lines reset, only when the LAST pinned one lets go.
+struct PinDevice {
+    int pinned = 0;            // simulations on this device that hold a window now
+    size_t original = 0;       // cudaLimitPersistingL2CacheSize before the first of them
+    bool raised = false;       // the library raised the limit above `original`
+};
+std::mutex g_pin_mu;
+PinDevice g_pin[64];
+
+bool pin_acquire(manta_sim *s)   // device current
+{
+    if (s->device < 0 || s->device >= 64) return false;
+    std::lock_guard<std::mutex> lock(g_pin_mu);
+    PinDevice &d = g_pin[s->device];
+    size_t now = 0;
+    if (cudaDeviceGetLimit(&now, cudaLimitPersistingL2CacheSize) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (d.pinned == 0) { d.original = now; d.raised = false; }
+    if (now < s->l2_want) {
+        if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, s->l2_want) != cudaSuccess) { cudaGetLastError(); return false; }
+        d.raised = true;
+    }
+    d.pinned++;
+    return true;
+}
+void pin_release(manta_sim *s)   // device current; the simulation's stream already synchronised
+{
+    std::lock_guard<std::mutex> lock(g_pin_mu);
+    PinDevice &d = g_pin[s->device];
+    if (d.pinned > 0 && --d.pinned == 0) {
+        cudaCtxResetPersistingL2Cache();
+        if (d.raised) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, d.original);
+        cudaGetLastError();
+        d.raised = false;
+    }
+}
 void pin_update(manta_sim *s)
 {
     const bool want = s->l2_want != 0 && s->live_slots >= MANTA_PIN_MIN_SLOTS;
     if (want && !s->l2_persist) {
-        cudaDeviceGetLimit(&s->l2_persist_before, cudaLimitPersistingL2CacheSize);
-        if (s->l2_persist_before >= s->l2_want || cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, s->l2_want) == cudaSuccess)
-            s->l2_persist = s->l2_want;
-        else
-            cudaGetLastError();
+        if (pin_acquire(s)) s->l2_persist = s->l2_want;
     } else if (!want && s->l2_persist) {
         cudaStreamSynchronize(s->stream);
-        cudaCtxResetPersistingL2Cache();
-        if (s->l2_persist_before < s->l2_persist) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, s->l2_persist_before);
-        cudaGetLastError();
+        pin_release(s);
         s->l2_persist = 0;
     }
 }
@@ -1011,14 +1046,30 @@ int manta_step_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps)
         fuse = fuse && s->fuse_admit;
     }
     CUDA_TRY(s0, cudaSetDevice(s0->device));
+    // A failure once kernels may have run (CUDA error, barrier time-out) leaves EVERY replica mid-step: all of them are
+    // marked unusable with the error text, not only the one the error was recorded on.  t advances only after success.
+    auto all_unusable = [&](int rc, const manta_sim *src) {
+        const std::string msg = "manta_step_batch failed, every simulation of the batch is unusable: " + src->err;
+        for (uint32_t r = 0; r < n_sims; r++) {
+            sims[r]->sticky_cuda = true;
+            sims[r]->err = msg;
+        }
+        g_last_error = msg;
+        return rc;
+    };
     int rc = n_sims == 2 ? launch_batch<2>(sims, n_sims, n_steps, s0->w256, fuse ? 1 : 0)
                          : launch_batch<4>(sims, n_sims, n_steps, s0->w256, fuse ? 1 : 0);
-    if (rc) return rc;
-    CUDA_TRY(s0, cudaGetLastError());
+    if (rc) return s0->sticky_cuda ? all_unusable(rc, s0) : rc;   // (not sticky: refused before anything was launched)
+    if (cudaGetLastError() != cudaSuccess) {
+        fail(s0, MANTA_ERR_CUDA, "kernel launch of the batch failed");
+        return all_unusable(MANTA_ERR_CUDA, s0);
+    }
+    for (uint32_t r = 0; r < n_sims; r++) {   // replica 0 first: the barrier words, and with them the abort flag, are its own
+        rc = manta_sync(sims[r]);
+        if (rc) return all_unusable(rc, sims[r]);
+    }
     for (uint32_t r = 0; r < n_sims; r++) sims[r]->t += n_steps;
-    rc = manta_sync(s0);   // (the barrier words, and with them the abort flag, are replica 0's)
-    for (uint32_t r = 1; r < n_sims && rc == MANTA_OK; r++) rc = manta_sync(sims[r]);
-    return rc;
+    return MANTA_OK;
 }
 
 int manta_step_timed(manta_sim *s, uint32_t n_steps, double phase_ms[3])
@@ -1068,22 +1119,20 @@ int manta_sync(manta_sim *s)
 {
     if (!s) return fail(nullptr, MANTA_ERR_INVALID_ARG, "null simulation");
     CUDA_TRY(s, cudaSetDevice(s->device));
+    // both reads are ordered on the stream behind the steps: one synchronisation for the call
+    unsigned int ab = 0;
+    const bool want_abort = s->loaded && s->grid_persist, want_slots = s->loaded && s->l2_want;
+    if (want_abort) CUDA_TRY(s, cudaMemcpyAsync(&ab, &s->P.ctr->abort, sizeof ab, cudaMemcpyDeviceToHost, s->stream));
+    if (want_slots) {   // slots in use now (dead ones included): what pin_update goes by
+        s->seg_cnt_host.resize(s->P.n_seg);
+        CUDA_TRY(s, cudaMemcpyAsync(s->seg_cnt_host.data(), s->P.seg_cnt, (uint64_t)s->P.n_seg * 4, cudaMemcpyDeviceToHost, s->stream));
+    }
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-    if (s->loaded && s->grid_persist) {
-        unsigned int ab = 0;
-        CUDA_TRY(s, cudaMemcpyAsync(&ab, &s->P.ctr->abort, sizeof ab, cudaMemcpyDeviceToHost, s->stream));
-        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-        if (ab) {
-            s->sticky_cuda = true;
-            return fail(s, MANTA_ERR_CUDA, "grid barrier of the persistent step kernel timed out");
-        }
+    if (ab) {
+        s->sticky_cuda = true;
+        return fail(s, MANTA_ERR_CUDA, "grid barrier of the persistent step kernel timed out");
     }
-    if (s->loaded && s->l2_want) {   // slots in use now (dead ones included): what pin_update goes by
-        std::vector<uint32_t> cnt(s->P.n_seg);
-        CUDA_TRY(s, cudaMemcpyAsync(cnt.data(), s->P.seg_cnt, (uint64_t)s->P.n_seg * 4, cudaMemcpyDeviceToHost, s->stream));
-        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-        s->live_slots = std::accumulate(cnt.begin(), cnt.end(), (uint64_t)0);
-    }
+    if (want_slots) s->live_slots = std::accumulate(s->seg_cnt_host.begin(), s->seg_cnt_host.end(), (uint64_t)0);
     return MANTA_OK;
 }
 
@@ -1192,14 +1241,16 @@ int manta_load_state(manta_sim *s, uint32_t t, const manta_state *st, const mant
     StateIn in{d_status, d_lane, d_tag, st->wait ? d_wait : nullptr, d_rpos, d_x, d_v, d_steps};
     const int g = (int)std::min<uint32_t>((std::max(n, s->P.n_queues) + 255) / 256, 4096);
     // pass 1: validation only -- a bad state leaves the simulation as it was
-    k_state_validate<<<g, 256, 0, s->stream>>>(s->P, in, s->d_trip_of_id, n, d_err);
+    k_state_validate<<<g, 256, 0, s->stream>>>(s->P, in, s->d_trip_of_id, n, t, d_err);
     uint32_t h_err = 0;
     TRY_LS(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s->stream));
     TRY_LS(cudaStreamSynchronize(s->stream));
     if (h_err) {
-        static const char *what[] = {"", "status value above 2", "route position beyond the trip's route", "lane, position, speed or stop counter out of range",
-                                     "an admitted trip stands behind a waiting one of the same origin edge (admission is first in, first out)"};
-        return done(fail(s, MANTA_ERR_INVALID_ARG, "manta_load_state: %s", what[std::min<uint32_t>(h_err, 4u)]));
+        static const char *what[] = {"", "status value above 2", "route position beyond the trip's route",
+                                     "lane, position or stop counter out of range, or a speed that is negative, not finite or above the fastest possible one (largest desired or initial speed + a dt)",
+                                     "an admitted trip stands behind a waiting one of the same origin edge (admission is first in, first out)",
+                                     "admit / arrive steps that contradict the status (WAITING: none; ACTIVE: admit_step <= t, no arrive_step; DONE: admit_step <= arrive_step <= t)"};
+        return done(fail(s, MANTA_ERR_INVALID_ARG, "manta_load_state: %s", what[std::min<uint32_t>(h_err, 5u)]));
     }
     // pass 2: rebuild.  Both occupancy planes empty (no vehicle has an earlier mark), claims unclaimed, counters restarted.
     const uint64_t plane_words = ((s->n_cells / 64 + 8) + 15) & ~15ull;
@@ -1212,9 +1263,12 @@ int manta_load_state(manta_sim *s, uint32_t t, const manta_state *st, const mant
     k_state_counts<<<(s->P.n_seg + 255) / 256, 256, 0, s->stream>>>(s->P, d_counter);
     s->launches += 3;
     TRY_LS(cudaGetLastError());
-    TRY_LS(cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, s->stream));
+    uint32_t h_tail[2] = {0u, 0u};   // {slots dealt out, error}
+    TRY_LS(cudaMemcpyAsync(h_tail, d_counter, 8, cudaMemcpyDeviceToHost, s->stream));
     TRY_LS(cudaStreamSynchronize(s->stream));
 #undef TRY_LS
+    h_err = h_tail[1];
+    s->live_slots = h_tail[0];
     s->t = t;
     if (h_err) {   // found while rebuilding: the state is unusable now
         s->sticky_cuda = true;

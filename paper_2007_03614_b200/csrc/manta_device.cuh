@@ -127,6 +127,7 @@ struct DevP {
     // model constants (R0), rounded once on the host from double
     float dt, a, T, s0, veh_len, C1, HALF_DT, VSCALE, ADT;
     float dlc_thr, alpha, gap_low, gap_high, eps_sigma;
+    float vcap;                  // R0: no vehicle is ever faster (largest desired or initial speed + a dt, rounded up); Z_out is built on it
     uint32_t H, lookback, L_c, Z_out, Z_in, Lam;
     int32_t L_fx;
     uint32_t seed_lo, seed_hi;

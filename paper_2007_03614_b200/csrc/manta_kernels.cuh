@@ -1626,23 +1626,31 @@ __global__ void k_place_initial(const DevP P, const uint4 *init, uint32_t n_init
     }
 }
 // manta_load_state, pass 1: nothing is written but the error word (1 bad status, 2 route position beyond the route,
-// 3 lane / position beyond the edge, 4 an admitted trip behind a waiting one in its origin queue).
+// 3 lane / position beyond the edge, stop counter above 7, speed negative, not finite or above vcap (the layout's
+// Z_out, cannot_cross and may_defer rest on v <= vcap: a faster vehicle would be moved outside its row),
+// 4 an admitted trip behind a waiting one in its origin queue, 5 admit / arrive steps that contradict the status).
 struct StateIn {
     const uint8_t *status, *lane, *tag, *wait;   // caller (trip) order; wait may be null
     const uint32_t *route_pos, *x_fx;
     const float *v;
     const uint2 *steps;                          // {admit_step, arrive_step} per trip
 };
-__global__ void k_state_validate(const DevP P, StateIn in, const uint32_t *trip_of_id, uint32_t n_trips, uint32_t *err)
+__global__ void k_state_validate(const DevP P, StateIn in, const uint32_t *trip_of_id, uint32_t n_trips, uint32_t t, uint32_t *err)
 {
     for (uint32_t id = blockIdx.x * blockDim.x + threadIdx.x; id < n_trips; id += gridDim.x * blockDim.x) {
         const uint32_t tr = trip_of_id[id];
         const uint32_t st = in.status[tr];
         if (st > 2u) { atomicMax(err, 1u); continue; }
+        const uint2 ab = in.steps[tr];
+        // WAITING: neither step; ACTIVE: admitted by now, not arrived; DONE: admitted, then arrived, by now
+        const bool steps_ok = st == 0u ? (ab.x == CELL_NONE && ab.y == CELL_NONE)
+                            : st == 1u ? (ab.x <= t && ab.y == CELL_NONE)
+                                       : (ab.x <= ab.y && ab.y <= t);
+        if (!steps_ok) atomicMax(err, 5u);
         if (st != 1u) continue;
         if (in.route_pos[tr] >= P.route_len[id]) { atomicMax(err, 2u); continue; }
         const uint4 rr = P.route[P.route_start[id] + in.route_pos[tr]];
-        if (in.lane[tr] >= GEOM_LANES(rr.y) || (in.x_fx[tr] >> 10) >= GEOM_LEN(rr.y) || (in.wait && in.wait[tr] > 7u) || !(in.v[tr] >= 0.0f))
+        if (in.lane[tr] >= GEOM_LANES(rr.y) || (in.x_fx[tr] >> 10) >= GEOM_LEN(rr.y) || (in.wait && in.wait[tr] > 7u) || !(in.v[tr] >= 0.0f) || !(in.v[tr] <= P.vcap))
             atomicMax(err, 3u);
     }
     for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < P.n_queues; k += gridDim.x * blockDim.x) {

@@ -502,11 +502,25 @@ def test_stop_control_mixed_nodes(oracle_mod, binding, stop_s):
     assert s["n_done"] > 200 and s["lane_changes"] > 50
 
 
+def test_small_time_step_without_stop_nodes(oracle_mod, binding):
+    """dt = 0.25 s with the default stop_time_s (8 steps, unused without STOP nodes): accepted, and bit-exact."""
+    net = wl.grid_network(nx=4, ny=4, lanes=2, ctrl=wl.PRIORITY)
+    o_, d_ = wl.uniform_od(net, 300, 71)
+    trips = wl.make_trips(net, o_, d_, wl.depart_uniform(300, 0.0, 60.0, 72), n_threads=2)
+    run_both(oracle_mod, binding, net, trips, dict(lookahead_cells=128, dt=0.25), 600, dense_until=100)
+
+
 def test_stop_control_limits(binding):
     net = wl.grid_network(nx=3, ny=3, lanes=1, ctrl=2)
     with pytest.raises(binding.MantaError) as e:
         binding.Sim(net, dict(stop_time_s=4.0))            # 8 steps: the counter has three bits
-    assert e.value.code == binding.ERR_INVALID_ARG
+    assert e.value.code == binding.ERR_INVALID_ARG and "stop_time_s" in str(e.value)
+    # the limit belongs to STOP nodes only: a network without them takes any time step with the default 2-s stop time
+    free = wl.grid_network(nx=3, ny=3, lanes=1, ctrl=wl.PRIORITY)
+    for dt in (0.25, 0.1):
+        binding.Sim(free, dict(dt=dt)).close()
+    with pytest.raises(binding.MantaError):
+        binding.Sim(net, dict(dt=0.25))                    # 2 s = 8 steps at a STOP node
     bad = dict(net)
     bad["node_ctrl"] = np.full(9, 3, np.uint8)
     with pytest.raises(binding.MantaError) as e:
@@ -652,6 +666,24 @@ def test_load_state_checkpoint_and_rewind(oracle_mod, binding):
     with pytest.raises(binding.MantaError) as e:
         b.load_state(1200, bad, None)
     assert e.value.code == binding.ERR_INVALID_ARG
+    # speeds the layout cannot hold (Z_out is built on v <= vcap): +inf, NaN, and anything above the fastest possible
+    act = np.nonzero(snap["status"] == ACTIVE)[0]
+    for bad_v in (np.inf, np.nan, 200.0, -1.0):
+        bad = dict(snap)
+        bad["v"] = snap["v"].copy()
+        bad["v"][act[3]] = bad_v
+        with pytest.raises(binding.MantaError) as e:
+            b.load_state(700, bad, None)
+        assert e.value.code == binding.ERR_INVALID_ARG and "speed" in str(e.value), bad_v
+    # steps that contradict the status: an ACTIVE trip that was never admitted, one admitted after t, a DONE trip without arrival
+    done = np.nonzero(snap["status"] == 2)[0]
+    for key, idx, val in (("admit_step", act[0], binding.NONE), ("admit_step", act[1], 701), ("arrive_step", done[0], binding.NONE)):
+        bad = dict(snap)
+        bad[key] = snap[key].copy()
+        bad[key][idx] = val
+        with pytest.raises(binding.MantaError) as e:
+            b.load_state(700, bad, None)
+        assert e.value.code == binding.ERR_INVALID_ARG and "contradict" in str(e.value), (key, val)
     b.step(100)
     o.step(100)
     assert states_equal(o.state(), b.readback()) == []
