@@ -13,9 +13,15 @@ over all active vehicles.  The simulation is first advanced (untimed: initialisa
              replicas -- "replicas only")
   e2e        same metric through the C ABI with HOST buffers: manta_load_trips (H2D of routes and departures) +
              manta_step from 05:00 to the end of the timed window + manta_readback (D2H), wall clock
-  roofline   update-pass kernel (k_update): SURVEY 8(d) useful bytes per launch / its CUDA-event duration, vs the
-             measured HBM peak (frac); the layout's own byte model and the committed ncu traffic beside it
-  cpu_baseline  the oracle (oracle/manta_oracle.c, single thread) on a bounded sample of the same workload
+  e2e        ... always the WHOLE morning (05:00-12:00), whatever --steps is; its stepping is three manta_step calls
+             (to the timed window's start, the 7,200 steps of the peak hour, the rest) so that
+  peak_hour  carries BASELINE.json's "wall-clock for simulated morning peak": device time of those 7,200 steps
+  roofline   the kernel the headline runs in, k_persistent (one launch = the K timed steps): SURVEY 8(d) useful
+             bytes of a whole step x updates / its CUDA-event duration, vs the measured HBM peak (frac); the
+             per-phase figures of k_update (kernel-per-phase mode), the layout's own byte model and the committed ncu
+             traffic of the persistent kernel beside it
+  cpu_baseline  the oracle (oracle/manta_oracle.c, single thread) started from the library's snapshot at the first
+             timed step (Oracle.set_state) and run over the same timesteps, capped at ORACLE_MAX_STEPS
 
 --impl reference times the oracle itself (there is no other reference implementation: the paper ships no code).
 """
@@ -157,11 +163,12 @@ def source_hash():
     return h.hexdigest()[:16]
 
 
-def ncu_traffic(config, start_step):
-    """DRAM bytes k_update moved per vehicle-update (dram__bytes_read.sum + dram__bytes_write.sum of one
-    `ncu --set full` capture, L2 flushed before the launch), from profiles/k_update_traffic.csv -- only a line
+def ncu_traffic(config, start_step, name="k_update_traffic.csv"):
+    """DRAM bytes a kernel moved per vehicle-update (dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` capture), from profiles/<name> -- k_update_traffic.csv: one k_update launch, L2 flushed before
+    it; k_persistent_traffic.csv: one k_persistent launch of 20 timesteps, caches left as they are -- only a line
     captured on THIS build of the sources (source_hash) and this workload window counts; None if there is none."""
-    path = os.path.join(ROOT, "profiles", "k_update_traffic.csv")
+    path = os.path.join(ROOT, "profiles", name)
     if not os.path.exists(path):
         return None
     sh = source_hash()
@@ -216,6 +223,27 @@ def oracle_sample(net, trips, params, start_step, n_sample_trips, n_steps, dt=0.
     s = o.summary()
     o.close()
     return s["vehicle_updates"], wall, len(cand), t_setup
+
+
+ORACLE_MAX_STEPS = 100      # ~229 k active vehicles x 100 steps = 2.3e7 updates: ~20 s of one host core
+
+
+def oracle_at_load(net, trips, params, t, snap, n_steps):
+    """The oracle at the load that is timed: started from the LIBRARY's snapshot at step t (manta_readback ->
+    Oracle.set_state: state transfer, no arithmetic of the method), run over n_steps timesteps on one host core.
+    Returns (vehicle-updates, wall seconds of the steps, set-up seconds)."""
+    from oracle import manta_oracle
+    t0 = time.perf_counter()
+    o = manta_oracle.Oracle(net, params, trips)
+    o.set_state(t, snap, snap["edge_entries"])
+    t_setup = time.perf_counter() - t0
+    u0 = o.summary()["vehicle_updates"]
+    t0 = time.perf_counter()
+    o.step(n_steps)
+    wall = time.perf_counter() - t0
+    upd = o.summary()["vehicle_updates"] - u0
+    o.close()
+    return upd, wall, t_setup
 
 
 def run_reference(args):
@@ -322,6 +350,8 @@ def main():
     sim.set_multi_kernel(bool(args.flags & 2))
     ev[1].record(stream)
     sim.step(W)                                           # warm-up steps
+    want_cpu = not args.no_cpu and rank == 0 and world == 1
+    snap0 = sim.readback() if want_cpu else None          # state at the first timed step: where the oracle starts too
     s0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
     launches0 = sim.launch_count
     clocks = ClockSampler(local)
@@ -373,24 +403,41 @@ def main():
     t_update = ph[1] / Kp * 1e-3
     achieved = c_update * upd_per_launch / t_update / 1e9
     tr = ncu_traffic(args.config, args.start_step)
-    roofline = {"bound": "hbm", "kernel": "k_update", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak,
-                "bytes_model": "SURVEY.md 8(d) useful bytes at the measured hbar, f_lc; k_update = all rows but the "
-                               "lane-change rows (those vehicles are finished by k_second)",
-                "bytes_per_update": c_update, "step_bytes_per_update": c_step,
-                "step_frac": c_step * value / world / 1e9 / peak,
-                "frac_layout": l_update * upd_per_launch / t_update / 1e9 / peak,
-                "bytes_per_update_layout": l_update, "step_bytes_per_update_layout": l_step,
-                "step_frac_layout": l_step * value / world / 1e9 / peak,
-                "traffic": tr["bytes_per_update"] * upd_per_launch if tr else None,
-                "frac_traffic": tr["bytes_per_update"] * upd_per_launch / t_update / 1e9 / peak if tr else None,
-                "traffic_source": ("profiles/k_update_traffic.csv, capture %s on this build (sources %s): %.0f B per "
-                                   "update, L2 flushed before the launch; scaled to this run's updates per launch"
-                                   % (tr["capture"], tr["source_hash"], tr["bytes_per_update"])) if tr else
-                                  "no ncu capture of this build (sources %s) at this window is committed" % source_hash(),
-                "target_frac": 0.5, "peak_source": peak_src,
-                "updates_per_launch": upd_per_launch, "avg_launch_us": t_update * 1e6, "hbar_cells": hbar, "f_lc": flc,
-                "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp}}
+    trp = ncu_traffic(args.config, args.start_step, "k_persistent_traffic.csv")
+    # The dominant kernel of the headline is k_persistent: ONE launch runs the K timed steps (all phases of every
+    # step), so "bytes per launch / launch duration" = step bytes x updates of the timed region / its device time.
+    persist = not (args.flags & 2)
+    n_launch = max(1, launches)
+    step_achieved = c_step * (upd / (ms * 1e-3)) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_persistent" if persist else "k_admit + k_update + k_second",
+                "achieved": step_achieved, "peak": peak, "unit": "GB/s", "frac": step_achieved / peak,
+                "bytes_model": "SURVEY.md 8(d) useful bytes of a WHOLE step at the measured hbar, f_lc.  Note: 2 hbar of "
+                               "them (%.0f of %.0f B) are the survey's 2-byte cells over the look-ahead; this layout "
+                               "reads 1 bit per cell (hbar / 8 B), so frac says how fast the survey's layout would "
+                               "have had to move data to keep up, and frac_layout / frac_traffic say what this one moves"
+                               % (2.0 * hbar, c_step),
+                "bytes_per_update": c_step, "bytes_per_launch": c_step * upd / n_launch,
+                "avg_launch_us": ms * 1e3 / n_launch, "launches": launches, "updates_per_launch": upd / n_launch,
+                "frac_layout": l_step * (upd / (ms * 1e-3)) / 1e9 / peak, "bytes_per_update_layout": l_step,
+                "traffic": trp["bytes_per_update"] * upd / n_launch if trp else None,
+                "frac_traffic": trp["bytes_per_update"] * (upd / (ms * 1e-3)) / 1e9 / peak if trp else None,
+                "traffic_source": ("profiles/k_persistent_traffic.csv, capture %s on this build (sources %s): %.0f B of DRAM "
+                                   "traffic per update (one 20-step launch at this window, caches left warm); scaled to "
+                                   "this run's updates per launch" % (trp["capture"], trp["source_hash"], trp["bytes_per_update"]))
+                                  if trp else "no ncu capture of k_persistent on this build (sources %s) at this window is committed" % source_hash(),
+                "target_frac": 0.5, "peak_source": peak_src, "hbar_cells": hbar, "f_lc": flc,
+                # the update pass alone, timed in kernel-per-phase mode (manta_step_timed) -- a mode the headline does
+                # not run in (its three launches per step cost 1.5 x the persistent kernel's step)
+                "k_update": {"achieved": achieved, "frac": achieved / peak, "bytes_per_update": c_update,
+                             "frac_layout": l_update * upd_per_launch / t_update / 1e9 / peak,
+                             "bytes_per_update_layout": l_update,
+                             "traffic": tr["bytes_per_update"] * upd_per_launch if tr else None,
+                             "frac_traffic": tr["bytes_per_update"] * upd_per_launch / t_update / 1e9 / peak if tr else None,
+                             "traffic_source": ("profiles/k_update_traffic.csv, capture %s (sources %s): %.0f B per update, L2 "
+                                                "flushed before the launch" % (tr["capture"], tr["source_hash"], tr["bytes_per_update"]))
+                                               if tr else "no ncu capture of k_update on this build is committed",
+                             "updates_per_launch": upd_per_launch, "avg_launch_us": t_update * 1e6,
+                             "phase_ms_per_step": {"admit": ph[0] / Kp, "update": ph[1] / Kp, "second": ph[2] / Kp}}}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -407,19 +454,41 @@ def main():
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------------
     if not args.no_e2e:
-        n_e2e = n_total if (args.start_step + W + K) <= n_total and K >= 7200 else args.start_step + W + K
+        # the whole simulated run, whatever --steps is; inside it the peak hour (7,200 steps from --start-step) between
+        # two CUDA events and two summary readbacks (their cost stays inside the end-to-end wall time)
+        n_e2e = max(n_total, args.start_step + 7200)
+        pk = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
         barrier()
         t0 = time.perf_counter()
         sim = binding.Sim(net, params, None, device=local, stream=stream)   # network upload = initialisation
         t1 = time.perf_counter()
         sim.load_trips(trips)                                                 # H2D: routes, departures
         t2 = time.perf_counter()
-        sim.step(n_e2e)
+        sim.step(args.start_step)
+        p0 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+        tp0 = time.perf_counter()
+        pk[0].record(stream)
+        sim.step_async(7200)
+        pk[1].record(stream)
+        sim.sync()
+        tp1 = time.perf_counter()
+        p1 = sim.readback(state=False, edge_entries=False, trips=False)["summary"]
+        sim.step(n_e2e - args.start_step - 7200)
         t3 = time.perf_counter()
         res = sim.readback()                                                  # D2H: state, per-edge counts, trip results
         t4 = time.perf_counter()
         sim.close()
         wall = t4 - t1
+        pk_ms = pk[0].elapsed_time(pk[1])
+        pk_upd = p1["vehicle_updates"] - p0["vehicle_updates"]
+        out["peak_hour"] = {"start_step": args.start_step, "steps": 7200, "simulated_s": 3600.0,
+                            "device_s": pk_ms * 1e-3, "wall_s": tp1 - tp0, "us_per_step": pk_ms * 1e3 / 7200,
+                            "vehicle_updates": pk_upd, "value": pk_upd / (pk_ms * 1e-3), "unit": UNIT,
+                            "sim_hours_per_wall_s": 1.0 / (pk_ms * 1e-3),
+                            "active_vehicles": {"start": p0["n_active"], "end": p1["n_active"]},
+                            "roofline_frac": c_step * pk_upd / (pk_ms * 1e-3) / 1e9 / peak,
+                            "note": "device time (CUDA events on the simulation's stream) of manta_step(7200) inside the "
+                                    "end-to-end run; roofline_frac by the same SURVEY 8(d) step bytes as roofline.frac"}
         h2d = trips["route_ptr"].nbytes + trips["route_edges"].nbytes + trips["depart_time_s"].nbytes
         d2h = n_trips * (1 + 4 + 1 + 1 + 4 + 4 + 4 + 8) + net["n_edges"] * 4
         e_upd = res["summary"]["vehicle_updates"]
@@ -427,18 +496,22 @@ def main():
                       "d2h_bytes_per_step": d2h / n_e2e, "timesteps": n_e2e, "wall_s": wall,
                       "load_trips_s": t2 - t1, "step_s": t3 - t2, "readback_s": t4 - t3, "create_s": t1 - t0,
                       "done_trips": res["summary"]["n_done"], "vehicle_updates": e_upd,
-                      "sim_hours_per_wall_s": n_e2e * 0.5 / 3600.0 / (t3 - t2)}
+                      "sim_hours_per_wall_s": n_e2e * 0.5 / 3600.0 / (t3 - t2),
+                      "what": "manta_load_trips + manta_step over the whole simulated run (three calls, two summary "
+                              "readbacks between them) + manta_readback, host buffers, wall clock"}
     # ---- the oracle beside it (rank 0, N = 1 only) -------------------------------------------------------
-    if not args.no_cpu and rank == 0 and world == 1:
+    if want_cpu:
         from oracle import manta_oracle
         manta_oracle.build()
-        n_s, k_s = ORACLE_SAMPLE_TRIPS, ORACLE_SAMPLE_STEPS
-        c_upd, c_wall, n_tr, _ = oracle_sample(net, trips, params, args.start_step, n_s, k_s)
+        k_s = min(K, ORACLE_MAX_STEPS)
+        c_upd, c_wall, c_setup = oracle_at_load(net, trips, params, args.start_step + W, snap0, k_s)
         model, cores = host_cpu()
         out["cpu_baseline"] = {"value": c_upd / c_wall, "unit": UNIT, "cores": 1, "kind": "oracle",
-                               "cpu_model": model, "host_cores": cores,
-                               "sample": "first %d trips departing from step %d of the same workload, %d timesteps "
-                                         "(%.2e updates in %.1f s)" % (n_tr, args.start_step, k_s, c_upd, c_wall)}
+                               "cpu_model": model, "host_cores": cores, "same_load": True,
+                               "sample": "the same workload at the same load: all %d trips, started from the library's "
+                                         "snapshot at timestep %d (%d active vehicles), the first %d of the %d timed "
+                                         "timesteps (%.2e updates in %.1f s; oracle set-up %.1f s not counted)"
+                                         % (n_trips, args.start_step + W, s0["n_active"], k_s, K, c_upd, c_wall, c_setup)}
     if rank == 0:
         print(json.dumps(out), flush=True)
     if world > 1:

@@ -238,6 +238,14 @@ int manta_readback_atlas(manta_sim *sim, uint16_t *occ, float *spd, uint32_t *ce
  * build has no checks compiled in and returns -1. */
 int manta_check_failures(manta_sim *sim);
 
+/* Self-test of the software grid barrier that separates the phases of a step inside the persistent kernel (tests).
+ * One cooperative launch in the step kernel's geometry (blocks of 512 threads, two per SM) runs n_rounds rounds of:
+ * every block writes the round number to its own 32 words (plain stores), barrier, every block reads all blocks'
+ * words (plain loads), barrier.  *n_stale = words read with another round's value (must be 0), *n_blocks (may be
+ * NULL) = blocks launched.  Uses cudaMalloc / the default stream of `cuda_device`; needs no simulation.  Errors:
+ * INVALID_ARG (NULL, 0 or more than 2^22 rounds), STATE (no cooperative launch), CUDA (time-out, lost arrivals). */
+int manta_selftest_grid_barrier(int cuda_device, uint32_t n_rounds, uint64_t *n_stale, uint32_t *n_blocks);
+
 int manta_set_stream(manta_sim *sim, void *cuda_stream);   /* cudaStream_t; work already enqueued is not moved */
 /* Process-wide: the stream (cudaStream_t, NULL = legacy default stream) that simulations created AFTERWARDS use from
  * manta_create on (its uploads and memsets included).  All work of a simulation and the frees of manta_destroy

@@ -28,7 +28,8 @@ EXPORTS = ("manta_set_allocator", "manta_create", "manta_load_trips", "manta_ste
            "manta_readback", "manta_readback_noalloc", "manta_load_state", "manta_readback_edge_speeds", "manta_atlas_cells", "manta_readback_atlas", "manta_set_stream", "manta_set_default_stream",
            "manta_set_multi_kernel",
            "manta_launch_count",
-           "manta_device_bytes", "manta_destroy", "manta_last_error", "manta_check_failures")
+           "manta_device_bytes", "manta_destroy", "manta_last_error", "manta_check_failures",
+           "manta_selftest_grid_barrier")
 
 
 class MantaError(RuntimeError):
@@ -110,6 +111,7 @@ def load_library():
     L.manta_destroy.argtypes = [C.c_void_p]
     L.manta_destroy.restype = None
     L.manta_check_failures.argtypes = [C.c_void_p]
+    L.manta_selftest_grid_barrier.argtypes = [C.c_int, C.c_uint32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32)]
     L.manta_last_error.argtypes = [C.c_void_p]
     L.manta_last_error.restype = C.c_char_p
     _lib = L
@@ -144,6 +146,15 @@ def use_torch_allocator():
 
 def _ptr(a):
     return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def selftest_grid_barrier(n_rounds, device=0):
+    """manta_selftest_grid_barrier: (words read stale, blocks launched)"""
+    stale, blocks = C.c_uint64(0), C.c_uint32(0)
+    rc = load_library().manta_selftest_grid_barrier(int(device), int(n_rounds), C.byref(stale), C.byref(blocks))
+    if rc != OK:
+        raise MantaError(rc, load_library().manta_last_error(None).decode())
+    return int(stale.value), int(blocks.value)
 
 
 def step_batch(sims, n=1):

@@ -63,7 +63,7 @@ LIB_FAST = os.path.join(_HERE, "libmanta_fast.so")
 
 def build_fast(force=False):
     """Fast mode: the same sources with FMA contraction allowed (-fmad=true).  Not bit-exact against
-    the oracle: held to a per-step tolerance instead (tests/test_gpu_parity.py::test_fast_mode_one_step)."""
+    the oracle: held to a per-step tolerance instead (tests/test_gpu_parity.py::test_fast_variant_one_step_and_aggregates, run by test_fast_mode)."""
     if (not force and os.path.exists(LIB_FAST)
             and os.path.getmtime(LIB_FAST) >= max(os.path.getmtime(d) for d in DEPS)):
         return LIB_FAST

@@ -1333,6 +1333,52 @@ int manta_readback_atlas(manta_sim *s, uint16_t *occ, float *spd, uint32_t *cell
 }
 
 
+int manta_selftest_grid_barrier(int cuda_device, uint32_t n_rounds, uint64_t *n_stale, uint32_t *n_blocks)
+{
+    if (!n_stale || n_rounds == 0 || n_rounds > (1u << 22)) return fail(nullptr, MANTA_ERR_INVALID_ARG, "manta_selftest_grid_barrier: null result or 0 / more than 2^22 rounds");
+    int n_dev = 0, sms = 0, coop = 0, occ = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device < 0 || cuda_device >= n_dev) {
+        cudaGetLastError();
+        return fail(nullptr, MANTA_ERR_CUDA, "no CUDA device %d (there is no CPU fallback)", cuda_device);
+    }
+    CUDA_TRY((manta_sim *)nullptr, cudaSetDevice(cuda_device));
+    CUDA_TRY((manta_sim *)nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device));
+    CUDA_TRY((manta_sim *)nullptr, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, cuda_device));
+    CUDA_TRY((manta_sim *)nullptr, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_barrier_litmus, MANTA_NT, 0));
+    if (!coop || occ < 1) return fail(nullptr, MANTA_ERR_STATE, "cooperative launches are not available on device %d", cuda_device);
+    const int grid = sms * std::min(occ, MANTA_MINB);   // the persistent step kernel's geometry: MANTA_MINB blocks of MANTA_NT threads per SM
+    uint8_t *buf = nullptr;
+    const size_t words_off = sizeof(Counters), stale_off = words_off + (size_t)grid * 32 * 4, total = stale_off + 8;
+    CUDA_TRY((manta_sim *)nullptr, cudaMalloc(&buf, total));
+    int rc = MANTA_OK;
+    cudaError_t e = cudaMemset(buf, 0, total);
+    if (e == cudaSuccess) {
+        Counters *c = (Counters *)buf;
+        uint32_t *words = (uint32_t *)(buf + words_off);
+        unsigned long long *stale = (unsigned long long *)(buf + stale_off);
+        void *args[] = {&c, &words, &n_rounds, &stale};
+        e = cudaLaunchCooperativeKernel((const void *)k_barrier_litmus, dim3((unsigned)grid), dim3(MANTA_NT), args, 0, 0);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        unsigned long long h_stale = 0;
+        unsigned int h_abort = 0, h_count = 0;
+        if (e == cudaSuccess) e = cudaMemcpy(&h_stale, stale, 8, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(&h_abort, &c->abort, 4, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(&h_count, &c->bar_count, 4, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) {
+            *n_stale = h_stale;
+            if (n_blocks) *n_blocks = (uint32_t)grid;
+            if (h_abort) rc = fail(nullptr, MANTA_ERR_CUDA, "grid barrier timed out in the self-test");
+#if MANTA_BAR >= 1
+            else if (h_count != 2u * n_rounds * (unsigned)grid)   // every block arrived at every barrier
+                rc = fail(nullptr, MANTA_ERR_CUDA, "grid barrier self-test: %u arrivals counted, %u expected", h_count, 2u * n_rounds * (unsigned)grid);
+#endif
+        }
+    }
+    if (e != cudaSuccess) rc = fail(nullptr, MANTA_ERR_CUDA, "grid barrier self-test: %s", cudaGetErrorString(e));
+    cudaFree(buf);
+    return rc;
+}
+
 // ---- manta_readback_noalloc: manta_readback without any device allocation ------------------------------------------
 namespace {
 constexpr int kNoallocMaxDevices = 64;

@@ -1388,6 +1388,24 @@ __device__ __forceinline__ bool grid_barrier(Counters *c, unsigned &gen, uint32_
     return *s_flag == 0u;
 }
 
+// Litmus test of grid_barrier (manta_selftest_grid_barrier): in every round each block writes the round number into
+// its own 32 words with PLAIN stores, passes the barrier, and every block reads ALL blocks' words with PLAIN loads --
+// the very pattern the step phases rely on (writes before the arrival are visible after the departure, through each
+// SM's L1) -- then a second barrier keeps the next round's writes behind everybody's reads.  Counts stale words.
+__global__ void __launch_bounds__(MANTA_NT, MANTA_MINB) k_barrier_litmus(Counters *c, uint32_t *words, uint32_t n_rounds, unsigned long long *n_stale)
+{
+    __shared__ uint32_t flag;
+    unsigned gen = 0u;
+    unsigned long long bad = 0ull;
+    for (uint32_t r = 1u; r <= n_rounds; r++) {
+        for (uint32_t k = threadIdx.x; k < 32u; k += blockDim.x) words[blockIdx.x * 32u + k] = r;
+        if (!grid_barrier(c, gen, &flag)) return;
+        for (uint32_t k = threadIdx.x; k < gridDim.x * 32u; k += blockDim.x) bad += words[k] != r ? 1ull : 0ull;
+        if (!grid_barrier(c, gen, &flag)) return;
+    }
+    if (bad) atomicAdd(n_stale, bad);
+}
+
 __device__ __forceinline__ bool sort_all(const DevP &P, UpdateSmem &sm, int from, unsigned &gen, Counters *ctr)
 {
     uint32_t n_live, per_seg;

@@ -813,6 +813,16 @@ def test_idle_and_tiny_inputs(oracle_mod, binding):
 
 # ---------------------------------------------------------------------------------------------------------
 # replica batching -- several parameter sets advanced in one cooperative launch
+def test_grid_barrier_litmus(binding):
+    """The software grid barrier of the persistent kernel (release reduction, relaxed polling, one acquire load): 100,000
+    rounds = 200,000 barriers over the step kernel's 296 blocks; after each one every block must read every other
+    block's plain stores of that round through plain loads.  No stale word, no lost arrival, no time-out."""
+    stale, blocks = binding.selftest_grid_barrier(100_000)
+    assert blocks >= 148 and stale == 0, (stale, blocks)
+    with pytest.raises(binding.MantaError):
+        binding.selftest_grid_barrier(0)
+
+
 @pytest.mark.parametrize("n_rep", [2, 3, 4])
 def test_replica_batching_bit_exact(oracle_mod, binding, n_rep):
     """n_rep simulations of one network and demand with different IDM parameters and seeds (a calibration sweep,
