@@ -172,7 +172,11 @@ int manta_sync(manta_sim *sim);
  * replicas between the same two grid barriers, so the per-step synchronisation is paid once for the batch.  Results
  * of every replica are exactly those of stepping it alone.  All simulations must be on the same device and stream, at
  * the same step counter, with the same launch geometry (n_sims = 1: plain manta_step).  Errors: INVALID_ARG, STATE
- * (the batch does not fit the device's shared memory), CUDA.  Returns after the steps completed. */
+ * (the batch does not fit the device's shared memory), CUDA.  Returns after the steps completed.
+ * MEASURED (profiles/r02_final.md, B200, configs[2] at 07:30): as built this is SLOWER than stepping the replicas in
+ * separate manta_step calls -- 31.4 us per replica-step with 2 replicas, 40 us with 4, against 26.7 us alone --
+ * because each block walks its replicas one after the other inside a phase.  Use it for its exactness guarantee
+ * (one launch, identical results), not for throughput; for a parameter sweep call manta_step per replica. */
 int manta_step_batch(manta_sim **sims, uint32_t n_sims, uint32_t n_steps);
 
 /* Same as manta_step, with CUDA events recorded on the simulation's stream around every phase; adds the device
