@@ -481,14 +481,23 @@ def main():
         wall = t4 - t1
         pk_ms = pk[0].elapsed_time(pk[1])
         pk_upd = p1["vehicle_updates"] - p0["vehicle_updates"]
+        # the step bytes of the HOUR: SURVEY 8(d) at the hour's own mean look-ahead and lane-change fraction (denser
+        # traffic finds its leaders sooner: fewer contract bytes per update than in the first seconds of the hour)
+        pk_hbar = (p1["cells_examined"] - p0["cells_examined"]) / max(1, pk_upd)
+        pk_flc = (p1["lc_evals"] - p0["lc_evals"]) / max(1, pk_upd)
+        pk_c_step = contract_bytes(pk_hbar, pk_flc)[1]
+        pk_l_step = layout_bytes(pk_hbar, pk_flc, params.get("lookback_cells", 64))[1]
         out["peak_hour"] = {"start_step": args.start_step, "steps": 7200, "simulated_s": 3600.0,
                             "device_s": pk_ms * 1e-3, "wall_s": tp1 - tp0, "us_per_step": pk_ms * 1e3 / 7200,
                             "vehicle_updates": pk_upd, "value": pk_upd / (pk_ms * 1e-3), "unit": UNIT,
                             "sim_hours_per_wall_s": 1.0 / (pk_ms * 1e-3),
                             "active_vehicles": {"start": p0["n_active"], "end": p1["n_active"]},
-                            "roofline_frac": c_step * pk_upd / (pk_ms * 1e-3) / 1e9 / peak,
+                            "hbar_cells": pk_hbar, "f_lc": pk_flc, "bytes_per_update": pk_c_step,
+                            "roofline_frac": pk_c_step * pk_upd / (pk_ms * 1e-3) / 1e9 / peak,
+                            "roofline_frac_layout": pk_l_step * pk_upd / (pk_ms * 1e-3) / 1e9 / peak,
                             "note": "device time (CUDA events on the simulation's stream) of manta_step(7200) inside the "
-                                    "end-to-end run; roofline_frac by the same SURVEY 8(d) step bytes as roofline.frac"}
+                                    "end-to-end run; roofline_frac = SURVEY 8(d) step bytes at THIS hour's hbar and f_lc "
+                                    "x updates / device time / peak (the formula of roofline.frac)"}
         h2d = trips["route_ptr"].nbytes + trips["route_edges"].nbytes + trips["depart_time_s"].nbytes
         d2h = n_trips * (1 + 4 + 1 + 1 + 4 + 4 + 4 + 8) + net["n_edges"] * 4
         e_upd = res["summary"]["vehicle_updates"]
